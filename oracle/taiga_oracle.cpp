@@ -1,0 +1,428 @@
+/* TEST INFRASTRUCTURE -- NOT PRODUCT CODE.  See taiga_oracle.h for scope, pins and build.
+ *
+ * Every function follows the passage it cites, step by step, in the paper's order and
+ * notation; no blocking, fusion or reordering.  Scalar fp64, compiled with
+ * -ffp-contract=off so that fma appears only where std::fma is written (O2.2).
+ */
+#include "taiga_oracle.h"
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* ------------------------------------------------------------------------------------ */
+/* O2.1  Philox4x32-10 (Salmon et al. 2011), the counter-based generator SURVEY.md 8(c)
+ * O2 fixes for the paper's "stochastic initialisation".                 */
+extern "C" void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        if (round > 0) { k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+        uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        uint32_t n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        uint32_t n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* O2.1  counter=(i_lo,i_hi,j,0), j=0,1,2 -> 12 words; U_k=((w_2k>>6)*2^26+(w_2k+1>>6)+0.5)*2^-52 */
+extern "C" void orc_uniforms(uint64_t seed, uint64_t index, double U[5]) {
+    uint32_t w[12];
+    uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    for (uint32_t j = 0; j < 3; ++j) {
+        uint32_t ctr[4] = {(uint32_t)index, (uint32_t)(index >> 32), j, 0u};
+        orc_philox4x32_10(ctr, key, w + 4 * j);
+    }
+    for (int k = 0; k < 5; ++k) {
+        uint64_t n = ((uint64_t)(w[2 * k] >> 6) << 26) + (uint64_t)(w[2 * k + 1] >> 6);
+        U[k] = ((double)n + 0.5) * 0x1p-52;            /* n+0.5 needs 53 bits: exact */
+    }
+}
+
+/* O2.2  find j with F_j <= U < F_{j+1} (upper-bound binary search), linear interpolation. */
+extern "C" double orc_cdf_invert(const double* F, int K, double x_max, double U) {
+    int lo = 0, hi = K;                       /* invariant: F[lo] <= U < F[hi] (F_0=0,F_K=1) */
+    while (hi - lo > 1) {
+        int mid = (lo + hi) / 2;
+        if (F[mid] <= U) lo = mid; else hi = mid;
+    }
+    double dx = x_max / (double)K;
+    double t = (U - F[lo]) / (F[lo + 1] - F[lo]);
+    return std::fma(t, dx, (double)lo * dx);
+}
+
+/* O2.3-4  PAPER.md L314 (profile used as CDF, random sampling), L128-134 (linear beam). */
+extern "C" void orc_seed(const orc_beam* b, uint64_t seed, uint64_t first_index, uint64_t n,
+                         double* x, double* y, double* z, double* vx, double* vy, double* vz) {
+    for (uint64_t j = 0; j < n; ++j) {
+        double U[5];
+        orc_uniforms(seed, first_index + j, U);
+        double d  = orc_cdf_invert(b->cdf_depth, b->n_depth, b->depth_max, U[0]);
+        double z1 = orc_cdf_invert(b->cdf_normal, b->n_normal, 2.0 * b->z_max, U[1]) - b->z_max;
+        double z2 = orc_cdf_invert(b->cdf_normal, b->n_normal, 2.0 * b->z_max, U[2]) - b->z_max;
+        double z3 = orc_cdf_invert(b->cdf_normal, b->n_normal, 2.0 * b->z_max, U[3]) - b->z_max;
+        double z4 = orc_cdf_invert(b->cdf_normal, b->n_normal, 2.0 * b->z_max, U[4]) - b->z_max;
+        double r[3], v[3];
+        for (int c = 0; c < 3; ++c)
+            r[c] = (b->origin[c] + d * b->axis[c]) + b->sigma_pos * (z1 * b->eT[c] + z2 * b->eZ[c]);
+        if (b->sigma_ang == 0.0) {
+            for (int c = 0; c < 3; ++c) v[c] = b->v0 * b->axis[c];
+        } else {
+            double thT = b->sigma_ang * z3, thZ = b->sigma_ang * z4;
+            double nrm = std::sqrt((1.0 + thT * thT) + thZ * thZ);
+            for (int c = 0; c < 3; ++c)
+                v[c] = (b->v0 * ((b->axis[c] + thT * b->eT[c]) + thZ * b->eZ[c])) / nrm;
+        }
+        x[j] = r[0]; y[j] = r[1]; z[j] = r[2];
+        vx[j] = v[0]; vy[j] = v[1]; vz[j] = v[2];
+    }
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* O1  dense Gaussian elimination with partial pivoting, m right-hand sides (columns of B) */
+static int solve_dense(int n, std::vector<double>& A, int m, double* B /*[n][m]*/) {
+    for (int col = 0; col < n; ++col) {
+        int piv = col;
+        for (int r = col + 1; r < n; ++r)
+            if (std::fabs(A[(size_t)r * n + col]) > std::fabs(A[(size_t)piv * n + col])) piv = r;
+        if (A[(size_t)piv * n + col] == 0.0) return -1;
+        if (piv != col) {
+            for (int c = 0; c < n; ++c) std::swap(A[(size_t)piv * n + c], A[(size_t)col * n + c]);
+            for (int c = 0; c < m; ++c) std::swap(B[(size_t)piv * m + c], B[(size_t)col * m + c]);
+        }
+        for (int r = col + 1; r < n; ++r) {
+            double f = A[(size_t)r * n + col] / A[(size_t)col * n + col];
+            if (f == 0.0) continue;
+            for (int c = col; c < n; ++c) A[(size_t)r * n + c] -= f * A[(size_t)col * n + c];
+            for (int c = 0; c < m; ++c) B[(size_t)r * m + c] -= f * B[(size_t)col * m + c];
+        }
+    }
+    for (int r = n - 1; r >= 0; --r) {
+        for (int c = 0; c < m; ++c) {
+            double s = B[(size_t)r * m + c];
+            for (int k = r + 1; k < n; ++k) s -= A[(size_t)r * n + k] * B[(size_t)k * m + c];
+            B[(size_t)r * m + c] = s / A[(size_t)r * n + r];
+        }
+    }
+    return 0;
+}
+
+/* O1  family of m 1-D interpolating cubic splines through Y[node][col] on a unit grid.
+ * Unknowns: second derivatives M_i.  C2 continuity: M_{i-1}+4M_i+M_{i+1}=6(y_{i-1}-2y_i+y_{i+1}).
+ * not-a-knot (A4): third derivative continuous at nodes 1 and n-2:
+ *     M_0-2M_1+M_2=0,  M_{n-3}-2M_{n-2}+M_{n-1}=0.
+ * periodic (kind 2, phi): indices cyclic, n unknowns, n intervals.
+ * Output C[interval][col][0..3]: S = c0 + c1 p + c2 p^2 + c3 p^3 on the interval.        */
+static int spline_family(bool periodic, int n, int m, const double* Y, double* C) {
+    if ((!periodic && n < 4) || (periodic && n < 3)) return -1;
+    std::vector<double> A((size_t)n * n, 0.0), M((size_t)n * m, 0.0);
+    auto y = [&](int i, int c) { return Y[(size_t)(((i % n) + n) % n) * m + c]; };
+    for (int i = 0; i < n; ++i) {
+        bool interior = periodic || (i > 0 && i < n - 1);
+        if (interior) {
+            int im = periodic ? (i + n - 1) % n : i - 1, ip = periodic ? (i + 1) % n : i + 1;
+            A[(size_t)i * n + im] += 1.0; A[(size_t)i * n + i] += 4.0; A[(size_t)i * n + ip] += 1.0;
+            for (int c = 0; c < m; ++c)
+                M[(size_t)i * m + c] = 6.0 * ((y(i - 1, c) - 2.0 * y(i, c)) + y(i + 1, c));
+        } else if (i == 0) {
+            A[0] = 1.0; A[1] = -2.0; A[2] = 1.0;
+        } else {
+            A[(size_t)i * n + n - 3] = 1.0; A[(size_t)i * n + n - 2] = -2.0; A[(size_t)i * n + n - 1] = 1.0;
+        }
+    }
+    if (solve_dense(n, A, m, M.data()) != 0) return -2;
+    int nint = periodic ? n : n - 1;
+    for (int i = 0; i < nint; ++i) {
+        int ip = periodic ? (i + 1) % n : i + 1;
+        for (int c = 0; c < m; ++c) {
+            double y0 = Y[(size_t)i * m + c], y1 = Y[(size_t)ip * m + c];
+            double M0 = M[(size_t)i * m + c], M1 = M[(size_t)ip * m + c];
+            double* o = C + ((size_t)i * m + c) * 4;
+            o[0] = y0;
+            o[1] = (y1 - y0) - (2.0 * M0 + M1) / 6.0;
+            o[2] = M0 / 2.0;
+            o[3] = (M1 - M0) / 6.0;
+        }
+    }
+    return 0;
+}
+
+extern "C" int orc_spline_notaknot(int n, const double* y, double* c) { return spline_family(false, n, 1, y, c); }
+extern "C" int orc_spline_periodic(int n, const double* y, double* c) { return spline_family(true, n, 1, y, c); }
+
+/* O1  tensor product (bicubic spline fitted to the grid points, coefficients
+ * extracted and stored): spline along Z for every R-node, then spline each of the four
+ * w-coefficients along R; kind 2: then a periodic spline along phi of each of the 16.     */
+extern "C" int orc_build_tables(int kind, int nR, int nZ, int nS, const double* nodal, double* coef) {
+    const int cR = nR - 1, cZ = nZ - 1;
+    std::vector<double> bic((size_t)nS * cR * cZ * 16);
+    std::vector<double> yz((size_t)nZ * nR), cz((size_t)cZ * nR * 4);
+    std::vector<double> yr((size_t)nR * cZ * 4), cr((size_t)cR * cZ * 4 * 4);
+    for (int k = 0; k < nS; ++k) {
+        const double* g = nodal + (size_t)k * nR * nZ;
+        /* along Z: nodes j, columns i */
+        for (int j = 0; j < nZ; ++j) for (int i = 0; i < nR; ++i) yz[(size_t)j * nR + i] = g[(size_t)i * nZ + j];
+        if (spline_family(false, nZ, nR, yz.data(), cz.data())) return -1;   /* cz[j][i][b] */
+        /* along R: nodes i, columns (j,b) */
+        for (int i = 0; i < nR; ++i) for (int j = 0; j < cZ; ++j) for (int b = 0; b < 4; ++b)
+            yr[((size_t)i * cZ + j) * 4 + b] = cz[((size_t)j * nR + i) * 4 + b];
+        if (spline_family(false, nR, cZ * 4, yr.data(), cr.data())) return -1; /* cr[i][j][b][a] */
+        for (int i = 0; i < cR; ++i) for (int j = 0; j < cZ; ++j) for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b)
+            bic[((((size_t)k * cR + i) * cZ + j) * 4 + a) * 4 + b] = cr[((((size_t)i * cZ + j) * 4 + b) * 4) + a];
+    }
+    if (kind != ORC_F_RZPHI) { std::memcpy(coef, bic.data(), bic.size() * sizeof(double)); return 0; }
+    /* along phi, periodic: nodes k, columns (i,j,a,b) */
+    const size_t m = (size_t)cR * cZ * 16;
+    std::vector<double> cp((size_t)nS * m * 4);
+    if (spline_family(true, nS, (int)m, bic.data(), cp.data())) return -1;   /* cp[k][col][c] */
+    for (int k = 0; k < nS; ++k) for (size_t cell = 0; cell < (size_t)cR * cZ; ++cell)
+        for (int c = 0; c < 4; ++c) for (int ab = 0; ab < 16; ++ab)
+            coef[(((size_t)k * cR * cZ + cell) * 4 + c) * 16 + ab] = cp[(((size_t)k * m) + cell * 16 + ab) * 4 + c];
+    return 0;
+}
+
+/* O1  evaluation: B(R,Z)=sum_ab c_ab p^a w^b, p=(R-R_i)/h_R, w=(Z-Z_j)/h_Z,
+ * i=clamp(floor((R-R_min)/h_R),0,nR-2) (outside the grid the boundary cell extrapolates). */
+static inline int cell_index(double x, double xmin, double h, int n, double* frac) {
+    int i = (int)std::floor((x - xmin) / h);
+    if (i < 0) i = 0;
+    if (i > n - 2) i = n - 2;
+    *frac = (x - (xmin + (double)i * h)) / h;
+    return i;
+}
+static inline double bicubic(const double* c, double p, double w) {
+    double s = 0.0;
+    for (int a = 3; a >= 0; --a) {
+        double row = ((c[a * 4 + 3] * w + c[a * 4 + 2]) * w + c[a * 4 + 1]) * w + c[a * 4 + 0];
+        s = s * p + row;
+    }
+    return s;
+}
+
+extern "C" void orc_field_cyl(const orc_field* f, double R, double Z, double s, double Bc[3]) {
+    const int cR = f->nR - 1, cZ = f->nZ - 1;
+    double hR = (f->Rmax - f->Rmin) / (double)cR, hZ = (f->Zmax - f->Zmin) / (double)cZ;
+    double p, w;
+    int i = cell_index(R, f->Rmin, hR, f->nR, &p);
+    int j = cell_index(Z, f->Zmin, hZ, f->nZ, &w);
+    size_t cell = (size_t)i * cZ + j;
+    if (f->kind == ORC_F_RZ) {
+        for (int c = 0; c < 3; ++c) Bc[c] = bicubic(f->coef[c] + cell * 16, p, w);
+    } else if (f->kind == ORC_F_RZT) {
+        /* B(t)=(1-tau)B_k+tau B_{k+1}, k=clamp(floor((t-s0)/ds),0,nS-2), tau=clamp(.,0,1): held
+         * outside the slice range (A16).                                                  */
+        double xs = (s - f->s0) / f->ds;
+        int k = (int)std::floor(xs);
+        if (k < 0) k = 0;
+        if (k > f->nS - 2) k = f->nS - 2;
+        double tau = xs - (double)k;
+        if (tau < 0.0) tau = 0.0;
+        if (tau > 1.0) tau = 1.0;
+        size_t stride = (size_t)cR * cZ * 16;
+        for (int c = 0; c < 3; ++c) {
+            double b0 = bicubic(f->coef[c] + k * stride + cell * 16, p, w);
+            double b1 = bicubic(f->coef[c] + (k + 1) * stride + cell * 16, p, w);
+            Bc[c] = (1.0 - tau) * b0 + tau * b1;
+        }
+    } else { /* ORC_F_RZPHI: periodic tricubic, 64 coefficients per cell; s = phi (A17) */
+        double xs = (s - f->s0) / f->ds;
+        xs = xs - (double)f->nS * std::floor(xs / (double)f->nS);      /* into [0,nS) */
+        int k = (int)std::floor(xs);
+        if (k < 0) k = 0;
+        if (k > f->nS - 1) k = f->nS - 1;
+        double q = xs - (double)k;
+        size_t base = ((size_t)k * cR * cZ + cell) * 64;
+        for (int c = 0; c < 3; ++c) {
+            const double* d = f->coef[c] + base;
+            double acc = 0.0;
+            for (int e = 3; e >= 0; --e) acc = acc * q + bicubic(d + e * 16, p, w);
+            Bc[c] = acc;
+        }
+    }
+}
+
+/* O0  Cartesian <-> poloidal plane: R=sqrt(X^2+Y^2), c=X/R, s=Y/R,
+ * B_X=B_R c-B_phi s, B_Y=B_R s+B_phi c.                                                   */
+extern "C" void orc_field_B(const orc_field* f, const double r[3], double t, double B[3]) {
+    switch (f->kind) {
+    case ORC_F_UNIFORM: B[0] = f->par[0]; B[1] = f->par[1]; B[2] = f->par[2]; return;
+    case ORC_F_GRADB:   B[0] = 0.0; B[1] = 0.0; B[2] = f->par[0] * (1.0 + f->par[1] * r[0]); return;
+    case ORC_F_INVR:    B[0] = 0.0; B[1] = 0.0; B[2] = f->par[0] / std::sqrt(r[0] * r[0] + r[1] * r[1]); return;
+    default: break;
+    }
+    double R = std::sqrt(r[0] * r[0] + r[1] * r[1]);
+    double c = r[0] / R, s = r[1] / R;
+    double Bc[3];
+    if (f->kind == ORC_F_SOLOVEV) {
+        double psa = f->par[0], R0 = f->par[1], a = f->par[2], kap = f->par[3], BT = f->par[4];
+        double Z = r[2];
+        Bc[0] = -2.0 * psa * R * Z / ((R0 * kap * a) * (R0 * kap * a));
+        Bc[1] = psa * ((R * R - R0 * R0) / ((R0 * a) * (R0 * a)) + 2.0 * Z * Z / ((R0 * kap * a) * (R0 * kap * a)));
+        Bc[2] = -BT * R0 / R;
+    } else {
+        double sarg = (f->kind == ORC_F_RZPHI) ? std::atan2(r[1], r[0]) : t;
+        orc_field_cyl(f, R, r[2], sarg, Bc);
+    }
+    B[0] = Bc[0] * c - Bc[2] * s;
+    B[1] = Bc[0] * s + Bc[2] * c;
+    B[2] = Bc[1];
+}
+
+/* Eq. 3: a = (q/m)(E + v x B) */
+static inline void accel(const orc_field* f, double qm, const double r[3], const double v[3], double t, double a[3]) {
+    double B[3];
+    orc_field_B(f, r, t, B);
+    a[0] = qm * (f->E[0] + (v[1] * B[2] - v[2] * B[1]));
+    a[1] = qm * (f->E[1] + (v[2] * B[0] - v[0] * B[2]));
+    a[2] = qm * (f->E[2] + (v[0] * B[1] - v[1] * B[0]));
+}
+
+/* O3  one Runge-Kutta-Nystrom step, Eq. 5-6 under readings A1-A3:
+ *  k1=a(r,v,t); k2=a(r+v dt/2+k1 dt^2/8, v+k1 dt/2, t+dt/2);
+ *  k3=a(r+v dt/2+K dt^2/8, v+k2 dt/2, t+dt/2), K=k1 (classical, variant 0) or k2 (printed, 1);
+ *  k4=a(r+v dt+k3 dt^2/2, v+k3 dt, t+dt);
+ *  r'=r+v dt+(k1+k2+k3) dt^2/6;  v'=v+(k1+2k2+2k3+k4) dt/6.                               */
+static inline void rkn_step(const orc_field* f, double qm, int variant, const double r[3], const double v[3],
+                            double t, double dt, double rn[3], double vn[3]) {
+    double k1[3], k2[3], k3[3], k4[3], rs[3], vs[3];
+    accel(f, qm, r, v, t, k1);
+    for (int c = 0; c < 3; ++c) { rs[c] = r[c] + v[c] * (dt / 2.0) + k1[c] * (dt * dt / 8.0); vs[c] = v[c] + k1[c] * (dt / 2.0); }
+    accel(f, qm, rs, vs, t + dt / 2.0, k2);
+    const double* K = variant ? k2 : k1;
+    for (int c = 0; c < 3; ++c) { rs[c] = r[c] + v[c] * (dt / 2.0) + K[c] * (dt * dt / 8.0); vs[c] = v[c] + k2[c] * (dt / 2.0); }
+    accel(f, qm, rs, vs, t + dt / 2.0, k3);
+    for (int c = 0; c < 3; ++c) { rs[c] = r[c] + v[c] * dt + k3[c] * (dt * dt / 2.0); vs[c] = v[c] + k3[c] * dt; }
+    accel(f, qm, rs, vs, t + dt, k4);
+    for (int c = 0; c < 3; ++c) {
+        rn[c] = r[c] + v[c] * dt + (k1[c] + k2[c] + k3[c]) * (dt * dt / 6.0);
+        vn[c] = v[c] + (k1[c] + 2.0 * k2[c] + 2.0 * k3[c] + k4[c]) * (dt / 6.0);
+    }
+}
+
+extern "C" void orc_rkn_advance(const orc_field* f, double qm, int variant, double r[3], double v[3],
+                                double* t, double dt, uint64_t nsteps) {
+    for (uint64_t s = 0; s < nsteps; ++s) {
+        double rn[3], vn[3];
+        rkn_step(f, qm, variant, r, v, *t, dt, rn, vn);
+        for (int c = 0; c < 3; ++c) { r[c] = rn[c]; v[c] = vn[c]; }
+        *t = *t + dt;
+    }
+}
+
+static const double GRAZE = 1e-9;   /* grazing thresholds, fp64 */
+
+static inline bool in_grid(const orc_field* f, const double r[3], bool* graze) {
+    if (f->kind >= 10) return true;                       /* analytic test fields: no grid */
+    double R = std::sqrt(r[0] * r[0] + r[1] * r[1]), Z = r[2];
+    if (std::fabs(R - f->Rmin) < GRAZE || std::fabs(R - f->Rmax) < GRAZE ||
+        std::fabs(Z - f->Zmin) < GRAZE || std::fabs(Z - f->Zmax) < GRAZE) *graze = true;
+    return !(R < f->Rmin || R > f->Rmax || Z < f->Zmin || Z > f->Zmax);
+}
+
+/* O4  PAPER.md L326 ("stops when a particle passes through the detector plane or reaches the
+ * maximum number of iterations ... an interpolation is applied to the detector plane using
+ * coordinates from the previous iteration step"), L318 (error value), L338 (two-state
+ * storage, linear interpolation), L330 (coordinate transformation to the plane).          */
+extern "C" void orc_trace(const orc_field* f, double qm, int variant, uint64_t n,
+                          const double* x, const double* y, const double* z,
+                          const double* vx, const double* vy, const double* vz, const double* t0,
+                          double dt, uint32_t max_steps, const orc_detector* det,
+                          int32_t* status, double* hit_u, double* hit_w, double* hit_xyz,
+                          uint32_t* steps, uint8_t* flags, int nthreads) {
+#ifdef _OPENMP
+    if (nthreads <= 0) nthreads = omp_get_max_threads();
+#pragma omp parallel for schedule(dynamic, 16) num_threads(nthreads)
+#endif
+    for (int64_t ii = 0; ii < (int64_t)n; ++ii) {
+        uint64_t i = (uint64_t)ii;
+        double r[3] = {x[i], y[i], z[i]}, v[3] = {vx[i], vy[i], vz[i]};
+        double t = t0 ? t0[i] : 0.0;
+        uint8_t fl = 0;
+        bool gz = false;
+        double s0 = det->normal[0] * (r[0] - det->origin[0]) + det->normal[1] * (r[1] - det->origin[1]) +
+                    det->normal[2] * (r[2] - det->origin[2]);
+        hit_u[i] = 0.0; hit_w[i] = 0.0;
+        if (hit_xyz) hit_xyz[3 * i] = hit_xyz[3 * i + 1] = hit_xyz[3 * i + 2] = 0.0;
+        if (std::fabs(s0) < GRAZE) fl |= 2;
+        bool inside = in_grid(f, r, &gz);
+        if (gz) fl |= 4;
+        if (!(s0 < 0.0) || !inside) { status[i] = -4; steps[i] = 0; flags[i] = fl; continue; }
+        int32_t st = -2;
+        uint32_t nst = max_steps;
+        for (uint32_t step = 1; step <= max_steps; ++step) {
+            double rn[3], vn[3];
+            rkn_step(f, qm, variant, r, v, t, dt, rn, vn);
+            double s1 = det->normal[0] * (rn[0] - det->origin[0]) + det->normal[1] * (rn[1] - det->origin[1]) +
+                        det->normal[2] * (rn[2] - det->origin[2]);
+            if (std::fabs(s1) < GRAZE) fl |= 2;
+            if (s0 < 0.0 && s1 >= 0.0) {
+                double lam = s0 / (s0 - s1);
+                double p[3];
+                for (int c = 0; c < 3; ++c) p[c] = r[c] + lam * (rn[c] - r[c]);
+                hit_u[i] = (p[0] - det->origin[0]) * det->eu[0] + (p[1] - det->origin[1]) * det->eu[1] + (p[2] - det->origin[2]) * det->eu[2];
+                hit_w[i] = (p[0] - det->origin[0]) * det->ew[0] + (p[1] - det->origin[1]) * det->ew[1] + (p[2] - det->origin[2]) * det->ew[2];
+                if (hit_xyz) { hit_xyz[3 * i] = p[0]; hit_xyz[3 * i + 1] = p[1]; hit_xyz[3 * i + 2] = p[2]; }
+                st = 0; nst = step;
+                break;
+            }
+            gz = false;
+            inside = in_grid(f, rn, &gz);
+            if (gz) fl |= 4;
+            if (!inside) { st = -3; nst = step; break; }
+            for (int c = 0; c < 3; ++c) { r[c] = rn[c]; v[c] = vn[c]; }
+            t = t + dt;
+            s0 = s1;
+        }
+        status[i] = st; steps[i] = nst; flags[i] = fl;
+    }
+}
+
+/* O5  PAPER.md L330 (segments with optional non-uniform size and gaps on a perpendicular
+ * grid), L344-350 (segment ID or error indicator per ion; atomically summed counters).
+ * Brute-force linear scan over all segments; half-open [lo,hi) (A11).                      */
+extern "C" void orc_histogram(uint64_t n, int32_t* cell_io, const double* hit_u, const double* hit_w,
+                              const uint16_t* group, uint8_t* flags, const orc_detector* det, int n_hist,
+                              uint64_t* counts, uint64_t* summary) {
+    for (uint64_t i = 0; i < n; ++i) {
+        int g = group ? (int)group[i] : 0;
+        if (g >= n_hist) continue;
+        uint64_t* sm = summary + (size_t)g * 6;
+        int32_t st = cell_io[i];
+        if (st >= -1) {
+            double u = hit_u[i], w = hit_w[i];
+            int iu = -1, iw = -1;
+            for (int k = 0; k < det->nu; ++k) {
+                if (det->u_lo[k] <= u && u < det->u_hi[k] && iu < 0) iu = k;
+                if (std::fabs(u - det->u_lo[k]) < GRAZE || std::fabs(u - det->u_hi[k]) < GRAZE) flags[i] |= 1;
+            }
+            for (int k = 0; k < det->nw; ++k) {
+                if (det->w_lo[k] <= w && w < det->w_hi[k] && iw < 0) iw = k;
+                if (std::fabs(w - det->w_lo[k]) < GRAZE || std::fabs(w - det->w_hi[k]) < GRAZE) flags[i] |= 1;
+            }
+            if (iu >= 0 && iw >= 0) {
+                cell_io[i] = iw * det->nu + iu;
+                counts[((size_t)g * det->nw + iw) * det->nu + iu] += 1;
+                sm[0] += 1;
+            } else { cell_io[i] = -1; sm[1] += 1; }
+        } else if (st == -2) sm[2] += 1;
+        else if (st == -3) sm[3] += 1;
+        else sm[4] += 1;
+        if (flags[i]) sm[5] += 1;
+    }
+}
+
+extern "C" int orc_max_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

@@ -1,0 +1,104 @@
+/* TEST INFRASTRUCTURE -- NOT PRODUCT CODE.
+ *
+ * Plain, slow, fp64 CPU oracle for the hot path of the ABP/TAIGA synthetic diagnostic
+ * (arxiv/paper_2506_15812), written from PAPER.md and the readings listed in DESIGN.md
+ * section 3 (= SURVEY.md 8(c) O0-O5, A1-A19).  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference leg may call it.  It shares no code with the
+ * CUDA path (paper_2506_15812_b200/csrc) and never includes anything from it.
+ *
+ * Parity pins (tests/test_oracle_pins.py): P1 Philox known answers; P2 RK4 amplification
+ * factor in uniform B; P3 Larmor radius / gyro-period; P4 exact parabola in uniform E;
+ * P5 kinetic-energy bound; P6 canonical momentum in axisymmetric fields; P7 step-halving
+ * order; P8 magnetic moment / grad-B drift; P9 spline properties + scipy cross-check;
+ * P10 CDF inversion exactness + statistics; P11 straight-line plane hit + brute-force
+ * binning; P12 independent naive evaluator end to end.
+ * Parity unpinned: nothing in this file; the paper's own figures that cannot be pinned
+ * (Fig. 10 loss rate, Table 1, Fig. 12 curves) are listed in DESIGN.md.
+ *
+ * Build: g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).
+ */
+#ifndef TAIGA_ORACLE_H
+#define TAIGA_ORACLE_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* field kinds: 0,1,2 = spline tables (2-D static, time slices, toroidal planes);
+ * >=10 analytic test fields used only by the pins (PAPER.md L274-282 scenarios). */
+enum { ORC_F_RZ = 0, ORC_F_RZT = 1, ORC_F_RZPHI = 2,
+       ORC_F_UNIFORM = 10,   /* B = (par0,par1,par2)                                   */
+       ORC_F_GRADB   = 11,   /* B = (0,0,par0*(1+par1*x))                              */
+       ORC_F_INVR    = 12,   /* B = (0,0,par0/sqrt(x^2+y^2))                           */
+       ORC_F_SOLOVEV = 13 }; /* analytic axisymmetric: par = psi_a,R0,a,kappa,B_T      */
+
+typedef struct {
+    int kind, nR, nZ, nS;
+    double Rmin, Rmax, Zmin, Zmax, s0, ds;
+    const double* coef[3];   /* BR, BZ, Bphi per-cell power-basis tables (orc_build_tables) */
+    double par[8];           /* analytic-field parameters */
+    double E[3];             /* uniform electric field (pins P4 only; 0 otherwise)      */
+} orc_field;
+
+typedef struct {
+    double origin[3], normal[3], eu[3], ew[3];
+    int nu, nw;
+    const double *u_lo, *u_hi, *w_lo, *w_hi;
+} orc_detector;
+
+typedef struct {
+    double v0;                       /* sqrt(2 E e / m), computed by the caller           */
+    double origin[3], axis[3], eT[3], eZ[3];
+    const double* cdf_depth;  int n_depth;  double depth_max;
+    const double* cdf_normal; int n_normal; double z_max;
+    double sigma_pos, sigma_ang;
+} orc_beam;
+
+/* O2.1  Philox4x32-10 */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+/* O2.1  five uniforms of ion `index` */
+void orc_uniforms(uint64_t seed, uint64_t index, double U[5]);
+/* O2.2  tabulated-CDF inversion; F has K+1 entries */
+double orc_cdf_invert(const double* F, int K, double x_max, double U);
+/* O2    seed ions first_index .. first_index+n-1 */
+void orc_seed(const orc_beam* b, uint64_t seed, uint64_t first_index, uint64_t n,
+              double* x, double* y, double* z, double* vx, double* vy, double* vz);
+
+/* O1  1-D splines on a unit-spaced grid: per-interval power coefficients c[i][0..3],
+ *     S(i+p) = c0 + c1 p + c2 p^2 + c3 p^3.  not-a-knot: n>=4 nodes, n-1 intervals;
+ *     periodic: n>=3 nodes, n intervals, y[n]==y[0] implied. */
+int orc_spline_notaknot(int n, const double* y, double* c);
+int orc_spline_periodic(int n, const double* y, double* c);
+/* O1  tables of ONE component.  kind 0/1: coef[nS][nR-1][nZ-1][a][b] (16 per cell);
+ *     kind 2: coef[nS][nR-1][nZ-1][c][a][b] (64 per cell).  nodal is [nS][nR][nZ]. */
+int orc_build_tables(int kind, int nR, int nZ, int nS, const double* nodal, double* coef);
+/* O0/O1 field at a Cartesian point and time: B Cartesian */
+void orc_field_B(const orc_field* f, const double r[3], double t, double B[3]);
+/* field components in the poloidal plane, (B_R,B_Z,B_phi), s = time or phi */
+void orc_field_cyl(const orc_field* f, double R, double Z, double s, double Bc[3]);
+
+/* O3  nsteps RKN steps of one ion, no termination tests (pins). variant 0 = classical
+ *     Nystrom (A1 default), 1 = k3 position from k2 (the printed Eq. 6 k3). */
+void orc_rkn_advance(const orc_field* f, double qm, int variant, double r[3], double v[3],
+                     double* t, double dt, uint64_t nsteps);
+
+/* O4  loop + termination + plane interpolation.  status: 0 crossed, -2 max_steps,
+ *     -3 left the grid, -4 bad start.  flags: bit1 plane grazing, bit2 grid grazing. */
+void orc_trace(const orc_field* f, double qm, int variant, uint64_t n,
+               const double* x, const double* y, const double* z,
+               const double* vx, const double* vy, const double* vz, const double* t0,
+               double dt, uint32_t max_steps, const orc_detector* det,
+               int32_t* status, double* hit_u, double* hit_w, double* hit_xyz /*[n][3] or 0*/,
+               uint32_t* steps, uint8_t* flags, int nthreads);
+
+/* O5  binning + counting.  cell_io in: status from orc_trace; out: cell / -1 / error.
+ *     counts[n_hist][nw][nu] and summary[n_hist][6] are accumulated into. */
+void orc_histogram(uint64_t n, int32_t* cell_io, const double* hit_u, const double* hit_w,
+                   const uint16_t* group, uint8_t* flags, const orc_detector* det, int n_hist,
+                   uint64_t* counts, uint64_t* summary);
+
+int orc_max_threads(void);
+#ifdef __cplusplus
+}
+#endif
+#endif
