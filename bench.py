@@ -1,0 +1,269 @@
+#!/usr/bin/env python
+"""bench.py -- whole hot path (a1 field precompute -> a2 seeding -> a3/a4 RKN trace -> a5
+histogram) of BASELINE.json config 2 (1,048,576 7Li+ ions, 257x513 grid) on N GPUs of one node.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2]
+
+Prints ONE JSON line (rank 0).  `value` = ion-steps/s with inputs resident in HBM; `e2e` = the
+same through the C ABI with HOST buffers (pinned nodal field H2D + counter D2H inside the timed
+region); `roofline` = the trace kernel against the FP64 issue rate measured live by a
+register-resident DFMA microkernel; `cpu_baseline` = the oracle timed on the host cores on a
+bounded prefix sample.  --impl reference times the oracle itself (rank 0 only).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+# FP64-pipe instructions per ion-step of the classical RKN step on a 2-D bicubic field
+# (3 field evaluations x 61 + 4 cross products x 6 + stage/Eq.5/plane 45).
+ALG_FP64_INSTR_PER_ION_STEP = {0: 252.0, 1: 402.0, 2: 840.0}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--ions", type=int, default=0, help="override ions per group (debug)")
+    ap.add_argument("--oracle-sample", type=int, default=131072)
+    ap.add_argument("--opt", action="append", default=[], help="key=value for taiga_set_option")
+    return ap.parse_args()
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([c.strip() for c in out.strip().split(",")])
+            except Exception:
+                pass
+            time.sleep(0.05)
+
+    def summary(self):
+        sm, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = max(mx, float(r[1]))
+                for nme, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nme)
+            except Exception:
+                continue
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx or None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_run(cfg_index, sample, nthreads=0):
+    """The oracle as it stands on a prefix sample; returns (ion_steps, ions, seconds, threads)."""
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import oracle as orc
+    from paper_2506_15812_b200 import workloads as wl
+    cfg = wl.config(cfg_index, n_override=max(sample // len(wl.config(cfg_index).groups), 1))
+    t0 = time.perf_counter()
+    res = orc.run_config(cfg, nthreads=nthreads)
+    dt = time.perf_counter() - t0
+    steps = sum(int(g["steps"].astype("int64").sum()) for g in res["groups"])
+    return steps, cfg.n_ions, dt, orc.max_threads(), cfg
+
+
+def main_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    for _ in range(min(args.warmup, 1)):
+        oracle_run(args.config, max(args.oracle_sample // 8, 1024))
+    tot_steps, tot_t, n_ions, cores = 0, 0.0, 0, 1
+    for _ in range(args.steps):
+        s, n, dt, cores, cfg = oracle_run(args.config, args.oracle_sample)
+        tot_steps += s; tot_t += dt; n_ions = n
+    v = tot_steps / tot_t
+    sample = "first %d ions of config %d (prefix sample; identical ions, Philox counter = ion index), whole path a1-a5 per step" % (n_ions, args.config)
+    print(json.dumps({
+        "impl": "reference", "metric": "ion-steps/s", "value": v, "unit": "ion-steps/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "cfg%d prefix sample of %d ions" % (args.config, n_ions)},
+        "cpu_baseline": {"value": v, "unit": "ion-steps/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": "ion-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "ions_per_s": n_ions * args.steps / tot_t}))
+
+
+def launches_per_step(cfg, kind):
+    a1 = 12 + (1 if kind == 2 else 0)          # 3 components x (3 line-solve + 1 assemble) [+ phi spline]
+    ntrace = 1 if cfg.detector is not None else len(cfg.groups)
+    return a1 + len(cfg.groups) + ntrace * (5 + 1) + ntrace      # seeds + (sort 5 + trace 1) + histogram
+
+
+def main_ours(args):
+    import numpy as np
+    import torch
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2506_15812_b200 import taiga, workloads as wl
+    dev = "cuda:%d" % local
+    cfg = wl.config(args.config, n_override=args.ions or None)
+    for g in cfg.groups:                        # weak scaling: every rank traces its own ions
+        g.first_index += rank << 40
+    grid, nodal = cfg.field_builder()
+    nodal_dev = [torch.from_numpy(np.ascontiguousarray(c)).to(dev) for c in nodal]
+    nodal_pin = [torch.from_numpy(np.ascontiguousarray(c)).pin_memory() for c in nodal]
+    tg = taiga.Taiga(local)
+    for kv in args.opt:
+        k, v = kv.split("=")
+        tg.set_option(k, int(v))
+    peak_dfma = tg.fp64_peak(100.0)             # FP64-pipe instructions / s, measured live
+    tg.set_option("stats", 0)                   # no host sync inside taiga_trace while timing
+    ions = taiga.Ions(cfg.n_ions, dev)
+    det0 = cfg.detector or cfg.groups[0].detector
+    counts = torch.zeros((cfg.n_hist, det0.nw, det0.nu), dtype=torch.int64, device=dev)
+    summary = torch.zeros((cfg.n_hist, 6), dtype=torch.int64, device=dev)
+    counts_pin = torch.zeros(counts.shape, dtype=torch.int64).pin_memory()
+    summary_pin = torch.zeros(summary.shape, dtype=torch.int64).pin_memory()
+    cd, cn = wl.depth_cdf(), wl.normal_cdf()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    trace_ms = []
+
+    def step(host, record=False):
+        if host:
+            fld = [d.copy_(p, non_blocking=True) for d, p in zip(nodal_dev, nodal_pin)]   # H2D from pinned
+        else:
+            fld = nodal_dev
+        tg.load_field(grid, fld)                                                        # a1
+        counts.zero_(); summary.zero_()
+        off, spans = 0, []
+        for g in cfg.groups:
+            v = ions.view(off, off + g.n_ions)
+            tg.seed_beam(g.beam, cd, cn, cfg.seed, v, g.first_index, g.group, g.t0)      # a2
+            spans.append((v, g)); off += g.n_ions
+        e0, e1 = ev(), ev()
+        e0.record()
+        if cfg.detector is not None:
+            b = cfg.groups[0].beam
+            tg.trace(ions, b.charge_C / b.mass_kg, cfg.dt, cfg.max_steps, cfg.detector)   # a3 + a4
+        else:
+            for v, g in spans:
+                tg.trace(v, g.beam.charge_C / g.beam.mass_kg, cfg.dt, cfg.max_steps, g.detector)
+        e1.record()
+        if cfg.detector is not None:
+            tg.detector_histogram(ions, cfg.detector, cfg.n_hist, counts, summary)       # a5
+        else:
+            for v, g in spans:
+                tg.detector_histogram(v, g.detector, cfg.n_hist, counts, summary)
+        if world > 1:
+            dist.all_reduce(counts); dist.all_reduce(summary)                            # exchange step: <= 0.5 MB
+        if host:
+            counts_pin.copy_(counts, non_blocking=True); summary_pin.copy_(summary, non_blocking=True)
+        if record:
+            trace_ms.append((e0, e1))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(host):
+        for _ in range(max(args.warmup, 3)):
+            step(host)
+        barrier()
+        times = []
+        for _ in range(args.steps):
+            flush.zero_()                       # L2 flush between timed iterations
+            torch.cuda.synchronize()
+            if host:
+                t0 = time.perf_counter(); step(True); torch.cuda.synchronize(); times.append((time.perf_counter() - t0) * 1e3)
+            else:
+                a, b = ev(), ev()
+                a.record(); step(False, record=True); b.record(); torch.cuda.synchronize()
+                times.append(a.elapsed_time(b))
+        barrier()
+        tot = torch.tensor([sum(times)], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(tot, op=dist.ReduceOp.MAX)
+        return float(tot.item())
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    total_ms = timed(False)
+    total_ms_e2e = timed(True)
+    sampler.stop_flag = True
+    ion_steps_rank = int(ions.steps.to(torch.int64).sum().item())
+    tsum = torch.tensor([ion_steps_rank, cfg.n_ions], dtype=torch.int64, device=dev)
+    if world > 1:
+        dist.all_reduce(tsum)
+    ion_steps, n_ions = int(tsum[0]), int(tsum[1])
+    t_trace = sum(a.elapsed_time(b) for a, b in trace_ms) / len(trace_ms)
+    kind = grid.kind
+    alg = ALG_FP64_INSTR_PER_ION_STEP[kind]
+    achieved = ion_steps_rank * alg / (t_trace * 1e-3)
+    h2d = sum(p.numel() * 8 for p in nodal_pin) + (len(cd) + len(cn)) * 8 * len(cfg.groups) + 4 * (det0.nu + det0.nw) * 8
+    d2h = counts.numel() * 8 + summary.numel() * 8
+    s_ok = int(summary[:, :5].sum().item()) == n_ions
+    out = {
+        "metric": "ion-steps/s", "value": ion_steps * args.steps / (total_ms * 1e-3), "unit": "ion-steps/s",
+        "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "BASELINE config %d (%s): %d ions/GPU, grid %dx%dx%d kind %d, dt=%g, max_steps=%d, whole path a1-a5 per step"
+                               % (args.config, cfg.name, cfg.n_ions, grid.nR, grid.nZ, grid.nS, kind, cfg.dt, cfg.max_steps),
+                   "l2": "256 MiB buffer written between timed iterations (L2 flush)",
+                   "ion_steps_per_step": ion_steps, "ions_per_step": n_ions, "invariant_counts_sum_to_n": s_ok},
+        "ions_per_s": n_ions * args.steps / (total_ms * 1e-3),
+        "trace_kernel": {"ms": t_trace, "ion_steps_per_s": ion_steps_rank / (t_trace * 1e-3)},
+        "e2e": {"value": ion_steps * args.steps / (total_ms_e2e * 1e-3), "unit": "ion-steps/s",
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": total_ms_e2e / args.steps,
+                "timing": "host wall clock around the C-ABI calls incl. pinned H2D of the nodal field and D2H of the counters"},
+        "gpu_launches": launches_per_step(cfg, kind) * args.steps,
+        "roofline": {"bound": "alu", "achieved": 2e-12 * achieved, "peak": 2e-12 * peak_dfma,
+                     "unit": "TFLOP/s (FP64 pipe; every FP64 instruction counted as one FMA = 2 flop)",
+                     "frac": achieved / peak_dfma, "traffic": None,
+                     "kernel": "k_trace", "alg_fp64_instr_per_ion_step": alg,
+                     "peak_source": "measured live: register-resident DFMA microkernel (taiga_measure_fp64_peak); "
+                                    "nominal 148 SM x 64 lanes x 1.965 GHz = 18.6e12 instr/s"},
+        "clocks": sampler.summary(),
+    }
+    if rank == 0:
+        if world == 1:
+            s, n, dt, cores, _ = oracle_run(args.config, args.oracle_sample)
+            out["cpu_baseline"] = {"value": s / dt, "unit": "ion-steps/s", "cores": cores, "kind": "oracle",
+                                   "ions_per_s": n / dt, "seconds": dt,
+                                   "sample": "first %d ions of config %d (prefix sample, identical ions), whole path a1-a5, OpenMP over ions" % (n, args.config)}
+        print(json.dumps(out))
+    tg.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        main_reference(a)
+    else:
+        main_ours(a)

@@ -1,0 +1,163 @@
+/* taiga.h -- C ABI of the B200-native hot path of the ABP/TAIGA synthetic diagnostic
+ * (arxiv/paper_2506_15812): field-coefficient precompute -> beam seeding -> Runge-Kutta-Nystrom
+ * trajectory integration -> detector-plane crossing -> Faraday-cup histogram.
+ *
+ * Conventions
+ *  - Every function returns 0 (TAIGA_OK) or a negative TAIGA_E_* code; nothing aborts or
+ *    throws.  taiga_last_error(ctx) returns a NUL-terminated message owned by ctx.
+ *  - "dev" pointers are CUDA device pointers owned by the caller (e.g. torch tensors);
+ *    "host" pointers are ordinary host memory, read during the call only.  The ctx owns only
+ *    its internal tables / scratch and frees them in taiga_destroy.
+ *  - All kernels are enqueued on the ctx's stream.  taiga_load_field, taiga_seed_beam and
+ *    taiga_detector_histogram return without synchronising; taiga_trace synchronises the
+ *    stream internally between compaction passes (it reads back one survivor counter).
+ *  - Coordinates: right-handed Cartesian (X,Y,Z), Z vertical, torus axis = Z,
+ *    R = sqrt(X^2+Y^2); (R,phi,Z) right-handed; SI units.
+ *  - There is no CPU fallback: every entry point needs an sm_100 device.
+ */
+#ifndef TAIGA_H
+#define TAIGA_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TAIGA_OK        0
+#define TAIGA_E_ARG    -1   /* null pointer, bad shape, non-monotone CDF, non-orthonormal frame */
+#define TAIGA_E_STATE  -2   /* call order: e.g. trace before load_field                        */
+#define TAIGA_E_CUDA   -3   /* a CUDA runtime call or kernel failed                            */
+#define TAIGA_E_NOMEM  -4   /* device allocation failed                                        */
+
+/* per-ion result codes written to taiga_ions.cell ("a segment ID
+ * value or an error indicator") */
+#define TAIGA_CELL_MISS      -1  /* crossed the plane, no segment (gap / outside); also the
+                                    value taiga_trace leaves for every plane-crossing ion until
+                                    taiga_detector_histogram assigns the segment              */
+#define TAIGA_CELL_MAXSTEPS  -2  /* max_steps reached (trapped)                                */
+#define TAIGA_CELL_OUT       -3  /* left the field grid                                        */
+#define TAIGA_CELL_BADSTART  -4  /* starts on/behind the plane or outside the grid             */
+/* taiga_ions.flags bits: results within 1e-9 m of a decision boundary */
+#define TAIGA_FLAG_EDGE   1      /* hit within 1e-9 m of a segment edge                        */
+#define TAIGA_FLAG_PLANE  2      /* |s| < 1e-9 m at an end of the crossing step                */
+#define TAIGA_FLAG_GRID   4      /* within 1e-9 m of the grid boundary when leaving it         */
+
+typedef struct taiga_ctx taiga_ctx;
+
+/* device: CUDA ordinal; cuda_stream: a cudaStream_t (0 = default stream). */
+int  taiga_create(taiga_ctx** out, int device, void* cuda_stream);
+int  taiga_destroy(taiga_ctx* ctx);
+const char* taiga_last_error(const taiga_ctx* ctx);
+
+/* ---- a1: field tables (PAPER.md "bicubic B-spline fitted to the grid points ... the
+ * coefficients are calculated and stored during the initialization"; L312; L65 toroidal
+ * symmetry).  Interpolating tensor-product cubic spline with not-a-knot ends in R and Z
+ * (reading A4), each of B_R, B_Z, B_phi separately (A5).
+ *   kind 0: static (R,Z).  kind 1: nS time slices, linear in t, held outside [s0, s0+(nS-1)ds]
+ *   (A16).  kind 2: nS toroidal planes spanning ONE period nS*ds, periodic cubic spline in phi
+ *   (tricubic, A17).  Grids are uniform; node (i,j) sits at Rmin+i*hR, Zmin+j*hZ. */
+typedef struct {
+    int kind, nR, nZ, nS;            /* nR,nZ >= 4; nS = 1 (kind 0), >= 2 (kind 1), >= 3 (kind 2) */
+    double Rmin, Rmax, Zmin, Zmax;
+    double s0, ds;                   /* first slice time, spacing [s]  |  phi0, dphi [rad]        */
+} taiga_grid;
+
+typedef struct {
+    int form;        /* 0: nodal values [nS][nR][nZ] row-major -> the precompute kernel runs
+                        1: ready per-cell power-basis coefficients, [nS][nR-1][nZ-1][16] (kind
+                           0/1, index a*4+b of p^a w^b) or [...][64] (kind 2, c*16+a*4+b of
+                           q^c p^a w^b): "read from the preprocessing database" mode (L312)   */
+    const double *BR, *BZ, *Bphi;    /* three components, tesla                                  */
+    int on_device;   /* 0: host pointers (copied inside the call)  1: dev pointers               */
+} taiga_coeffs;
+
+int taiga_load_field(taiga_ctx* ctx, const taiga_grid* grid, const taiga_coeffs* coeffs);
+
+/* test / inspection hooks for a1: evaluate (B_R,B_Z,B_phi) at n points (dev arrays; s = time
+ * or phi, may be null), and copy the internal per-cell table of one component back in the
+ * form-1 layout above (host buffer of nS*(nR-1)*(nZ-1)*{16|64} doubles). */
+int taiga_field_eval(taiga_ctx* ctx, uint64_t n, const double* R_dev, const double* Z_dev,
+                     const double* s_dev, double* BR_dev, double* BZ_dev, double* Bphi_dev);
+int taiga_field_table(taiga_ctx* ctx, int component, double* table_host);
+
+/* ---- ion storage: SoA, dev, caller-owned, length n each.  x..vz are written by
+ * taiga_seed_beam and only read by taiga_trace (so one seeding can be traced against several
+ * detectors).  group/t0 may be null in taiga_trace / taiga_detector_histogram (=> 0). */
+typedef struct {
+    double *x, *y, *z, *vx, *vy, *vz;    /* initial position [m], velocity [m/s]              */
+    double *hit_u, *hit_w;               /* detector-plane coordinates of the hit [m]          */
+    int32_t *cell;                       /* segment iw*nu+iu, or TAIGA_CELL_*                  */
+    uint32_t *steps;                     /* RKN steps taken                                    */
+    uint8_t *flags;                      /* TAIGA_FLAG_*                                       */
+    uint16_t *group;                     /* histogram index (energy / time slice)              */
+    double *t0;                          /* birth time [s] (kind-1 fields)                     */
+    uint64_t n;                          /* < 2^32                                             */
+} taiga_ions;
+
+/* ---- a2: beam seeding (PAPER.md L314 stochastic initialisation: "the primary attenuation
+ * profile as a cumulative distribution function ... randomly sampling it", on the GPU;
+ * L128-134 linear beam model: ionisation depends on the position along the beam only).
+ * Ion j (0 <= j < ions->n) uses Philox4x32-10 with key=(seed lo,hi), counters
+ * (i lo, i hi, b, 0), b=0,1,2, i = first_index + j; five 52-bit uniforms; every draw is a
+ * tabulated-CDF inversion with linear interpolation (bit-identical on any IEEE machine):
+ *   depth d along `axis` from cdf_depth; cross-section offsets sigma_pos*(z1 eT + z2 eZ) and
+ *   divergence angles sigma_ang*(z3, z4) from cdf_normal (table on [-z_max, z_max]);
+ *   speed v0 = sqrt(2 energy_eV e / m) with e = charge_C.
+ * CDF tables: host pointers, K+1 entries, F[0]=0, F[K]=1, non-decreasing. */
+typedef struct {
+    double mass_kg, charge_C, energy_eV;
+    double origin[3], axis[3], eT[3], eZ[3];       /* orthonormal (axis, eT, eZ)              */
+    const double* cdf_depth;  int n_depth;  double depth_max;
+    const double* cdf_normal; int n_normal; double z_max;
+    double sigma_pos_m, sigma_ang_rad;
+    uint64_t first_index;
+    uint16_t group; double t0;                     /* written to ions->group / ions->t0       */
+} taiga_beam_params;
+
+int taiga_seed_beam(taiga_ctx* ctx, const taiga_beam_params* params, uint64_t seed,
+                    taiga_ions* ions);
+
+/* ---- detector (plane normal + perpendicular grid of segments with optional
+ * non-uniform size and gaps; coordinate transformation to the plane).  u = (p-origin).eu,
+ * w = (p-origin).ew.  Segment k of an axis is the half-open interval [lo[k], hi[k]); segments
+ * must be ordered and non-overlapping.  Edge arrays are host pointers. */
+typedef struct {
+    double origin[3], normal[3], eu[3], ew[3];     /* orthonormal (normal, eu, ew)            */
+    int nu, nw;
+    const double *u_lo, *u_hi, *w_lo, *w_hi;
+} taiga_detector;
+
+/* ---- a3 + a4: integrator and termination (Eq. 3; Eq. 5-6 L218-235 with
+ * readings A1-A3; L326 stop at the plane or at max_steps; L338 two-state storage and linear
+ * interpolation to the plane; L318 error value).  E = 0.  charge_C/mass_kg of the LAST
+ * taiga_seed_beam call is NOT implied: q/m is passed explicitly.
+ * Writes hit_u, hit_w, cell (TAIGA_CELL_MISS for every plane-crossing ion, or an error code),
+ * steps, flags.  rkn_variant: 0 = classical Nystrom (default reading A1), 1 = k3 position
+ * increment from k2 (Eq. 6 as printed). */
+int taiga_trace(taiga_ctx* ctx, taiga_ions* ions, double q_over_m, double dt,
+                uint32_t max_steps, const taiga_detector* det, int rkn_variant);
+
+/* ---- a5: binning + histogram (segment ID per ion; atomically summed
+ * per-segment counters; only the compact counter array is returned).
+ * counts_dev [n_hist][nw][nu] and summary_dev [n_hist][6] = {hit, miss, maxsteps, out,
+ * badstart, flagged} are ACCUMULATED into (caller zeroes).  Rewrites ions->cell for plane
+ * crossers (segment id or TAIGA_CELL_MISS) and ORs TAIGA_FLAG_EDGE into ions->flags. */
+int taiga_detector_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det,
+                             int n_hist, unsigned long long* counts_dev,
+                             unsigned long long* summary_dev);
+
+/* ---- tuning / measurement hooks (not part of the method) */
+/* integer options: "sort" (1: order ions by birth cell before tracing, default 1),
+ * "chunk0", "chunk" (steps per compaction pass), "min_active" (spill threshold),
+ * "ctas_per_sm", "variant" (kernel variant), "stats" (collect counters). */
+int taiga_set_option(taiga_ctx* ctx, const char* key, long long value);
+/* counters of the last taiga_trace: [0] ion-steps, [1] warp-steps*32 (lane slots issued),
+ * [2] passes, [3] kernel launches, [4] cell reloads, [5] survivors after pass 0. */
+int taiga_get_stats(taiga_ctx* ctx, unsigned long long stats_host[8]);
+/* register-resident DFMA microkernel: measured FP64 FMA instructions per second (thread-level,
+ * i.e. lanes x instr) over ~`ms` milliseconds; the roofline denominator. */
+int taiga_measure_fp64_peak(taiga_ctx* ctx, double ms, double* dfma_per_s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,113 @@
+// a2: beam seeding (PAPER.md L314 stochastic initialisation on the GPU; L128-134 linear beam
+// model).  One thread per ion; counter-based Philox4x32-10 keyed by (seed, global ion index) so
+// the result is independent of launch geometry and sharding; every draw is a tabulated-CDF
+// inversion using only +,-,*,/,fma,sqrt (IEEE, explicitly rounded intrinsics so that nvcc
+// never contracts them): bit-identical on any IEEE-754 machine.
+#include "taiga_internal.h"
+
+struct SeedParams {
+    double v0, origin[3], axis[3], eT[3], eZ[3];
+    const double* cdf_depth;  int n_depth;  double depth_max;
+    const double* cdf_normal; int n_normal; double z_max;
+    double sigma_pos, sigma_ang;
+    unsigned long long first_index, seed, n;
+    unsigned short group; double t0;
+};
+
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1, uint32_t out[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        if (r > 0) { k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+        uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// 52-bit uniform in (0,1): ((w0>>6)*2^26 + (w1>>6) + 0.5) * 2^-52, exact in fp64
+__device__ __forceinline__ double u52(uint32_t w0, uint32_t w1) {
+    unsigned long long n = ((unsigned long long)(w0 >> 6) << 26) + (unsigned long long)(w1 >> 6);
+    return __dmul_rn(__dadd_rn((double)n, 0.5), 0x1p-52);
+}
+
+// find j with F_j <= U < F_{j+1}; x = fma(t, dx, j*dx), t = (U-F_j)/(F_{j+1}-F_j), dx = x_max/K
+__device__ __forceinline__ double cdf_invert(const double* __restrict__ F, int K, double x_max, double U) {
+    int lo = 0, hi = K;
+    while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (__ldg(F + mid) <= U) lo = mid; else hi = mid;
+    }
+    double dx = __ddiv_rn(x_max, (double)K);
+    double Fl = __ldg(F + lo), Fh = __ldg(F + lo + 1);
+    double t = __ddiv_rn(__dsub_rn(U, Fl), __dsub_rn(Fh, Fl));
+    return __fma_rn(t, dx, __dmul_rn((double)lo, dx));
+}
+
+__global__ void __launch_bounds__(256) k_beam_seed(SeedParams P, double* __restrict__ x, double* __restrict__ y,
+                                                   double* __restrict__ z, double* __restrict__ vx,
+                                                   double* __restrict__ vy, double* __restrict__ vz,
+                                                   unsigned short* __restrict__ group, double* __restrict__ t0) {
+    unsigned long long j = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= P.n) return;
+    unsigned long long idx = P.first_index + j;
+    uint32_t w[12];
+#pragma unroll
+    for (uint32_t b = 0; b < 3; ++b)
+        philox4x32_10((uint32_t)idx, (uint32_t)(idx >> 32), b, 0u, (uint32_t)P.seed, (uint32_t)(P.seed >> 32), w + 4 * b);
+    double U[5];
+#pragma unroll
+    for (int k = 0; k < 5; ++k) U[k] = u52(w[2 * k], w[2 * k + 1]);
+    double zw = __dmul_rn(2.0, P.z_max);
+    double d = cdf_invert(P.cdf_depth, P.n_depth, P.depth_max, U[0]);
+    double z1 = __dsub_rn(cdf_invert(P.cdf_normal, P.n_normal, zw, U[1]), P.z_max);
+    double z2 = __dsub_rn(cdf_invert(P.cdf_normal, P.n_normal, zw, U[2]), P.z_max);
+    double r[3], v[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c)   // r = (origin + d axis) + sigma_pos (z1 eT + z2 eZ)
+        r[c] = __dadd_rn(__dadd_rn(P.origin[c], __dmul_rn(d, P.axis[c])),
+                         __dmul_rn(P.sigma_pos, __dadd_rn(__dmul_rn(z1, P.eT[c]), __dmul_rn(z2, P.eZ[c]))));
+    if (P.sigma_ang == 0.0) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) v[c] = __dmul_rn(P.v0, P.axis[c]);
+    } else {
+        double z3 = __dsub_rn(cdf_invert(P.cdf_normal, P.n_normal, zw, U[3]), P.z_max);
+        double z4 = __dsub_rn(cdf_invert(P.cdf_normal, P.n_normal, zw, U[4]), P.z_max);
+        double thT = __dmul_rn(P.sigma_ang, z3), thZ = __dmul_rn(P.sigma_ang, z4);
+        double nrm = __dsqrt_rn(__dadd_rn(__dadd_rn(1.0, __dmul_rn(thT, thT)), __dmul_rn(thZ, thZ)));
+#pragma unroll
+        for (int c = 0; c < 3; ++c)   // v = v0 ((axis + thT eT) + thZ eZ) / nrm
+            v[c] = __ddiv_rn(__dmul_rn(P.v0, __dadd_rn(__dadd_rn(P.axis[c], __dmul_rn(thT, P.eT[c])), __dmul_rn(thZ, P.eZ[c]))), nrm);
+    }
+    x[j] = r[0]; y[j] = r[1]; z[j] = r[2];
+    vx[j] = v[0]; vy[j] = v[1]; vz[j] = v[2];
+    if (group) group[j] = P.group;
+    if (t0) t0[j] = P.t0;
+}
+
+int tg_seed(taiga_ctx* ctx, const taiga_beam_params* p, uint64_t seed, taiga_ions* ions, double v0) {
+    size_t cd = ctx->cap_depth, cn = ctx->cap_normal;
+    int rc = tg_reserve(ctx, &ctx->cdf_depth, &cd, (size_t)p->n_depth + 1);
+    ctx->cap_depth = (int)cd;
+    if (rc) return rc;
+    rc = tg_reserve(ctx, &ctx->cdf_normal, &cn, (size_t)p->n_normal + 1);
+    ctx->cap_normal = (int)cn;
+    if (rc) return rc;
+    // pageable-source async copies are staged before returning, so the host tables may be freed
+    TG_CUDA(ctx, cudaMemcpyAsync(ctx->cdf_depth, p->cdf_depth, ((size_t)p->n_depth + 1) * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    TG_CUDA(ctx, cudaMemcpyAsync(ctx->cdf_normal, p->cdf_normal, ((size_t)p->n_normal + 1) * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    SeedParams P;
+    P.v0 = v0;
+    for (int c = 0; c < 3; ++c) { P.origin[c] = p->origin[c]; P.axis[c] = p->axis[c]; P.eT[c] = p->eT[c]; P.eZ[c] = p->eZ[c]; }
+    P.cdf_depth = ctx->cdf_depth; P.n_depth = p->n_depth; P.depth_max = p->depth_max;
+    P.cdf_normal = ctx->cdf_normal; P.n_normal = p->n_normal; P.z_max = p->z_max;
+    P.sigma_pos = p->sigma_pos_m; P.sigma_ang = p->sigma_ang_rad;
+    P.first_index = p->first_index; P.seed = seed; P.n = ions->n;
+    P.group = p->group; P.t0 = p->t0;
+    unsigned blocks = (unsigned)((ions->n + 255) / 256);
+    k_beam_seed<<<blocks, 256, 0, ctx->stream>>>(P, ions->x, ions->y, ions->z, ions->vx, ions->vy, ions->vz, ions->group, ions->t0);
+    TG_CUDA(ctx, cudaGetLastError());
+    return TAIGA_OK;
+}

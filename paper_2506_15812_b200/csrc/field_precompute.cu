@@ -1,0 +1,246 @@
+// a1: field-coefficient precompute.  Interpolating tensor-product cubic
+// spline, not-a-knot in R and Z, periodic in phi (kind 2).  Line-parallel solves: one thread
+// per grid line for the second derivatives, then one thread per (cell, component) assembles
+// the 16 power-basis coefficients from {y, y_zz, y_rr, y_rrzz} at the 4 corners.
+//
+// not-a-knot on a unit-spaced line, unknowns M_i = S''(x_i):
+//   M_{i-1} + 4 M_i + M_{i+1} = 6 (y_{i-1} - 2 y_i + y_{i+1}),   i = 1..n-2
+//   M_0 - 2 M_1 + M_2 = 0   =>  substituting into row 1:  M_1 = y_0 - 2 y_1 + y_2
+//   (same at the far end), so the system is tridiagonal in M_2..M_{n-3} with known ends.
+#include <vector>
+
+#include "field_device.cuh"
+
+// cp[i] = Thomas pivots of the (1,4,1) interior system: cp[2] = 1/4, cp[i] = 1/(4 - cp[i-1]).
+__global__ void k_spline_lines(const double* __restrict__ y, double* __restrict__ M, const double* __restrict__ cp,
+                               int n, long long stride, int lines_inner, long long inner_stride,
+                               long long outer_stride, int nlines) {
+    int line = blockIdx.x * blockDim.x + threadIdx.x;
+    if (line >= nlines) return;
+    long long base = (long long)(line / lines_inner) * outer_stride + (long long)(line % lines_inner) * inner_stride;
+    const double* yl = y + base;
+    double* Ml = M + base;
+    auto Y = [&](int i) { return yl[(long long)i * stride]; };
+    auto d2 = [&](int i) { return (Y(i - 1) - 2.0 * Y(i)) + Y(i + 1); };
+    double M1 = d2(1), Mn2 = d2(n - 2);
+    Ml[stride] = M1;
+    Ml[(long long)(n - 2) * stride] = Mn2;
+    double dprev = 0.0;
+    for (int i = 2; i <= n - 3; ++i) {
+        double rhs = 6.0 * d2(i);
+        if (i == 2) rhs -= M1;
+        if (i == n - 3) rhs -= Mn2;
+        double dp = (i == 2) ? rhs * cp[i] : (rhs - dprev) * cp[i];
+        Ml[(long long)i * stride] = dp;
+        dprev = dp;
+    }
+    for (int i = n - 4; i >= 2; --i)
+        Ml[(long long)i * stride] = Ml[(long long)i * stride] - cp[i] * Ml[(long long)(i + 1) * stride];
+    double M2 = Ml[2 * stride], Mn3 = Ml[(long long)(n - 3) * stride];
+    Ml[0] = 2.0 * M1 - M2;
+    Ml[(long long)(n - 1) * stride] = 2.0 * Mn2 - Mn3;
+}
+
+// power-basis coefficients of one interval from end values g0,g1 and end second derivatives G0,G1
+__device__ __forceinline__ void seg_coef(double g0, double g1, double G0, double G1, double c[4]) {
+    c[0] = g0;
+    c[1] = (g1 - g0) - (2.0 * G0 + G1) / 6.0;
+    c[2] = G0 / 2.0;
+    c[3] = (G1 - G0) / 6.0;
+}
+
+// thread per (slice, cell, comp).  nodal arrays of one component: 4 planes of [nS][nR][nZ].
+// out index by `mode`: 0 -> kind-0/1 internal layout, 1 -> temp layout [k][cell][comp][16] for kind 2
+__global__ void k_assemble(const double* __restrict__ y, const double* __restrict__ Mz, const double* __restrict__ Myr,
+                           const double* __restrict__ Mzr, double* __restrict__ out, int nS, int nR, int nZ,
+                           int comp, int mode) {
+    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    int cR = nR - 1, cZ = nZ - 1;
+    long long ncell = (long long)cR * cZ;
+    if (t >= ncell * nS) return;
+    int k = (int)(t / ncell);
+    long long cell = t % ncell;
+    int i = (int)(cell / cZ), j = (int)(cell % cZ);
+    long long n00 = ((long long)k * nR + i) * nZ + j, n10 = n00 + nZ;
+    double cz[2][4], Dz[2][4];                 // w-coefficients of y and of y_rr at R-nodes i, i+1
+    seg_coef(y[n00], y[n00 + 1], Mz[n00], Mz[n00 + 1], cz[0]);
+    seg_coef(y[n10], y[n10 + 1], Mz[n10], Mz[n10 + 1], cz[1]);
+    seg_coef(Myr[n00], Myr[n00 + 1], Mzr[n00], Mzr[n00 + 1], Dz[0]);
+    seg_coef(Myr[n10], Myr[n10 + 1], Mzr[n10], Mzr[n10 + 1], Dz[1]);
+    double* o = (mode == 0) ? out + ((cell * nS + k) * 3 + comp) * 16
+                            : out + (((long long)k * ncell + cell) * 3 + comp) * 16;
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+        double ca[4];
+        seg_coef(cz[0][b], cz[1][b], Dz[0][b], Dz[1][b], ca);
+#pragma unroll
+        for (int a = 0; a < 4; ++a) o[a * 4 + b] = ca[a];
+    }
+}
+
+// kind 2: periodic spline in phi of every bicubic coefficient.  G = first column of the inverse
+// of the circulant (1,4,1) matrix.  thread per (cell, comp, ab).
+#define TG_MAX_PLANES 128
+__global__ void k_phi_spline(const double* __restrict__ bic, const double* __restrict__ G, double* __restrict__ out,
+                             int nS, long long ncell) {
+    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= ncell * 48) return;
+    long long cell = t / 48;
+    int comp = (int)((t % 48) / 16), ab = (int)(t % 16);
+    double c[TG_MAX_PLANES], rhs[TG_MAX_PLANES];
+    for (int k = 0; k < nS; ++k) c[k] = bic[(((long long)k * ncell + cell) * 3 + comp) * 16 + ab];
+    for (int k = 0; k < nS; ++k) rhs[k] = 6.0 * ((c[(k + nS - 1) % nS] - 2.0 * c[k]) + c[(k + 1) % nS]);
+    double Mprev = 0.0, M0 = 0.0;
+    for (int kk = 0; kk <= nS; ++kk) {          // M_k for k = 0..nS (M_nS = M_0), emit interval k-1
+        int k = kk % nS;
+        double M = 0.0;
+        for (int m = 0; m < nS; ++m) M = fma(G[(k - m + nS) % nS], rhs[m], M);
+        if (kk == 0) M0 = M;
+        if (kk == nS) M = M0;
+        if (kk > 0) {
+            double d[4];
+            seg_coef(c[kk - 1], c[k], Mprev, M, d);
+            double* o = out + (((long long)(kk - 1) * ncell + cell) * 3 + comp) * 64;
+#pragma unroll
+            for (int e = 0; e < 4; ++e) o[e * 16 + ab] = d[e];
+        }
+        Mprev = M;
+    }
+}
+
+// form-1 input (per-cell coefficients [nS][cell][per]) <-> internal layout
+__global__ void k_relayout(const double* __restrict__ src, double* __restrict__ dst, int kind, int nS, long long ncell,
+                           int comp, int to_internal) {
+    int per = (kind == 2) ? 64 : 16;
+    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= ncell * nS * per) return;
+    int e = (int)(t % per);
+    long long cell = (t / per) % ncell;
+    int k = (int)(t / per / ncell);
+    long long in = (kind == 2) ? (((long long)k * ncell + cell) * 3 + comp) * 64 + e
+                               : ((cell * nS + k) * 3 + comp) * 16 + e;
+    if (to_internal) dst[in] = src[t]; else dst[t] = src[in];
+}
+
+__global__ void k_field_eval(FieldDev f, unsigned long long n, const double* R, const double* Z, const double* s,
+                             double* BR, double* BZ, double* Bp) {
+    unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double a, b, c;
+    tg_field_cyl(f, R[i], Z[i], s ? s[i] : 0.0, a, b, c);
+    BR[i] = a; BZ[i] = b; Bp[i] = c;
+}
+
+static std::vector<double> thomas_pivots(int n) {
+    std::vector<double> cp(n > 0 ? n : 1, 0.0);
+    for (int i = 2; i <= n - 3; ++i) cp[i] = (i == 2) ? 0.25 : 1.0 / (4.0 - cp[i - 1]);
+    return cp;
+}
+
+// first column of inverse of circulant(4,1,0,...,0,1), by Gaussian elimination (n <= 128)
+static std::vector<double> circulant_inverse_col(int n) {
+    std::vector<double> A((size_t)n * n, 0.0), x(n, 0.0);
+    for (int i = 0; i < n; ++i) { A[(size_t)i * n + i] += 4.0; A[(size_t)i * n + (i + 1) % n] += 1.0; A[(size_t)i * n + (i + n - 1) % n] += 1.0; }
+    x[0] = 1.0;
+    for (int c = 0; c < n; ++c)                   // diagonally dominant: no pivoting needed
+        for (int r = c + 1; r < n; ++r) {
+            double f = A[(size_t)r * n + c] / A[(size_t)c * n + c];
+            if (f == 0.0) continue;
+            for (int k = c; k < n; ++k) A[(size_t)r * n + k] -= f * A[(size_t)c * n + k];
+            x[r] -= f * x[c];
+        }
+    for (int r = n - 1; r >= 0; --r) {
+        double s = x[r];
+        for (int k = r + 1; k < n; ++k) s -= A[(size_t)r * n + k] * x[k];
+        x[r] = s / A[(size_t)r * n + r];
+    }
+    return x;
+}
+
+int tg_precompute(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c) {
+    const int nR = g->nR, nZ = g->nZ, nS = g->nS, cR = nR - 1, cZ = nZ - 1;
+    const long long ncell = (long long)cR * cZ, nnode = (long long)nS * nR * nZ;
+    const int per = (g->kind == 2) ? 64 : 16;
+    if (g->kind == 2 && nS > TG_MAX_PLANES) { TG_SET_ERR(ctx, "kind 2: nS <= %d", TG_MAX_PLANES); return TAIGA_E_ARG; }
+    size_t table_n = (size_t)ncell * nS * 3 * per;
+    size_t tcap = ctx->table_bytes / sizeof(double);
+    int rc = tg_reserve(ctx, &ctx->table, &tcap, table_n);
+    ctx->table_bytes = tcap * sizeof(double);
+    if (rc) return rc;
+    cudaStream_t st = ctx->stream;
+    const double* src[3] = {c->BR, c->BZ, c->Bphi};
+    const int TPB = 128;
+
+    if (c->form == 1) {
+        size_t need = (size_t)ncell * nS * per, scap = ctx->scratch_bytes / sizeof(double);
+        if (!c->on_device) { rc = tg_reserve(ctx, &ctx->scratch, &scap, need); ctx->scratch_bytes = scap * sizeof(double); if (rc) return rc; }
+        for (int m = 0; m < 3; ++m) {
+            const double* s = src[m];
+            if (!c->on_device) { TG_CUDA(ctx, cudaMemcpyAsync(ctx->scratch, src[m], need * sizeof(double), cudaMemcpyHostToDevice, st)); s = ctx->scratch; }
+            k_relayout<<<(unsigned)((need + TPB - 1) / TPB), TPB, 0, st>>>(s, ctx->table, g->kind, nS, ncell, m, 1);
+        }
+    } else {
+        // scratch: [nodal(if host)] y | Mz | Myr | Mzr (one component at a time) | pivots | temp bicubic (kind 2) | G
+        size_t n_tmp = (g->kind == 2) ? (size_t)ncell * nS * 48 : 0;
+        size_t need = 4 * (size_t)nnode + nR + nZ + n_tmp + TG_MAX_PLANES, scap = ctx->scratch_bytes / sizeof(double);
+        rc = tg_reserve(ctx, &ctx->scratch, &scap, need);
+        ctx->scratch_bytes = scap * sizeof(double);
+        if (rc) return rc;
+        double *y = ctx->scratch, *Mz = y + nnode, *Myr = Mz + nnode, *Mzr = Myr + nnode;
+        double *cpZ = Mzr + nnode, *cpR = cpZ + nZ, *tmp = cpR + nR, *G = tmp + n_tmp;
+        std::vector<double> pz = thomas_pivots(nZ), pr = thomas_pivots(nR);
+        TG_CUDA(ctx, cudaMemcpyAsync(cpZ, pz.data(), nZ * sizeof(double), cudaMemcpyHostToDevice, st));
+        TG_CUDA(ctx, cudaMemcpyAsync(cpR, pr.data(), nR * sizeof(double), cudaMemcpyHostToDevice, st));
+        std::vector<double> Gh;
+        if (g->kind == 2) { Gh = circulant_inverse_col(nS); TG_CUDA(ctx, cudaMemcpyAsync(G, Gh.data(), nS * sizeof(double), cudaMemcpyHostToDevice, st)); }
+        TG_CUDA(ctx, cudaStreamSynchronize(st));       // host vectors above go out of use
+        for (int m = 0; m < 3; ++m) {
+            const double* yy = src[m];
+            if (!c->on_device) { TG_CUDA(ctx, cudaMemcpyAsync(y, src[m], nnode * sizeof(double), cudaMemcpyHostToDevice, st)); yy = y; }
+            int linesZ = nS * nR, linesR = nS * nZ;
+            // along Z: line (k,i) at (k*nR+i)*nZ, stride 1
+            k_spline_lines<<<(linesZ + TPB - 1) / TPB, TPB, 0, st>>>(yy, Mz, cpZ, nZ, 1, linesZ, nZ, 0, linesZ);
+            // along R: line (k,j) at k*nR*nZ + j, stride nZ  -- of y and of Mz
+            k_spline_lines<<<(linesR + TPB - 1) / TPB, TPB, 0, st>>>(yy, Myr, cpR, nR, nZ, nZ, 1, (long long)nR * nZ, linesR);
+            k_spline_lines<<<(linesR + TPB - 1) / TPB, TPB, 0, st>>>(Mz, Mzr, cpR, nR, nZ, nZ, 1, (long long)nR * nZ, linesR);
+            long long nt = ncell * nS;
+            k_assemble<<<(unsigned)((nt + TPB - 1) / TPB), TPB, 0, st>>>(yy, Mz, Myr, Mzr, g->kind == 2 ? tmp : ctx->table,
+                                                                      nS, nR, nZ, m, g->kind == 2 ? 1 : 0);
+        }
+        if (g->kind == 2) {
+            long long nt = ncell * 48;
+            k_phi_spline<<<(unsigned)((nt + TPB - 1) / TPB), TPB, 0, st>>>(tmp, G, ctx->table, nS, ncell);
+        }
+    }
+    TG_CUDA(ctx, cudaGetLastError());
+    FieldDev& f = ctx->field;
+    f.kind = g->kind; f.nR = nR; f.nZ = nZ; f.nS = nS; f.cR = cR; f.cZ = cZ;
+    f.Rmin = g->Rmin; f.Rmax = g->Rmax; f.Zmin = g->Zmin; f.Zmax = g->Zmax;
+    double hR = (g->Rmax - g->Rmin) / cR, hZ = (g->Zmax - g->Zmin) / cZ;
+    f.inv_hR = 1.0 / hR; f.inv_hZ = 1.0 / hZ;
+    f.offR = g->Rmin / hR; f.offZ = g->Zmin / hZ;
+    f.s0 = g->s0; f.inv_ds = (g->kind == 0) ? 0.0 : 1.0 / g->ds;
+    f.table = ctx->table;
+    return TAIGA_OK;
+}
+
+int tg_field_eval(taiga_ctx* ctx, uint64_t n, const double* R, const double* Z, const double* s, double* BR, double* BZ, double* Bp) {
+    k_field_eval<<<(unsigned)((n + 127) / 128), 128, 0, ctx->stream>>>(ctx->field, n, R, Z, s, BR, BZ, Bp);
+    TG_CUDA(ctx, cudaGetLastError());
+    return TAIGA_OK;
+}
+
+int tg_field_table(taiga_ctx* ctx, int comp, double* host) {
+    const FieldDev& f = ctx->field;
+    int per = (f.kind == 2) ? 64 : 16;
+    long long ncell = (long long)f.cR * f.cZ;
+    size_t need = (size_t)ncell * f.nS * per;
+    double* tmp = nullptr;
+    TG_CUDA(ctx, cudaMalloc((void**)&tmp, need * sizeof(double)));
+    k_relayout<<<(unsigned)((need + 127) / 128), 128, 0, ctx->stream>>>(ctx->table, tmp, f.kind, f.nS, ncell, comp, 0);
+    cudaError_t e = cudaMemcpyAsync(host, tmp, need * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaFree(tmp);
+    TG_CUDA(ctx, e);
+    return TAIGA_OK;
+}

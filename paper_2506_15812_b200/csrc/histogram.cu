@@ -1,0 +1,132 @@
+// a5: binning + Faraday-cup histogram (PAPER.md L330 segment geometry with optional non-uniform
+// size and gaps; L344-350 segment ID or error indicator per ion, atomically summed counters;
+// L352 only the compact counter array goes back to the host).
+//
+// One thread per ion.  Segment search: uniform-pitch guess verified against the real edges
+// (half-open [lo,hi), reading A11), binary search otherwise.  Counting: block-private shared
+// histogram flushed once when the whole matrix fits (<= 8192 counters), else warp-aggregated
+// global atomics (__match_any_sync: one atomic per distinct counter per warp).
+#include "taiga_internal.h"
+
+#define HIST_SMEM_BINS 8192
+#define TG_GRAZE 1e-9
+
+struct HistParams {
+    const double *hit_u, *hit_w;
+    int32_t* cell;
+    uint8_t* flags;
+    const unsigned short* group;
+    unsigned long long n;
+    const double *u_lo, *u_hi, *w_lo, *w_hi;
+    int nu, nw, n_hist;
+    double inv_pu, inv_pw;            // 1/pitch when the axis is uniform with zero gaps, else 0
+    unsigned long long *counts, *summary;
+};
+
+// index of the segment containing v, or -1; sets `graze` when v is within 1e-9 of an edge
+__device__ __forceinline__ int find_segment(const double* __restrict__ lo, const double* __restrict__ hi, int n,
+                                            double inv_pitch, double v, bool& graze) {
+    int k;
+    if (inv_pitch > 0.0) {                      // guess, then verify against the stored edges
+        double g = floor((v - __ldg(lo)) * inv_pitch);
+        k = (g < 0.0) ? -1 : (g >= (double)n ? n - 1 : (int)g);
+        while (k >= 0 && v < __ldg(lo + k)) --k;
+        while (k + 1 < n && v >= __ldg(lo + k + 1)) ++k;
+    } else {                                    // last k with lo[k] <= v
+        int a = -1, b = n;
+        while (b - a > 1) { int m = (a + b) >> 1; if (__ldg(lo + m) <= v) a = m; else b = m; }
+        k = a;
+    }
+    // nearest edges: lo[k], hi[k], lo[k+1] (segments are ordered and non-overlapping)
+    if (k >= 0 && (fabs(v - __ldg(lo + k)) < TG_GRAZE || fabs(v - __ldg(hi + k)) < TG_GRAZE)) graze = true;
+    if (k + 1 < n && fabs(v - __ldg(lo + k + 1)) < TG_GRAZE) graze = true;
+    return (k >= 0 && v < __ldg(hi + k)) ? k : -1;
+}
+
+template <bool SMEM>
+__global__ void __launch_bounds__(256) k_histogram(HistParams P) {
+    __shared__ unsigned int sh[SMEM ? HIST_SMEM_BINS : 1];
+    const int nbins = P.n_hist * P.nw * P.nu;
+    if (SMEM) {
+        for (int b = threadIdx.x; b < nbins; b += blockDim.x) sh[b] = 0u;
+        __syncthreads();
+    }
+    unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    int g = 0, cat = -1, bin = -1;
+    bool flagged = false;
+    if (i < P.n) {
+        g = P.group ? (int)P.group[i] : 0;
+        if (g < P.n_hist) {
+            int st = P.cell[i];
+            uint8_t fl = P.flags[i];
+            if (st >= TAIGA_CELL_MISS) {        // crossed the plane
+                bool gz = false;
+                int iu = find_segment(P.u_lo, P.u_hi, P.nu, P.inv_pu, P.hit_u[i], gz);
+                int iw = find_segment(P.w_lo, P.w_hi, P.nw, P.inv_pw, P.hit_w[i], gz);
+                if (gz) { fl |= TAIGA_FLAG_EDGE; P.flags[i] = fl; }
+                if (iu >= 0 && iw >= 0) { int c = iw * P.nu + iu; P.cell[i] = c; bin = (g * P.nw + iw) * P.nu + iu; cat = 0; }
+                else { P.cell[i] = TAIGA_CELL_MISS; cat = 1; }
+            } else cat = (st == TAIGA_CELL_MAXSTEPS) ? 2 : (st == TAIGA_CELL_OUT ? 3 : 4);
+            flagged = fl != 0;
+        }
+    }
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    // per-segment counters
+    if (SMEM) {
+        if (bin >= 0) atomicAdd(&sh[bin], 1u);
+    } else {
+        unsigned m = __match_any_sync(FULL, bin);
+        if (bin >= 0 && lane == __ffs(m) - 1) atomicAdd(&P.counts[bin], (unsigned long long)__popc(m));
+    }
+    // summary counters {hit, miss, maxsteps, out, badstart, flagged} per histogram
+    int key = (cat >= 0) ? g * 8 + cat : -1;
+    unsigned m1 = __match_any_sync(FULL, key);
+    if (key >= 0 && lane == __ffs(m1) - 1) atomicAdd(&P.summary[(size_t)g * 6 + cat], (unsigned long long)__popc(m1));
+    int key2 = (flagged && cat >= 0) ? g : -1;
+    unsigned m2 = __match_any_sync(FULL, key2);
+    if (key2 >= 0 && lane == __ffs(m2) - 1) atomicAdd(&P.summary[(size_t)g * 6 + 5], (unsigned long long)__popc(m2));
+    if (SMEM) {
+        __syncthreads();
+        for (int b = threadIdx.x; b < nbins; b += blockDim.x) {
+            unsigned v = sh[b];
+            if (v) atomicAdd(&P.counts[b], (unsigned long long)v);
+        }
+    }
+}
+
+static double uniform_inv_pitch(const double* lo, const double* hi, int n) {
+    double pitch = hi[0] - lo[0];
+    for (int k = 0; k < n; ++k) {
+        if (fabs((hi[k] - lo[k]) - pitch) > 1e-12 * fabs(pitch)) return 0.0;
+        if (k + 1 < n && hi[k] != lo[k + 1]) return 0.0;
+    }
+    return 1.0 / pitch;
+}
+
+int tg_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
+                 unsigned long long* counts, unsigned long long* summary) {
+    size_t ne = 2 * ((size_t)det->nu + det->nw), cap = ctx->cap_edges;
+    int rc = tg_reserve(ctx, &ctx->edges, &cap, ne);
+    ctx->cap_edges = (int)cap;
+    if (rc) return rc;
+    cudaStream_t st = ctx->stream;
+    double* e = ctx->edges;
+    TG_CUDA(ctx, cudaMemcpyAsync(e, det->u_lo, det->nu * sizeof(double), cudaMemcpyHostToDevice, st));
+    TG_CUDA(ctx, cudaMemcpyAsync(e + det->nu, det->u_hi, det->nu * sizeof(double), cudaMemcpyHostToDevice, st));
+    TG_CUDA(ctx, cudaMemcpyAsync(e + 2 * det->nu, det->w_lo, det->nw * sizeof(double), cudaMemcpyHostToDevice, st));
+    TG_CUDA(ctx, cudaMemcpyAsync(e + 2 * det->nu + det->nw, det->w_hi, det->nw * sizeof(double), cudaMemcpyHostToDevice, st));
+    HistParams P;
+    P.hit_u = ions->hit_u; P.hit_w = ions->hit_w; P.cell = ions->cell; P.flags = ions->flags; P.group = ions->group;
+    P.n = ions->n;
+    P.u_lo = e; P.u_hi = e + det->nu; P.w_lo = e + 2 * det->nu; P.w_hi = e + 2 * det->nu + det->nw;
+    P.nu = det->nu; P.nw = det->nw; P.n_hist = n_hist;
+    P.inv_pu = uniform_inv_pitch(det->u_lo, det->u_hi, det->nu);
+    P.inv_pw = uniform_inv_pitch(det->w_lo, det->w_hi, det->nw);
+    P.counts = counts; P.summary = summary;
+    unsigned blocks = (unsigned)((ions->n + 255) / 256);
+    if ((long long)n_hist * det->nw * det->nu <= HIST_SMEM_BINS) k_histogram<true><<<blocks, 256, 0, st>>>(P);
+    else k_histogram<false><<<blocks, 256, 0, st>>>(P);
+    TG_CUDA(ctx, cudaGetLastError());
+    return TAIGA_OK;
+}

@@ -1,0 +1,191 @@
+// C ABI entry points: argument validation, context lifetime, dispatch (include/taiga.h).
+#include <math.h>
+#include <new>
+
+#include "taiga_internal.h"
+
+static bool orthonormal(const double a[3], const double b[3], const double c[3]) {
+    auto dot = [](const double* p, const double* q) { return p[0] * q[0] + p[1] * q[1] + p[2] * q[2]; };
+    const double tol = 1e-12;
+    return fabs(dot(a, a) - 1) < tol && fabs(dot(b, b) - 1) < tol && fabs(dot(c, c) - 1) < tol &&
+           fabs(dot(a, b)) < tol && fabs(dot(a, c)) < tol && fabs(dot(b, c)) < tol;
+}
+
+static bool cdf_ok(const double* F, int K) {
+    if (!F || K < 1 || F[0] != 0.0 || F[K] != 1.0) return false;
+    for (int i = 0; i < K; ++i) if (!(F[i] <= F[i + 1])) return false;
+    return true;
+}
+
+extern "C" int taiga_create(taiga_ctx** out, int device, void* cuda_stream) {
+    if (!out) return TAIGA_E_ARG;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return TAIGA_E_CUDA;
+    taiga_ctx* ctx = new (std::nothrow) taiga_ctx();
+    if (!ctx) return TAIGA_E_NOMEM;
+    memset(ctx, 0, sizeof(*ctx));
+    ctx->device = device;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    if (cudaSetDevice(device) != cudaSuccess) { delete ctx; return TAIGA_E_CUDA; }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { delete ctx; return TAIGA_E_CUDA; }
+    if (prop.major < 10) { delete ctx; return TAIGA_E_CUDA; }     // sm_100a code only
+    ctx->sm_count = prop.multiProcessorCount;
+    if (cudaMalloc((void**)&ctx->counters, 16 * sizeof(unsigned long long)) != cudaSuccess ||
+        cudaMallocHost((void**)&ctx->counters_host, 16 * sizeof(unsigned long long)) != cudaSuccess) {
+        delete ctx; return TAIGA_E_NOMEM;
+    }
+    ctx->opt_sort = 1; ctx->opt_sort_sub = 4;
+    ctx->opt_chunk0 = 0; ctx->opt_chunk = 2048; ctx->opt_min_active = 12;
+    ctx->opt_ctas_per_sm = 0; ctx->opt_variant = 0; ctx->opt_stats = 1;
+    strcpy(ctx->err, "ok");
+    *out = ctx;
+    return TAIGA_OK;
+}
+
+extern "C" int taiga_destroy(taiga_ctx* ctx) {
+    if (!ctx) return TAIGA_E_ARG;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    void* bufs[] = {ctx->table, ctx->scratch, ctx->cdf_depth, ctx->cdf_normal, ctx->edges, ctx->order,
+                    ctx->bins, ctx->surv[0], ctx->surv[1], ctx->surv_idx[0], ctx->surv_idx[1],
+                    ctx->surv_steps[0], ctx->surv_steps[1], ctx->counters};
+    for (void* b : bufs) if (b) cudaFree(b);
+    if (ctx->counters_host) cudaFreeHost(ctx->counters_host);
+    delete ctx;
+    return TAIGA_OK;
+}
+
+extern "C" const char* taiga_last_error(const taiga_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+extern "C" int taiga_load_field(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c) {
+    if (!ctx) return TAIGA_E_ARG;
+    if (!g || !c || !c->BR || !c->BZ || !c->Bphi) { TG_SET_ERR(ctx, "load_field: null argument"); return TAIGA_E_ARG; }
+    if (g->kind < 0 || g->kind > 2 || g->nR < 4 || g->nZ < 4 || !(g->Rmax > g->Rmin) || !(g->Zmax > g->Zmin) ||
+        !(g->Rmin > 0.0) || (g->kind == 0 && g->nS != 1) || (g->kind == 1 && g->nS < 2) ||
+        (g->kind == 2 && g->nS < 3) || (g->kind != 0 && !(g->ds > 0.0)) || (c->form != 0 && c->form != 1)) {
+        TG_SET_ERR(ctx, "load_field: bad grid (kind=%d nR=%d nZ=%d nS=%d form=%d)", g->kind, g->nR, g->nZ, g->nS, c->form);
+        return TAIGA_E_ARG;
+    }
+    TG_CUDA(ctx, cudaSetDevice(ctx->device));
+    ctx->field_loaded = false;
+    int rc = tg_precompute(ctx, g, c);
+    if (rc == TAIGA_OK) ctx->field_loaded = true;
+    return rc;
+}
+
+extern "C" int taiga_field_eval(taiga_ctx* ctx, uint64_t n, const double* R, const double* Z, const double* s,
+                                double* BR, double* BZ, double* Bp) {
+    if (!ctx) return TAIGA_E_ARG;
+    if (!ctx->field_loaded) { TG_SET_ERR(ctx, "field_eval before load_field"); return TAIGA_E_STATE; }
+    if (n && (!R || !Z || !BR || !BZ || !Bp)) { TG_SET_ERR(ctx, "field_eval: null argument"); return TAIGA_E_ARG; }
+    TG_CUDA(ctx, cudaSetDevice(ctx->device));
+    return n ? tg_field_eval(ctx, n, R, Z, s, BR, BZ, Bp) : TAIGA_OK;
+}
+
+extern "C" int taiga_field_table(taiga_ctx* ctx, int comp, double* host) {
+    if (!ctx) return TAIGA_E_ARG;
+    if (!ctx->field_loaded) { TG_SET_ERR(ctx, "field_table before load_field"); return TAIGA_E_STATE; }
+    if (comp < 0 || comp > 2 || !host) { TG_SET_ERR(ctx, "field_table: bad argument"); return TAIGA_E_ARG; }
+    TG_CUDA(ctx, cudaSetDevice(ctx->device));
+    return tg_field_table(ctx, comp, host);
+}
+
+static int check_ions(taiga_ctx* ctx, const taiga_ions* ions, bool need_out) {
+    if (!ions) { TG_SET_ERR(ctx, "null ions"); return TAIGA_E_ARG; }
+    if (ions->n >= (1ull << 32)) { TG_SET_ERR(ctx, "ions->n must be < 2^32"); return TAIGA_E_ARG; }
+    if (ions->n == 0) return TAIGA_OK;
+    if (!ions->x || !ions->y || !ions->z || !ions->vx || !ions->vy || !ions->vz) { TG_SET_ERR(ctx, "null ion state array"); return TAIGA_E_ARG; }
+    if (need_out && (!ions->hit_u || !ions->hit_w || !ions->cell || !ions->steps || !ions->flags)) {
+        TG_SET_ERR(ctx, "null ion result array"); return TAIGA_E_ARG;
+    }
+    return TAIGA_OK;
+}
+
+extern "C" int taiga_seed_beam(taiga_ctx* ctx, const taiga_beam_params* p, uint64_t seed, taiga_ions* ions) {
+    if (!ctx) return TAIGA_E_ARG;
+    if (!p) { TG_SET_ERR(ctx, "seed_beam: null params"); return TAIGA_E_ARG; }
+    int rc = check_ions(ctx, ions, false);
+    if (rc) return rc;
+    if (!(p->mass_kg > 0) || !(p->charge_C != 0) || !(p->energy_eV > 0) || !(p->depth_max > 0) || !(p->z_max > 0) ||
+        p->sigma_pos_m < 0 || p->sigma_ang_rad < 0) { TG_SET_ERR(ctx, "seed_beam: bad beam parameters"); return TAIGA_E_ARG; }
+    if (!orthonormal(p->axis, p->eT, p->eZ)) { TG_SET_ERR(ctx, "seed_beam: (axis,eT,eZ) not orthonormal"); return TAIGA_E_ARG; }
+    if (!cdf_ok(p->cdf_depth, p->n_depth) || !cdf_ok(p->cdf_normal, p->n_normal)) {
+        TG_SET_ERR(ctx, "seed_beam: CDF table must have F[0]=0, F[K]=1 and be non-decreasing"); return TAIGA_E_ARG;
+    }
+    if (ions->n == 0) return TAIGA_OK;
+    TG_CUDA(ctx, cudaSetDevice(ctx->device));
+    double v0 = sqrt(2.0 * p->energy_eV * fabs(p->charge_C) / p->mass_kg);   // IEEE sqrt, host
+    return tg_seed(ctx, p, seed, ions, v0);
+}
+
+static int check_det(taiga_ctx* ctx, const taiga_detector* d, bool need_edges) {
+    if (!d) { TG_SET_ERR(ctx, "null detector"); return TAIGA_E_ARG; }
+    if (!orthonormal(d->normal, d->eu, d->ew)) { TG_SET_ERR(ctx, "detector: (normal,eu,ew) not orthonormal"); return TAIGA_E_ARG; }
+    if (!need_edges) return TAIGA_OK;
+    if (d->nu < 1 || d->nw < 1 || d->nu > 4096 || d->nw > 4096 || !d->u_lo || !d->u_hi || !d->w_lo || !d->w_hi) {
+        TG_SET_ERR(ctx, "detector: bad segment arrays"); return TAIGA_E_ARG;
+    }
+    for (int ax = 0; ax < 2; ++ax) {
+        const double *lo = ax ? d->w_lo : d->u_lo, *hi = ax ? d->w_hi : d->u_hi;
+        int n = ax ? d->nw : d->nu;
+        for (int k = 0; k < n; ++k)
+            if (!(lo[k] < hi[k]) || (k + 1 < n && !(hi[k] <= lo[k + 1]))) {
+                TG_SET_ERR(ctx, "detector: segments must be ordered and non-overlapping"); return TAIGA_E_ARG;
+            }
+    }
+    return TAIGA_OK;
+}
+
+extern "C" int taiga_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t max_steps,
+                           const taiga_detector* det, int variant) {
+    if (!ctx) return TAIGA_E_ARG;
+    if (!ctx->field_loaded) { TG_SET_ERR(ctx, "trace before load_field"); return TAIGA_E_STATE; }
+    int rc = check_ions(ctx, ions, true);
+    if (rc) return rc;
+    rc = check_det(ctx, det, false);
+    if (rc) return rc;
+    if (!(dt > 0) || !isfinite(qm) || qm == 0 || (variant != 0 && variant != 1)) { TG_SET_ERR(ctx, "trace: bad dt / q_over_m / variant"); return TAIGA_E_ARG; }
+    if (ions->n == 0) return TAIGA_OK;
+    TG_CUDA(ctx, cudaSetDevice(ctx->device));
+    DetDev dd;
+    for (int c = 0; c < 3; ++c) { dd.origin[c] = det->origin[c]; dd.normal[c] = det->normal[c]; dd.eu[c] = det->eu[c]; dd.ew[c] = det->ew[c]; }
+    return tg_trace(ctx, ions, qm, dt, max_steps, dd, variant);
+}
+
+extern "C" int taiga_detector_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
+                                        unsigned long long* counts, unsigned long long* summary) {
+    if (!ctx) return TAIGA_E_ARG;
+    int rc = check_ions(ctx, ions, true);
+    if (rc) return rc;
+    rc = check_det(ctx, det, true);
+    if (rc) return rc;
+    if (n_hist < 1 || n_hist > 65536 || !counts || !summary) { TG_SET_ERR(ctx, "histogram: bad n_hist / null output"); return TAIGA_E_ARG; }
+    if (ions->n == 0) return TAIGA_OK;
+    TG_CUDA(ctx, cudaSetDevice(ctx->device));
+    return tg_histogram(ctx, ions, det, n_hist, counts, summary);
+}
+
+extern "C" int taiga_set_option(taiga_ctx* ctx, const char* key, long long v) {
+    if (!ctx || !key) return TAIGA_E_ARG;
+    struct { const char* k; int* p; } tab[] = {
+        {"sort", &ctx->opt_sort}, {"sort_sub", &ctx->opt_sort_sub}, {"chunk0", &ctx->opt_chunk0},
+        {"chunk", &ctx->opt_chunk}, {"min_active", &ctx->opt_min_active},
+        {"ctas_per_sm", &ctx->opt_ctas_per_sm}, {"variant", &ctx->opt_variant}, {"stats", &ctx->opt_stats}};
+    for (auto& t : tab) if (!strcmp(key, t.k)) { *t.p = (int)v; return TAIGA_OK; }
+    TG_SET_ERR(ctx, "set_option: unknown key '%s'", key);
+    return TAIGA_E_ARG;
+}
+
+extern "C" int taiga_get_stats(taiga_ctx* ctx, unsigned long long out[8]) {
+    if (!ctx || !out) return TAIGA_E_ARG;
+    for (int i = 0; i < 8; ++i) out[i] = ctx->stats[i];
+    return TAIGA_OK;
+}
+
+extern "C" int taiga_measure_fp64_peak(taiga_ctx* ctx, double ms, double* rate) {
+    if (!ctx || !rate || !(ms > 0)) return TAIGA_E_ARG;
+    TG_CUDA(ctx, cudaSetDevice(ctx->device));
+    return tg_fp64_peak(ctx, ms, rate);
+}

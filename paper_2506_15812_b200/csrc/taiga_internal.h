@@ -1,0 +1,94 @@
+// Internal declarations of libtaiga (sm_100a).  Not part of the ABI.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/taiga.h"
+
+// Grid geometry as the kernels want it (derived once in taiga_load_field).
+struct FieldDev {
+    int kind, nR, nZ, nS;            // nodes
+    int cR, cZ;                      // cells
+    double Rmin, Rmax, Zmin, Zmax;
+    double inv_hR, inv_hZ;           // 1/h
+    double offR, offZ;               // Rmin/hR, Zmin/hZ   (p_total = R*inv_hR - offR)
+    double s0, inv_ds;
+    // kind 0: [iR][iZ][comp][16]            (384 B per cell, one 128-B line per component)
+    // kind 1: [iR][iZ][slice][comp][16]     (the two slices of a cell are adjacent)
+    // kind 2: [iphi][iR][iZ][comp][64]
+    const double* table;
+};
+
+struct DetDev {
+    double origin[3], normal[3], eu[3], ew[3];
+};
+
+struct taiga_ctx {
+    int device;
+    cudaStream_t stream;
+    char err[512];
+    int sm_count;
+
+    // field
+    bool field_loaded;
+    FieldDev field;
+    double* table;            size_t table_bytes;
+    double* scratch;          size_t scratch_bytes;     // precompute work arrays
+
+    // seeding tables
+    double *cdf_depth, *cdf_normal;  int cap_depth, cap_normal;
+
+    // detector edges (histogram)
+    double* edges;            int cap_edges;
+
+    // trace scratch
+    uint32_t* order;          size_t cap_order;          // permutation (sorted by birth cell)
+    uint32_t* bins;           size_t cap_bins;           // counting-sort bins
+    double* surv[2];          size_t cap_surv;           // survivor state, ping-pong: 7 doubles/ion
+    uint32_t* surv_idx[2];
+    uint32_t* surv_steps[2];
+    unsigned long long* counters;                        // device counters (16)
+    unsigned long long* counters_host;                   // pinned mirror
+    unsigned long long stats[8];
+
+    // options
+    int opt_sort, opt_chunk0, opt_chunk, opt_min_active, opt_ctas_per_sm, opt_variant, opt_stats;
+    int opt_sort_sub;
+};
+
+#define TG_SET_ERR(ctx, ...) snprintf((ctx)->err, sizeof((ctx)->err), __VA_ARGS__)
+
+#define TG_CUDA(ctx, call)                                                            \
+    do {                                                                              \
+        cudaError_t e_ = (call);                                                      \
+        if (e_ != cudaSuccess) {                                                      \
+            TG_SET_ERR(ctx, "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+            return (e_ == cudaErrorMemoryAllocation) ? TAIGA_E_NOMEM : TAIGA_E_CUDA;  \
+        }                                                                             \
+    } while (0)
+
+// grow-only device buffer
+template <typename T>
+static inline int tg_reserve(taiga_ctx* ctx, T** p, size_t* cap, size_t need) {
+    if (*cap >= need && *p) return TAIGA_OK;
+    if (*p) cudaFree(*p);
+    *p = nullptr; *cap = 0;
+    cudaError_t e = cudaMalloc((void**)p, need * sizeof(T));
+    if (e != cudaSuccess) { TG_SET_ERR(ctx, "cudaMalloc(%zu B): %s", need * sizeof(T), cudaGetErrorString(e)); return TAIGA_E_NOMEM; }
+    *cap = need;
+    return TAIGA_OK;
+}
+
+// implemented in the per-kernel translation units
+int tg_precompute(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c);
+int tg_seed(taiga_ctx* ctx, const taiga_beam_params* p, uint64_t seed, taiga_ions* ions, double v0);
+int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t max_steps,
+             const DetDev& det, int variant);
+int tg_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
+                 unsigned long long* counts, unsigned long long* summary);
+int tg_field_eval(taiga_ctx* ctx, uint64_t n, const double* R, const double* Z, const double* s,
+                  double* BR, double* BZ, double* Bp);
+int tg_field_table(taiga_ctx* ctx, int comp, double* host);
+int tg_fp64_peak(taiga_ctx* ctx, double ms, double* rate);

@@ -1,0 +1,392 @@
+// a3 + a4: Runge-Kutta-Nystrom integrator, termination and plane interpolation.
+//
+// PAPER.md Eq. 3 (L172) with E = 0; Eq. 5-6 (L218-235) under readings A1-A3:
+//   k1 = a(r, v);  k2 = a(r + v dt/2 + k1 dt^2/8, v + k1 dt/2);
+//   k3 = a(r + v dt/2 + K dt^2/8, v + k2 dt/2), K = k1 (classical) | k2 (printed Eq. 6);
+//   k4 = a(r + v dt + k3 dt^2/2, v + k3 dt);
+//   r' = r + v dt + (k1+k2+k3) dt^2/6;   v' = v + (k1+2k2+2k3+k4) dt/6.
+// L326/L338: stop at the detector plane, linear interpolation from the previous step;
+// L318: error value for trapped / unreachable ions.
+//
+// B200 design (not the paper's one-thread-per-ion launch):
+//  * one persistent kernel, 8 warps per SM; each LANE owns one ion whose state lives in
+//    registers; finished lanes are refilled from a global queue of ions ordered by birth cell
+//    (deep-born = long-running ions first), so warps stay full through the long tail and the
+//    ions sharing a warp sit in the same few field cells;
+//  * the velocity is carried as u = (q/m) v, so a = u x B needs no scaling per evaluation;
+//  * classical variant: k2 and k3 share their position, so B is evaluated 3x, not 4x, per step;
+//  * kind 0 (static 2-D): the 48 coefficients of the lane's current cell are cached in
+//    registers and re-read (24 x 128-bit loads, one 128-B line per component) only when the
+//    lane leaves the cell (~0.35 times per step);
+//  * 1/R by MUFU.RSQ64H seed + one cubic (Halley) step: 6 FP64 instructions instead of ~30.
+#include "field_device.cuh"
+
+struct TraceParams {
+    FieldDev f;
+    DetDev det;
+    double nrD;                       // normal . origin
+    double a1, a2, b1;                // dt/(2 qm), dt^2/8, qm dt/2   (stage 2/3)
+    double c6, d6, dtq;               // dt^2/6, qm dt/6, dt/qm
+    double qm, dt;
+    uint32_t max_steps, n;
+    int variant, refill_min;
+    const double *x, *y, *z, *vx, *vy, *vz, *t0;
+    const uint32_t* order;
+    double *hit_u, *hit_w;
+    int32_t* cell;
+    uint32_t* steps;
+    uint8_t* flags;
+    unsigned long long* counters;     // [0] queue head, [1] warp-steps, [2] reloads, [3] ion-steps
+};
+
+#define TG_GRAZE 1e-9
+
+__device__ __forceinline__ double tg_rsqrt(double a) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+    double e = fma(-(a * y), y, 1.0);          // 1 - a y^2, |e| <~ 2^-22
+    double q = fma(0.375, e, 0.5);
+    return fma(y * e, q, y);                   // y (1 + e/2 + 3 e^2/8): cubic convergence
+}
+
+// t in [0,1)  <=>  sign 0 and exponent < 1023  <=>  (unsigned) hi word < 0x3FF00000
+__device__ __forceinline__ bool tg_in01(double t) { return (unsigned)__double2hiint(t) < 0x3FF00000u; }
+
+template <int KIND>
+struct CellCache;                              // register cache of the current cell (kind 0)
+template <>
+struct CellCache<0> {
+    double c[48];
+    double oR, oZ;                             // offR + i, offZ + j of the cached cell
+};
+template <>
+struct CellCache<1> {};
+template <>
+struct CellCache<2> {};
+
+__device__ __forceinline__ double tg_horner16(const double* c, double p, double w) {
+    double r0 = fma(fma(fma(c[3], w, c[2]), w, c[1]), w, c[0]);
+    double r1 = fma(fma(fma(c[7], w, c[6]), w, c[5]), w, c[4]);
+    double r2 = fma(fma(fma(c[11], w, c[10]), w, c[9]), w, c[8]);
+    double r3 = fma(fma(fma(c[15], w, c[14]), w, c[13]), w, c[12]);
+    return fma(fma(fma(r3, p, r2), p, r1), p, r0);
+}
+
+// Cartesian B at (X,Y,Z,t) given R2 = X^2+Y^2, rinv = 1/R, R.
+template <int KIND, bool CACHED>
+__device__ __forceinline__ void tg_fieldB(const TraceParams& P, CellCache<KIND>& cc, int& reloads, double X, double Y,
+                                          double Z, double t, double R, double rinv, double& Bx, double& By, double& Bz) {
+    double BR, BZ, Bp;
+    if constexpr (KIND == 0 && CACHED) {
+        double tR = fma(R, P.f.inv_hR, -cc.oR), tZ = fma(Z, P.f.inv_hZ, -cc.oZ);
+        if (!(tg_in01(tR) && tg_in01(tZ))) {
+            double pR = fma(R, P.f.inv_hR, -P.f.offR), pZ = fma(Z, P.f.inv_hZ, -P.f.offZ);
+            int i = tg_clampi(__double2int_rd(pR), 0, P.f.cR - 1), j = tg_clampi(__double2int_rd(pZ), 0, P.f.cZ - 1);
+            cc.oR = P.f.offR + (double)i; cc.oZ = P.f.offZ + (double)j;
+            const double2* src = reinterpret_cast<const double2*>(P.f.table + ((size_t)i * P.f.cZ + j) * 48);
+#pragma unroll
+            for (int k = 0; k < 24; ++k) { double2 v = __ldg(src + k); cc.c[2 * k] = v.x; cc.c[2 * k + 1] = v.y; }
+            tR = fma(R, P.f.inv_hR, -cc.oR); tZ = fma(Z, P.f.inv_hZ, -cc.oZ);
+            ++reloads;
+        }
+        BR = tg_horner16(cc.c, tR, tZ); BZ = tg_horner16(cc.c + 16, tR, tZ); Bp = tg_horner16(cc.c + 32, tR, tZ);
+    } else {
+        double s = t;
+        if constexpr (KIND == 2) s = atan2(Y, X);
+        tg_field_cyl(P.f, R, Z, s, BR, BZ, Bp);
+    }
+    double c = X * rinv, s_ = Y * rinv;        // O0: B_X = B_R c - B_phi s, B_Y = B_R s + B_phi c
+    Bx = fma(BR, c, -(Bp * s_));
+    By = fma(BR, s_, Bp * c);
+    Bz = BZ;
+}
+
+template <int KIND, bool CACHED>
+__global__ void __launch_bounds__(128, 2) k_trace(const TraceParams P) {
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    CellCache<KIND> cc;
+    if constexpr (KIND == 0 && CACHED) { cc.oR = 1e300; cc.oZ = 1e300;
+#pragma unroll
+        for (int k = 0; k < 48; ++k) cc.c[k] = 0.0; }
+    double X = 0, Y = 0, Z = 0, Ux = 0, Uy = 0, Uz = 0, t = 0, s0 = -1.0;
+    uint32_t idx = 0, nst = 0;
+    bool alive = false, exhausted = false;
+    int reloads = 0;
+    unsigned long long warp_steps = 0, ion_steps = 0;
+
+    while (true) {
+        unsigned freem = __ballot_sync(FULL, !alive);
+        int nfree = __popc(freem);
+        if (!exhausted && (nfree >= P.refill_min || nfree == 32)) {
+            unsigned long long base = 0;
+            if (lane == 0) base = atomicAdd(&P.counters[0], (unsigned long long)nfree);
+            base = __shfl_sync(FULL, base, 0);
+            if (base + nfree >= P.n) exhausted = true;
+            unsigned long long q = base + __popc(freem & ((1u << lane) - 1u));
+            if (!alive && q < P.n) {
+                idx = P.order ? P.order[q] : (uint32_t)q;
+                X = P.x[idx]; Y = P.y[idx]; Z = P.z[idx];
+                Ux = P.qm * P.vx[idx]; Uy = P.qm * P.vy[idx]; Uz = P.qm * P.vz[idx];
+                t = P.t0 ? P.t0[idx] : 0.0;
+                nst = 0;
+                s0 = fma(P.det.normal[0], X, fma(P.det.normal[1], Y, fma(P.det.normal[2], Z, -P.nrD)));
+                alive = true;
+                if (!(s0 < 0.0)) {             // O4: must start in front of the plane
+                    P.hit_u[idx] = 0.0; P.hit_w[idx] = 0.0; P.cell[idx] = TAIGA_CELL_BADSTART; P.steps[idx] = 0;
+                    P.flags[idx] = (fabs(s0) < TG_GRAZE) ? TAIGA_FLAG_PLANE : 0;
+                    alive = false;
+                }
+            }
+        }
+        if (!__any_sync(FULL, alive)) { if (exhausted) break; else continue; }
+        ++warp_steps;
+        if (alive) {
+            // ---- stage 1 at (r, u); R of r also serves the out-of-grid test of the previous step
+            double R2 = fma(X, X, Y * Y), rinv = tg_rsqrt(R2), R = R2 * rinv;
+            bool outside = (R < P.f.Rmin) | (R > P.f.Rmax) | (Z < P.f.Zmin) | (Z > P.f.Zmax);
+            if (outside || nst == P.max_steps) {
+                uint8_t fl = 0;
+                if (outside && (fabs(R - P.f.Rmin) < TG_GRAZE || fabs(R - P.f.Rmax) < TG_GRAZE ||
+                                fabs(Z - P.f.Zmin) < TG_GRAZE || fabs(Z - P.f.Zmax) < TG_GRAZE)) fl = TAIGA_FLAG_GRID;
+                P.hit_u[idx] = 0.0; P.hit_w[idx] = 0.0;
+                P.cell[idx] = outside ? (nst == 0 ? TAIGA_CELL_BADSTART : TAIGA_CELL_OUT) : TAIGA_CELL_MAXSTEPS;
+                P.steps[idx] = nst; P.flags[idx] = fl;
+                alive = false;
+            } else {
+                double Bx, By, Bz;
+                tg_fieldB<KIND, CACHED>(P, cc, reloads, X, Y, Z, t, R, rinv, Bx, By, Bz);
+                double k1x = fma(Uy, Bz, -(Uz * By)), k1y = fma(Uz, Bx, -(Ux * Bz)), k1z = fma(Ux, By, -(Uy * Bx));
+                // ---- stage 2 (and 3, classical: same position)
+                double Xm = fma(k1x, P.a2, fma(Ux, P.a1, X)), Ym = fma(k1y, P.a2, fma(Uy, P.a1, Y)), Zm = fma(k1z, P.a2, fma(Uz, P.a1, Z));
+                double ux = fma(k1x, P.b1, Ux), uy = fma(k1y, P.b1, Uy), uz = fma(k1z, P.b1, Uz);
+                double tm = t + 0.5 * P.dt;
+                R2 = fma(Xm, Xm, Ym * Ym); rinv = tg_rsqrt(R2); R = R2 * rinv;
+                tg_fieldB<KIND, CACHED>(P, cc, reloads, Xm, Ym, Zm, tm, R, rinv, Bx, By, Bz);
+                double k2x = fma(uy, Bz, -(uz * By)), k2y = fma(uz, Bx, -(ux * Bz)), k2z = fma(ux, By, -(uy * Bx));
+                ux = fma(k2x, P.b1, Ux); uy = fma(k2y, P.b1, Uy); uz = fma(k2z, P.b1, Uz);
+                if (P.variant) {               // printed Eq. 6: k3 position increment from k2
+                    Xm = fma(k2x, P.a2, fma(Ux, P.a1, X)); Ym = fma(k2y, P.a2, fma(Uy, P.a1, Y)); Zm = fma(k2z, P.a2, fma(Uz, P.a1, Z));
+                    R2 = fma(Xm, Xm, Ym * Ym); rinv = tg_rsqrt(R2); R = R2 * rinv;
+                    tg_fieldB<KIND, false>(P, cc, reloads, Xm, Ym, Zm, tm, R, rinv, Bx, By, Bz);
+                }
+                double k3x = fma(uy, Bz, -(uz * By)), k3y = fma(uz, Bx, -(ux * Bz)), k3z = fma(ux, By, -(uy * Bx));
+                // ---- stage 4
+                double Xe = fma(k3x, 4.0 * P.a2, fma(Ux, 2.0 * P.a1, X)), Ye = fma(k3y, 4.0 * P.a2, fma(Uy, 2.0 * P.a1, Y)),
+                       Ze = fma(k3z, 4.0 * P.a2, fma(Uz, 2.0 * P.a1, Z));
+                ux = fma(k3x, 2.0 * P.b1, Ux); uy = fma(k3y, 2.0 * P.b1, Uy); uz = fma(k3z, 2.0 * P.b1, Uz);
+                R2 = fma(Xe, Xe, Ye * Ye); rinv = tg_rsqrt(R2); R = R2 * rinv;
+                tg_fieldB<KIND, CACHED>(P, cc, reloads, Xe, Ye, Ze, t + P.dt, R, rinv, Bx, By, Bz);
+                double k4x = fma(uy, Bz, -(uz * By)), k4y = fma(uz, Bx, -(ux * Bz)), k4z = fma(ux, By, -(uy * Bx));
+                // ---- Eq. 5
+                double Tx = k2x + k3x, Ty = k2y + k3y, Tz = k2z + k3z;
+                double Xn = fma(k1x + Tx, P.c6, fma(Ux, P.dtq, X)), Yn = fma(k1y + Ty, P.c6, fma(Uy, P.dtq, Y)),
+                       Zn = fma(k1z + Tz, P.c6, fma(Uz, P.dtq, Z));
+                Ux = fma(fma(2.0, Tx, k1x + k4x), P.d6, Ux);
+                Uy = fma(fma(2.0, Ty, k1y + k4y), P.d6, Uy);
+                Uz = fma(fma(2.0, Tz, k1z + k4z), P.d6, Uz);
+                ++nst; ++ion_steps;
+                double s1 = fma(P.det.normal[0], Xn, fma(P.det.normal[1], Yn, fma(P.det.normal[2], Zn, -P.nrD)));
+                if (s1 >= 0.0) {               // O4: s0 < 0 <= s1 -> interpolate to the plane (L326, L338)
+                    double lam = s0 / (s0 - s1);
+                    double px = fma(lam, Xn - X, X) - P.det.origin[0], py = fma(lam, Yn - Y, Y) - P.det.origin[1],
+                           pz = fma(lam, Zn - Z, Z) - P.det.origin[2];
+                    P.hit_u[idx] = fma(px, P.det.eu[0], fma(py, P.det.eu[1], pz * P.det.eu[2]));
+                    P.hit_w[idx] = fma(px, P.det.ew[0], fma(py, P.det.ew[1], pz * P.det.ew[2]));
+                    P.cell[idx] = TAIGA_CELL_MISS;      // segment assigned by the histogram kernel (a5)
+                    P.steps[idx] = nst;
+                    P.flags[idx] = (fabs(s0) < TG_GRAZE || fabs(s1) < TG_GRAZE) ? TAIGA_FLAG_PLANE : 0;
+                    alive = false;
+                }
+                X = Xn; Y = Yn; Z = Zn; t += P.dt; s0 = s1;
+            }
+        }
+    }
+    // per-warp statistics
+    unsigned long long ws = warp_steps;
+    for (int o = 16; o > 0; o >>= 1) {
+        reloads += __shfl_down_sync(FULL, reloads, o);
+        ion_steps += __shfl_down_sync(FULL, ion_steps, o);
+    }
+    if (lane == 0) {
+        atomicAdd(&P.counters[1], ws);
+        atomicAdd(&P.counters[2], (unsigned long long)reloads);
+        atomicAdd(&P.counters[3], ion_steps);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Ordering of the ion queue: counting sort by birth cell (R-major, so that deep-born = long
+// running ions are dequeued first and the ions sharing a warp fly through the same cells).
+// Output is written by ion index, so the order never shows in the results.
+#define SORT_NBR 512
+#define SORT_NBZ 256
+#define SCAN_ITEMS 8
+#define SCAN_TPB 1024
+
+struct SortParams {
+    const double *x, *y, *z, *t0;
+    uint32_t n;
+    double Rmin, Zmin, minwR, minwZ, s0, inv_ds;
+    int n_major, nS;
+    unsigned long long* bbox;          // [4]: min a, max a, min b, max b (bit patterns of doubles >= 0)
+};
+
+__device__ __forceinline__ void sort_ab(const SortParams& S, uint32_t i, double& a, double& b) {
+    double X = S.x[i], Y = S.y[i];
+    a = fmax(sqrt(fma(X, X, Y * Y)) - S.Rmin, 0.0);
+    b = fmax(S.z[i] - S.Zmin, 0.0);
+    if (!(a < 1e30)) a = 0.0;          // NaN / inf guards
+    if (!(b < 1e30)) b = 0.0;
+}
+
+__global__ void k_sort_bbox(SortParams S) {
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    double a = 0, b = 0;
+    bool v = i < S.n;
+    if (v) sort_ab(S, i, a, b);
+    unsigned long long amin = v ? (unsigned long long)__double_as_longlong(a) : ~0ull, amax = v ? (unsigned long long)__double_as_longlong(a) : 0ull;
+    unsigned long long bmin = v ? (unsigned long long)__double_as_longlong(b) : ~0ull, bmax = v ? (unsigned long long)__double_as_longlong(b) : 0ull;
+    for (int o = 16; o > 0; o >>= 1) {
+        amin = min(amin, __shfl_xor_sync(0xffffffffu, amin, o)); amax = max(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+        bmin = min(bmin, __shfl_xor_sync(0xffffffffu, bmin, o)); bmax = max(bmax, __shfl_xor_sync(0xffffffffu, bmax, o));
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicMin(&S.bbox[0], amin); atomicMax(&S.bbox[1], amax);
+        atomicMin(&S.bbox[2], bmin); atomicMax(&S.bbox[3], bmax);
+    }
+}
+
+__device__ __forceinline__ uint32_t sort_key(const SortParams& S, uint32_t i) {
+    double a, b;
+    sort_ab(S, i, a, b);
+    double a0 = __longlong_as_double((long long)S.bbox[0]), a1 = __longlong_as_double((long long)S.bbox[1]);
+    double b0 = __longlong_as_double((long long)S.bbox[2]), b1 = __longlong_as_double((long long)S.bbox[3]);
+    double wR = fmax((a1 - a0) / SORT_NBR, S.minwR), wZ = fmax((b1 - b0) / SORT_NBZ, S.minwZ);
+    int bR = min(max((int)((a - a0) / wR), 0), SORT_NBR - 1), bZ = min(max((int)((b - b0) / wZ), 0), SORT_NBZ - 1);
+    int m = 0;
+    if (S.n_major > 1 && S.t0) {
+        int k = min(max((int)floor((S.t0[i] - S.s0) * S.inv_ds), 0), S.nS - 1);
+        m = (int)(((long long)k * S.n_major) / S.nS);
+    }
+    return (uint32_t)((m * SORT_NBR + bR) * SORT_NBZ + bZ);
+}
+
+__global__ void k_sort_count(SortParams S, uint32_t* bins) {
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < S.n) atomicAdd(&bins[sort_key(S, i)], 1u);
+}
+
+// exclusive scan of `bins` in blocks of SCAN_TPB*SCAN_ITEMS; block totals to sums[]
+__global__ void __launch_bounds__(SCAN_TPB) k_scan_blocks(uint32_t* bins, uint32_t nb, uint32_t* sums) {
+    __shared__ uint32_t wsum[32];
+    uint32_t base = (blockIdx.x * SCAN_TPB + threadIdx.x) * SCAN_ITEMS;
+    uint32_t v[SCAN_ITEMS], tot = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) { v[k] = (base + k < nb) ? bins[base + k] : 0u; tot += v[k]; }
+    uint32_t inc = tot;
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int o = 1; o < 32; o <<= 1) { uint32_t u = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += u; }
+    if (lane == 31) wsum[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+        uint32_t s = wsum[lane], si = s;
+        for (int o = 1; o < 32; o <<= 1) { uint32_t u = __shfl_up_sync(0xffffffffu, si, o); if (lane >= o) si += u; }
+        wsum[lane] = si - s;
+        if (lane == 31 && sums) sums[blockIdx.x] = si;
+    }
+    __syncthreads();
+    uint32_t run = wsum[w] + inc - tot;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) { if (base + k < nb) bins[base + k] = run; run += v[k]; }
+}
+
+__global__ void k_sort_scatter(SortParams S, uint32_t* bins, const uint32_t* sums, uint32_t* order) {
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= S.n) return;
+    uint32_t key = sort_key(S, i);
+    uint32_t pos = atomicAdd(&bins[key], 1u) + sums[key / (SCAN_TPB * SCAN_ITEMS)];
+    order[pos] = i;
+}
+
+static int build_order(taiga_ctx* ctx, const taiga_ions* ions) {
+    const FieldDev& f = ctx->field;
+    uint32_t n = (uint32_t)ions->n;
+    int n_major = (f.kind == 1 && ions->t0) ? (f.nS < 64 ? f.nS : 64) : 1;
+    uint32_t nb = (uint32_t)n_major * SORT_NBR * SORT_NBZ;
+    uint32_t nblk = (nb + SCAN_TPB * SCAN_ITEMS - 1) / (SCAN_TPB * SCAN_ITEMS);   // <= 1024
+    int rc = tg_reserve(ctx, &ctx->order, &ctx->cap_order, (size_t)n);
+    if (rc) return rc;
+    rc = tg_reserve(ctx, &ctx->bins, &ctx->cap_bins, (size_t)nb + 2 * SCAN_TPB * SCAN_ITEMS);
+    if (rc) return rc;
+    uint32_t* sums = ctx->bins + nb;                 // nblk entries (+ padding for the second scan)
+    cudaStream_t st = ctx->stream;
+    TG_CUDA(ctx, cudaMemsetAsync(ctx->bins, 0, ((size_t)nb + 2 * SCAN_TPB * SCAN_ITEMS) * sizeof(uint32_t), st));
+    unsigned long long init[4] = {~0ull, 0ull, ~0ull, 0ull};
+    TG_CUDA(ctx, cudaMemcpyAsync(ctx->counters + 8, init, sizeof(init), cudaMemcpyHostToDevice, st));
+    SortParams S;
+    S.x = ions->x; S.y = ions->y; S.z = ions->z; S.t0 = ions->t0; S.n = n;
+    S.Rmin = f.Rmin; S.Zmin = f.Zmin;
+    int sub = ctx->opt_sort_sub > 0 ? ctx->opt_sort_sub : 4;
+    S.minwR = 1.0 / (f.inv_hR * sub); S.minwZ = 1.0 / (f.inv_hZ * sub);
+    S.s0 = f.s0; S.inv_ds = f.inv_ds; S.n_major = n_major; S.nS = f.nS;
+    S.bbox = ctx->counters + 8;
+    unsigned gb = (n + 255) / 256;
+    k_sort_bbox<<<gb, 256, 0, st>>>(S);
+    k_sort_count<<<gb, 256, 0, st>>>(S, ctx->bins);
+    k_scan_blocks<<<nblk, SCAN_TPB, 0, st>>>(ctx->bins, nb, sums);
+    k_scan_blocks<<<1, SCAN_TPB, 0, st>>>(sums, nblk, nullptr);
+    k_sort_scatter<<<gb, 256, 0, st>>>(S, ctx->bins, sums, ctx->order);
+    TG_CUDA(ctx, cudaGetLastError());
+    return TAIGA_OK;
+}
+
+int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t max_steps, const DetDev& det, int variant) {
+    cudaStream_t st = ctx->stream;
+    TraceParams P;
+    P.f = ctx->field; P.det = det;
+    P.nrD = det.normal[0] * det.origin[0] + det.normal[1] * det.origin[1] + det.normal[2] * det.origin[2];
+    P.qm = qm; P.dt = dt;
+    P.a1 = dt / (2.0 * qm); P.a2 = dt * dt / 8.0; P.b1 = qm * dt / 2.0;
+    P.c6 = dt * dt / 6.0; P.d6 = qm * dt / 6.0; P.dtq = dt / qm;
+    P.max_steps = max_steps; P.n = (uint32_t)ions->n; P.variant = variant;
+    P.refill_min = ctx->opt_min_active > 0 ? (ctx->opt_min_active > 32 ? 32 : ctx->opt_min_active) : 1;
+    P.x = ions->x; P.y = ions->y; P.z = ions->z; P.vx = ions->vx; P.vy = ions->vy; P.vz = ions->vz; P.t0 = ions->t0;
+    P.hit_u = ions->hit_u; P.hit_w = ions->hit_w; P.cell = ions->cell; P.steps = ions->steps; P.flags = ions->flags;
+    P.counters = ctx->counters;
+    P.order = nullptr;
+    int launches = 0;
+    if (ctx->opt_sort && ions->n > 64) {
+        int rc = build_order(ctx, ions);
+        if (rc) return rc;
+        P.order = ctx->order;
+        launches += 5;
+    }
+    TG_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, 8 * sizeof(unsigned long long), st));
+    int per_sm = ctx->opt_ctas_per_sm > 0 ? ctx->opt_ctas_per_sm : 2;
+    unsigned grid = (unsigned)(ctx->sm_count * per_sm);
+    unsigned need = (unsigned)((ions->n + 127) / 128);
+    if (grid > need) grid = need;
+    bool cached = ctx->opt_variant == 0 && variant == 0;
+    switch (ctx->field.kind) {
+    case 0:
+        if (cached) k_trace<0, true><<<grid, 128, 0, st>>>(P);
+        else        k_trace<0, false><<<grid, 128, 0, st>>>(P);
+        break;
+    case 1: k_trace<1, false><<<grid, 128, 0, st>>>(P); break;
+    default: k_trace<2, false><<<grid, 128, 0, st>>>(P); break;
+    }
+    ++launches;
+    TG_CUDA(ctx, cudaGetLastError());
+    if (ctx->opt_stats) {
+        TG_CUDA(ctx, cudaMemcpyAsync(ctx->counters_host, ctx->counters, 8 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+        TG_CUDA(ctx, cudaStreamSynchronize(st));
+        ctx->stats[0] = ctx->counters_host[3];
+        ctx->stats[1] = ctx->counters_host[1] * 32ull;
+        ctx->stats[2] = 1;
+        ctx->stats[3] = (unsigned long long)launches;
+        ctx->stats[4] = ctx->counters_host[2];
+        ctx->stats[5] = 0;
+    }
+    return TAIGA_OK;
+}

@@ -1,0 +1,299 @@
+"""GPU-vs-oracle parity through the C ABI (run on the B200 box: -m gpu).
+
+Acceptance (BASELINE.json north_star): initial conditions bit-exact; cell / status / steps /
+histograms bit-exact excluding ions flagged (by either side) as grazing within 1e-9 m;
+(u, w) within 1e-9 m."""
+import math
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+import oracle as orc  # noqa: E402
+from paper_2506_15812_b200 import workloads as wl  # noqa: E402
+
+TOL_UW = 1e-9
+
+
+@pytest.fixture(scope="module")
+def tg():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2506_15812_b200 import taiga
+    t = taiga.Taiga(0)
+    yield t
+    t.close()
+
+
+def _np(t):
+    return t.detach().cpu().numpy()
+
+
+def compare_groups(ions, ref, label=""):
+    """Element-by-element comparison of a run_config result with the oracle's."""
+    off = 0
+    stats = dict(n=0, flagged=0, max_du=0.0, max_dw=0.0)
+    for g in ref["groups"]:
+        n = len(g["status"])
+        v = ions.view(off, off + n)
+        for k, a in zip(("x", "y", "z", "vx", "vy", "vz"), g["state0"]):
+            assert np.array_equal(_np(v.a[k]), a), "%s: seeding not bit-exact (%s)" % (label, k)
+        assert np.array_equal(_np(v.group).astype(np.uint16), g["group"])
+        fl = (_np(v.flags) | g["flags"]) != 0
+        ok = ~fl
+        cell, steps = _np(v.cell), _np(v.steps).astype(np.uint32)
+        bad = ok & ((cell != g["cell"]) | (steps != g["steps"]))
+        assert not bad.any(), "%s: %d unflagged ions differ, first %s: gpu cell/steps %s/%s oracle %s/%s" % (
+            label, bad.sum(), np.flatnonzero(bad)[:5], cell[bad][:5], steps[bad][:5], g["cell"][bad][:5], g["steps"][bad][:5])
+        cr = ok & (g["status"] == 0)
+        if cr.any():
+            du = np.abs(_np(v.hit_u)[cr] - g["u"][cr]).max()
+            dw = np.abs(_np(v.hit_w)[cr] - g["w"][cr]).max()
+            assert du < TOL_UW and dw < TOL_UW, (label, du, dw)
+            stats["max_du"], stats["max_dw"] = max(stats["max_du"], du), max(stats["max_dw"], dw)
+        stats["n"] += n
+        stats["flagged"] += int(fl.sum())
+        off += n
+    return stats
+
+
+def check_histogram(cfg, ions, counts, summary, ref):
+    """Histograms bit-exact after removing the flagged ions from both sides."""
+    c_gpu = _np(counts).astype(np.int64).copy()
+    c_ref = ref["counts"].astype(np.int64).copy()
+    off = 0
+    for g in ref["groups"]:
+        n = len(g["status"])
+        v = ions.view(off, off + n)
+        fl = (_np(v.flags) | g["flags"]) != 0
+        det = None
+        for i in np.flatnonzero(fl):
+            gi = int(g["group"][i])
+            cg, cr = int(_np(v.cell)[i]), int(g["cell"][i])
+            if cg >= 0:
+                c_gpu[gi].reshape(-1)[cg] -= 1
+            if cr >= 0:
+                c_ref[gi].reshape(-1)[cr] -= 1
+        off += n
+    assert np.array_equal(c_gpu, c_ref)
+    s = _np(summary)
+    for h in range(cfg.n_hist):
+        n_h = sum(int(np.sum(g["group"] == h)) for g in ref["groups"])
+        assert s[h, 0] == _np(counts)[h].sum()
+        assert s[h, :5].sum() == n_h                       # O5 invariant
+
+
+@pytest.mark.parametrize("opts", [dict(), dict(sort=0), dict(variant=1), dict(min_active=1), dict(min_active=32)])
+def test_cfg1_full_parity(tg, opts):
+    from paper_2506_15812_b200 import taiga
+    cfg = wl.config(1)
+    for k, v in dict(sort=1, variant=0, min_active=12).items():
+        tg.set_option(k, v)
+    for k, v in opts.items():
+        tg.set_option(k, v)
+    ions, counts, summary = taiga.run_config(tg, cfg)
+    torch.cuda.synchronize()
+    ref = orc.run_config(cfg)
+    st = compare_groups(ions, ref, "cfg1 %s" % opts)
+    check_histogram(cfg, ions, counts, summary, ref)
+    assert st["flagged"] < 20
+    for k, v in dict(sort=1, variant=0, min_active=12).items():
+        tg.set_option(k, v)
+
+
+def test_cfg1_printed_k3_variant(tg):
+    from paper_2506_15812_b200 import taiga
+    cfg = wl.config(1)
+    ions, counts, summary = taiga.run_config(tg, cfg, rkn_variant=1)
+    torch.cuda.synchronize()
+    ref = orc.run_config(cfg, variant=1)
+    compare_groups(ions, ref, "cfg1 k3-from-k2")
+    ref0 = orc.run_config(cfg, variant=0)
+    cr = (ref0["groups"][0]["status"] == 0) & (ref["groups"][0]["status"] == 0)
+    # the two readings differ by more than the tolerance (A1): the switch is live
+    assert np.abs(ref0["groups"][0]["u"][cr] - ref["groups"][0]["u"][cr]).max() > 5e-10
+
+
+@pytest.mark.parametrize("icfg,n", [(2, 16384), (3, 4096), (4, 256), (5, 4096)])
+def test_prefix_parity(tg, icfg, n):
+    """Prefix subsamples of configs 2-5: identical ions (Philox counter = global ion index),
+    sizes spanning many warps plus a ragged tail (n is per group)."""
+    from paper_2506_15812_b200 import taiga
+    n = n + 37 if icfg in (2, 5) else n
+    cfg = wl.config(icfg, n_override=n)
+    ions, counts, summary = taiga.run_config(tg, cfg)
+    torch.cuda.synchronize()
+    ref = orc.run_config(cfg)
+    st = compare_groups(ions, ref, cfg.name)
+    check_histogram(cfg, ions, counts, summary, ref)
+    assert st["flagged"] <= max(8, st["n"] // 500)
+    ngpu = int(_np(ions.steps).astype(np.int64).sum())
+    assert tg.stats()["launches"] >= 1
+    assert ngpu > 0
+
+
+def test_seeding_bit_exact_large_indices_and_divergence(tg):
+    from paper_2506_15812_b200 import taiga
+    beam = wl.Beam(wl.MASS_NA23, wl.E_CHARGE, 40e3, sigma_pos_m=7e-3, sigma_ang_rad=3e-3,
+                   origin=(0.8, 0.01, -0.02), axis=(-0.6, 0.0, 0.8), eT=(0.0, 1.0, 0.0), eZ=(0.8, 0.0, 0.6))
+    cd, cn = wl.depth_cdf(0.035, 0.15, 777), wl.normal_cdf(5.0, 1000)
+    beam.depth_max, beam.z_max = 0.15, 5.0
+    for first, seed, n in ((0, 0, 1), ((1 << 40) + 12345, 0xDEADBEEFCAFEF00D, 10007), (2 ** 32 - 5, 7, 64)):
+        ions = taiga.Ions(n)
+        tg.seed_beam(beam, cd, cn, seed, ions, first_index=first, group=3, t0=2.5e-6)
+        torch.cuda.synchronize()
+        ref = orc.seed(beam, cd, cn, seed, first, n)
+        for k, a in zip(("x", "y", "z", "vx", "vy", "vz"), ref):
+            assert np.array_equal(_np(ions.a[k]), a), (k, first)
+        assert np.all(_np(ions.group) == 3) and np.all(_np(ions.t0) == 2.5e-6)
+
+
+@pytest.mark.parametrize("kind", [0, 1, 2])
+def test_field_precompute_vs_oracle_tables(tg, kind):
+    if kind == 0:
+        grid, nodal = wl.nodal_field_2d(33, 65)
+    elif kind == 1:
+        grid, nodal = wl.nodal_field_time_slices(17, 33, 5)
+    else:
+        grid, nodal = wl.nodal_field_ripple(17, 33, 8)
+    rng = np.random.default_rng(kind)
+    nodal = [c + 1e-3 * rng.standard_normal(c.shape) for c in nodal]      # not a polynomial
+    f = orc.OracleField(grid, nodal)
+    for host in (True, False):
+        tg.load_field(grid, nodal if host else [torch.from_numpy(np.ascontiguousarray(c)).cuda() for c in nodal])
+        for comp in range(3):
+            tab = tg.field_table(comp, f.tables[comp].shape)
+            scale = np.abs(f.tables[comp]).max()
+            assert np.abs(tab - f.tables[comp]).max() < 2e-13 * max(scale, 1.0), (kind, comp)
+    # evaluation at random points, inside and outside (extrapolation) the grid
+    n = 4000
+    R = rng.uniform(grid.Rmin - 0.01, grid.Rmax + 0.01, n)
+    Z = rng.uniform(grid.Zmin - 0.01, grid.Zmax + 0.01, n)
+    s = rng.uniform(-2 * grid.ds, (grid.nS + 2) * grid.ds, n)
+    out = tg.field_eval(torch.from_numpy(R).cuda(), torch.from_numpy(Z).cuda(), torch.from_numpy(s).cuda())
+    out = [_np(o) for o in out]
+    for i in range(0, n, 7):
+        b = f.cyl(R[i], Z[i], s[i])
+        for c in range(3):
+            assert abs(out[c][i] - b[c]) < 1e-12, (kind, i, c)
+    # form 1: ready coefficients (the paper's "read from the preprocessing database" mode)
+    tg.load_field(grid, f.tables, form=1)
+    out1 = [_np(o) for o in tg.field_eval(torch.from_numpy(R).cuda(), torch.from_numpy(Z).cuda(), torch.from_numpy(s).cuda())]
+    for c in range(3):
+        assert np.abs(out1[c] - out[c]).max() < 1e-12
+
+
+@pytest.mark.parametrize("n_hist,nu,nw", [(3, 4, 3), (40, 16, 16)])
+def test_histogram_vs_oracle_gapped_detector(tg, n_hist, nu, nw):
+    from paper_2506_15812_b200 import taiga
+    rng = np.random.default_rng(11)
+    n = 100003
+    eu = np.sort(rng.uniform(-5e-3, 5e-3, 2 * nu))
+    ew = np.sort(rng.uniform(-5e-3, 5e-3, 2 * nw))
+    det = wl.Detector((0.82, 0, 0), (1, 0, 0), (0, 1, 0), (0, 0, 1), eu[0::2].copy(), eu[1::2].copy(),
+                      ew[0::2].copy(), ew[1::2].copy())
+    status = rng.choice([-1, -1, -1, -2, -3, -4], n).astype(np.int32)
+    u = rng.uniform(-6e-3, 6e-3, n)
+    w = rng.uniform(-6e-3, 6e-3, n)
+    u[:nu] = det.u_lo                     # exactly on edges
+    u[nu:2 * nu] = det.u_hi
+    status[:2 * nu] = -1
+    grp = rng.integers(0, n_hist + 1, n).astype(np.uint16)      # some out-of-range groups: skipped
+    ions = taiga.Ions(n)
+    ions.a["cell"].copy_(torch.from_numpy(status))
+    ions.a["hit_u"].copy_(torch.from_numpy(u))
+    ions.a["hit_w"].copy_(torch.from_numpy(w))
+    ions.a["group"].copy_(torch.from_numpy(grp.astype(np.int16)))
+    counts = torch.zeros((n_hist, nw, nu), dtype=torch.int64, device="cuda")
+    summary = torch.zeros((n_hist, 6), dtype=torch.int64, device="cuda")
+    tg.detector_histogram(ions, det, n_hist, counts, summary)
+    torch.cuda.synchronize()
+    res = dict(status=np.where(status == -1, 0, status).astype(np.int32), u=u, w=w, flags=np.zeros(n, np.uint8))
+    c_ref, s_ref = orc.histogram(res, grp, det, n_hist)
+    assert np.array_equal(_np(counts).astype(np.uint64), c_ref)
+    assert np.array_equal(_np(summary).astype(np.uint64), s_ref)
+    valid = grp < n_hist
+    assert np.array_equal(_np(ions.cell)[valid], res["cell"][valid])
+    assert np.array_equal(_np(ions.flags)[valid], res["flags"][valid])
+
+
+def test_edge_cases_and_errors(tg):
+    from paper_2506_15812_b200 import taiga
+    cfg = wl.config(1)
+    grid, nodal = cfg.field_builder()
+    t2 = taiga.Taiga(0)
+    ions = taiga.Ions(8)
+    with pytest.raises(taiga.TaigaError) as e:
+        t2.trace(ions, 1.0, 1e-9, 10, cfg.detector)
+    assert e.value.code == taiga.E_STATE
+    t2.load_field(grid, nodal)
+    for bad in (dict(dt=-1.0), dict(qm=0.0)):
+        with pytest.raises(taiga.TaigaError) as e:
+            t2.trace(ions, bad.get("qm", 1.0), bad.get("dt", 1e-9), 10, cfg.detector)
+        assert e.value.code == taiga.E_ARG
+    skew = wl.Detector((0.82, 0, 0), (1, 0, 0), (0, 1, 0), (0, 0.1, 1.0), *([np.array([0.0]), np.array([1.0])] * 2))
+    with pytest.raises(taiga.TaigaError):
+        t2.trace(ions, 1.0, 1e-9, 10, skew)
+    badcdf = wl.depth_cdf().copy()
+    badcdf[5] = 0.9
+    with pytest.raises(taiga.TaigaError):
+        t2.seed_beam(cfg.groups[0].beam, badcdf, wl.normal_cdf(), 0, ions)
+    # empty and tiny inputs
+    t2.seed_beam(cfg.groups[0].beam, wl.depth_cdf(), wl.normal_cdf(), 0, taiga.Ions(0))
+    t2.trace(taiga.Ions(0), 1.0, 1e-9, 10, cfg.detector)
+    for n in (1, 31, 33):
+        c = wl.config(1, n_override=n)
+        io, counts, summary = taiga.run_config(t2, c, field_loaded=True)
+        torch.cuda.synchronize()
+        compare_groups(io, orc.run_config(c), "n=%d" % n)
+    # degenerate: max_steps = 0 and 1; every ion starts behind the plane
+    c = wl.config(1, n_override=257)
+    for ms in (0, 1):
+        c.max_steps = ms
+        io, counts, summary = taiga.run_config(t2, c, field_loaded=True)
+        torch.cuda.synchronize()
+        compare_groups(io, orc.run_config(c), "max_steps=%d" % ms)
+        assert int(summary[0, 2]) == 257
+    c = wl.config(1, n_override=100)
+    c.detector = wl.uniform_detector(0.02, 0.18, 8, 2.5e-3, x_plane=0.5)
+    io, counts, summary = taiga.run_config(t2, c, field_loaded=True)
+    torch.cuda.synchronize()
+    compare_groups(io, orc.run_config(c), "behind plane")
+    assert int(summary[0, 4]) == 100
+    t2.close()
+
+
+def test_cfg2_full_size_bench_configuration(tg):
+    """BASELINE config 2 at full size in the launch configuration bench.py times: invariants at
+    any size + sampled ions checked one by one against the oracle."""
+    from paper_2506_15812_b200 import taiga
+    cfg = wl.config(2)
+    ions, counts, summary = taiga.run_config(tg, cfg)
+    torch.cuda.synchronize()
+    s = _np(summary)[0]
+    assert s[:5].sum() == cfg.n_ions and s[0] == _np(counts).sum()
+    st = tg.stats()
+    assert st["ion_steps"] == int(_np(ions.steps).astype(np.int64).sum())
+    rng = np.random.default_rng(2)
+    idx = np.sort(rng.choice(cfg.n_ions, 6000, replace=False))
+    grid, nodal = cfg.field_builder()
+    f = orc.OracleField(grid, nodal)
+    g = cfg.groups[0]
+    state = [_np(ions.a[k])[idx] for k in ("x", "y", "z", "vx", "vy", "vz")]
+    seeds = orc.seed(g.beam, wl.depth_cdf(), wl.normal_cdf(), cfg.seed, 0, int(idx.max()) + 1)
+    for a, b in zip(state, seeds):
+        assert np.array_equal(a, b[idx])
+    res = orc.trace(f, g.beam.charge_C / g.beam.mass_kg, state, None, cfg.dt, cfg.max_steps, cfg.detector)
+    orc.histogram(res, None, cfg.detector, 1)
+    fl = (_np(ions.flags)[idx] | res["flags"]) != 0
+    ok = ~fl
+    assert np.array_equal(_np(ions.cell)[idx][ok], res["cell"][ok])
+    assert np.array_equal(_np(ions.steps)[idx][ok].astype(np.uint32), res["steps"][ok])
+    cr = ok & (res["status"] == 0)
+    assert np.abs(_np(ions.hit_u)[idx][cr] - res["u"][cr]).max() < TOL_UW
+    assert np.abs(_np(ions.hit_w)[idx][cr] - res["w"][cr]).max() < TOL_UW
+    # mean steps / structure of the workload (SURVEY 8(d) probe: ~1038 steps/ion, 96.3 % cross)
+    assert 900 < st["ion_steps"] / cfg.n_ions < 1200
+    assert 0.955 < (s[0] + s[1]) / cfg.n_ions < 0.97
