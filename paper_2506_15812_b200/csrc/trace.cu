@@ -101,8 +101,8 @@ __device__ __forceinline__ void tg_fieldB(const TraceParams& P, CellCache<KIND>&
     Bz = BZ;
 }
 
-template <int KIND, bool CACHED>
-__global__ void __launch_bounds__(128, 2) k_trace(const TraceParams P) {
+template <int KIND, bool CACHED, int MINB>
+__global__ void __launch_bounds__(128, MINB) k_trace(const TraceParams P) {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     CellCache<KIND> cc;
@@ -363,19 +363,24 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         launches += 5;
     }
     TG_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, 8 * sizeof(unsigned long long), st));
-    int per_sm = ctx->opt_ctas_per_sm > 0 ? ctx->opt_ctas_per_sm : 2;
+    // kernel variants (option "variant"): 0 = register cell cache, 2 CTAs/SM (kind 0 only);
+    // 1 = uncached, 2 CTAs/SM; 2 = uncached, 4 CTAs/SM; 3 = cached, 3 CTAs/SM
+    int kv = ctx->opt_variant;
+    if (ctx->field.kind != 0 || variant != 0) { if (kv == 0) kv = 1; if (kv == 3) kv = 2; }
+    int per_sm = ctx->opt_ctas_per_sm > 0 ? ctx->opt_ctas_per_sm : (kv == 2 ? 4 : (kv == 3 ? 3 : 2));
     unsigned grid = (unsigned)(ctx->sm_count * per_sm);
     unsigned need = (unsigned)((ions->n + 127) / 128);
     if (grid > need) grid = need;
-    bool cached = ctx->opt_variant == 0 && variant == 0;
+#define TG_LAUNCH(K, C, B) k_trace<K, C, B><<<grid, 128, 0, st>>>(P)
     switch (ctx->field.kind) {
     case 0:
-        if (cached) k_trace<0, true><<<grid, 128, 0, st>>>(P);
-        else        k_trace<0, false><<<grid, 128, 0, st>>>(P);
+        if (kv == 0) TG_LAUNCH(0, true, 2); else if (kv == 3) TG_LAUNCH(0, true, 3);
+        else if (kv == 2) TG_LAUNCH(0, false, 4); else TG_LAUNCH(0, false, 2);
         break;
-    case 1: k_trace<1, false><<<grid, 128, 0, st>>>(P); break;
-    default: k_trace<2, false><<<grid, 128, 0, st>>>(P); break;
+    case 1: if (kv == 2) TG_LAUNCH(1, false, 4); else TG_LAUNCH(1, false, 2); break;
+    default: if (kv == 2) TG_LAUNCH(2, false, 4); else TG_LAUNCH(2, false, 2); break;
     }
+#undef TG_LAUNCH
     ++launches;
     TG_CUDA(ctx, cudaGetLastError());
     if (ctx->opt_stats) {
