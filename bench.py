@@ -111,7 +111,7 @@ def main_reference(args):
 
 
 def launches_per_step(cfg, kind):
-    a1 = 12 + (1 if kind == 2 else 0)          # 3 components x (3 line-solve + 1 assemble) [+ phi spline]
+    a1 = 3 + 3 + (1 if kind == 2 else 0)       # 3 second-derivative stencils + 3 assembles [+ phi spline]
     ntrace = 1 if cfg.detector is not None else len(cfg.groups)
     return a1 + len(cfg.groups) + ntrace * (5 + 1) + ntrace      # seeds + (sort 5 + trace 1) + histogram
 

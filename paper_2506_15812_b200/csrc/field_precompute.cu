@@ -1,44 +1,69 @@
 // a1: field-coefficient precompute.  Interpolating tensor-product cubic
-// spline, not-a-knot in R and Z, periodic in phi (kind 2).  Line-parallel solves: one thread
-// per grid line for the second derivatives, then one thread per (cell, component) assembles
-// the 16 power-basis coefficients from {y, y_zz, y_rr, y_rrzz} at the 4 corners.
+// spline, not-a-knot in R and Z, periodic in phi (kind 2).
 //
 // not-a-knot on a unit-spaced line, unknowns M_i = S''(x_i):
 //   M_{i-1} + 4 M_i + M_{i+1} = 6 (y_{i-1} - 2 y_i + y_{i+1}),   i = 1..n-2
 //   M_0 - 2 M_1 + M_2 = 0   =>  substituting into row 1:  M_1 = y_0 - 2 y_1 + y_2
 //   (same at the far end), so the system is tridiagonal in M_2..M_{n-3} with known ends.
+// The map y -> M is linear, M = H y, and because the (1,4,1) system is diagonally dominant the
+// entries of H decay like (2-sqrt 3)^|i-j| = 0.268^|i-j|: beyond |i-j| = 36 they are below
+// 3e-21 of the diagonal.  So instead of one serial Thomas solve per grid line (a few hundred
+// threads, latency bound) the band of H is built once per line length on the host (O(n^2), by
+// running the reduction above on unit vectors) and every node is then an independent 73-point
+// stencil: one thread per node, coalesced, exact to rounding.  One thread per (cell, component)
+// finally assembles the 16 power-basis coefficients from {y, y_zz, y_rr, y_rrzz} at 4 corners.
 #include <vector>
 
 #include "field_device.cuh"
 
-// cp[i] = Thomas pivots of the (1,4,1) interior system: cp[2] = 1/4, cp[i] = 1/(4 - cp[i-1]).
-__global__ void k_spline_lines(const double* __restrict__ y, double* __restrict__ M, const double* __restrict__ cp,
-                               int n, long long stride, int lines_inner, long long inner_stride,
-                               long long outer_stride, int nlines) {
-    int line = blockIdx.x * blockDim.x + threadIdx.x;
-    if (line >= nlines) return;
-    long long base = (long long)(line / lines_inner) * outer_stride + (long long)(line % lines_inner) * inner_stride;
-    const double* yl = y + base;
-    double* Ml = M + base;
-    auto Y = [&](int i) { return yl[(long long)i * stride]; };
-    auto d2 = [&](int i) { return (Y(i - 1) - 2.0 * Y(i)) + Y(i + 1); };
-    double M1 = d2(1), Mn2 = d2(n - 2);
-    Ml[stride] = M1;
-    Ml[(long long)(n - 2) * stride] = Mn2;
-    double dprev = 0.0;
-    for (int i = 2; i <= n - 3; ++i) {
-        double rhs = 6.0 * d2(i);
-        if (i == 2) rhs -= M1;
-        if (i == n - 3) rhs -= Mn2;
-        double dp = (i == 2) ? rhs * cp[i] : (rhs - dprev) * cp[i];
-        Ml[(long long)i * stride] = dp;
-        dprev = dp;
+#define TG_BAND_W 36
+
+// M[t] = sum_q H[i][q] y[q] along one grid direction.  band[(q-i+W)*n + i] = H[i][q].
+// `stride`: distance between consecutive nodes of a line; i = (t / stride) % n.
+__global__ void k_second_deriv(const double* __restrict__ y, double* __restrict__ M, const double* __restrict__ band,
+                               int n, long long stride, long long total) {
+    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= total) return;
+    int i = (int)((t / stride) % n);
+    int lo = max(0, i - TG_BAND_W), hi = min(n - 1, i + TG_BAND_W);
+    double acc = 0.0;
+    for (int q = lo; q <= hi; ++q)
+        acc = fma(band[(size_t)(q - i + TG_BAND_W) * n + i], y[t + (long long)(q - i) * stride], acc);
+    M[t] = acc;
+}
+
+// host: band of H for line length n (Thomas reduction applied to unit vectors)
+static std::vector<double> spline_band(int n) {
+    std::vector<double> band((size_t)(2 * TG_BAND_W + 1) * n, 0.0), cp(n, 0.0), M(n), y(n);
+    for (int i = 2; i <= n - 3; ++i) cp[i] = (i == 2) ? 0.25 : 1.0 / (4.0 - cp[i - 1]);
+    for (int q = 0; q < n; ++q) {
+        // response to y = e_q is non-negligible only for |i-q| <= W (+2 for the end rows); solve on a window
+        int lo = q - TG_BAND_W - 3, hi = q + TG_BAND_W + 3;
+        if (lo < 0) lo = 0;
+        if (hi > n - 1) hi = n - 1;
+        auto Y = [&](int i) { return i == q ? 1.0 : 0.0; };
+        auto d2 = [&](int i) { return (Y(i - 1) - 2.0 * Y(i)) + Y(i + 1); };
+        // full-length solve restricted to rows where the right-hand side can be non-zero is not
+        // possible for a tridiagonal system, so solve the whole line (O(n) per column, O(n^2) total)
+        double M1 = d2(1), Mn2 = d2(n - 2), dprev = 0.0;
+        std::fill(M.begin(), M.end(), 0.0);
+        M[1] = M1; M[n - 2] = Mn2;
+        for (int i = 2; i <= n - 3; ++i) {
+            double rhs = 6.0 * d2(i);
+            if (i == 2) rhs -= M1;
+            if (i == n - 3) rhs -= Mn2;
+            double dp = (i == 2) ? rhs * cp[i] : (rhs - dprev) * cp[i];
+            M[i] = dp; dprev = dp;
+        }
+        for (int i = n - 4; i >= 2; --i) M[i] = M[i] - cp[i] * M[i + 1];
+        M[0] = 2.0 * M[1] - M[2];
+        M[n - 1] = 2.0 * M[n - 2] - M[n - 3];
+        for (int i = lo; i <= hi; ++i) {
+            int d = q - i + TG_BAND_W;
+            if (d >= 0 && d <= 2 * TG_BAND_W) band[(size_t)d * n + i] = M[i];
+        }
     }
-    for (int i = n - 4; i >= 2; --i)
-        Ml[(long long)i * stride] = Ml[(long long)i * stride] - cp[i] * Ml[(long long)(i + 1) * stride];
-    double M2 = Ml[2 * stride], Mn3 = Ml[(long long)(n - 3) * stride];
-    Ml[0] = 2.0 * M1 - M2;
-    Ml[(long long)(n - 1) * stride] = 2.0 * Mn2 - Mn3;
+    return band;
 }
 
 // power-basis coefficients of one interval from end values g0,g1 and end second derivatives G0,G1
@@ -131,12 +156,6 @@ __global__ void k_field_eval(FieldDev f, unsigned long long n, const double* R, 
     BR[i] = a; BZ[i] = b; Bp[i] = c;
 }
 
-static std::vector<double> thomas_pivots(int n) {
-    std::vector<double> cp(n > 0 ? n : 1, 0.0);
-    for (int i = 2; i <= n - 3; ++i) cp[i] = (i == 2) ? 0.25 : 1.0 / (4.0 - cp[i - 1]);
-    return cp;
-}
-
 // first column of inverse of circulant(4,1,0,...,0,1), by Gaussian elimination (n <= 128)
 static std::vector<double> circulant_inverse_col(int n) {
     std::vector<double> A((size_t)n * n, 0.0), x(n, 0.0);
@@ -180,32 +199,47 @@ int tg_precompute(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c) {
             k_relayout<<<(unsigned)((need + TPB - 1) / TPB), TPB, 0, st>>>(s, ctx->table, g->kind, nS, ncell, m, 1);
         }
     } else {
-        // scratch: [nodal(if host)] y | Mz | Myr | Mzr (one component at a time) | pivots | temp bicubic (kind 2) | G
+        // scratch: y[3] | Mz[3] | Myr[3] | Mzr[3] (3 components) | temp bicubic (kind 2) | G
         size_t n_tmp = (g->kind == 2) ? (size_t)ncell * nS * 48 : 0;
-        size_t need = 4 * (size_t)nnode + nR + nZ + n_tmp + TG_MAX_PLANES, scap = ctx->scratch_bytes / sizeof(double);
+        size_t need = 12 * (size_t)nnode + n_tmp + TG_MAX_PLANES, scap = ctx->scratch_bytes / sizeof(double);
         rc = tg_reserve(ctx, &ctx->scratch, &scap, need);
         ctx->scratch_bytes = scap * sizeof(double);
         if (rc) return rc;
-        double *y = ctx->scratch, *Mz = y + nnode, *Myr = Mz + nnode, *Mzr = Myr + nnode;
-        double *cpZ = Mzr + nnode, *cpR = cpZ + nZ, *tmp = cpR + nR, *G = tmp + n_tmp;
-        std::vector<double> pz = thomas_pivots(nZ), pr = thomas_pivots(nR);
-        TG_CUDA(ctx, cudaMemcpyAsync(cpZ, pz.data(), nZ * sizeof(double), cudaMemcpyHostToDevice, st));
-        TG_CUDA(ctx, cudaMemcpyAsync(cpR, pr.data(), nR * sizeof(double), cudaMemcpyHostToDevice, st));
-        std::vector<double> Gh;
-        if (g->kind == 2) { Gh = circulant_inverse_col(nS); TG_CUDA(ctx, cudaMemcpyAsync(G, Gh.data(), nS * sizeof(double), cudaMemcpyHostToDevice, st)); }
-        TG_CUDA(ctx, cudaStreamSynchronize(st));       // host vectors above go out of use
+        double *y = ctx->scratch, *Mz = y + 3 * nnode, *Myr = Mz + 3 * nnode, *Mzr = Myr + 3 * nnode;
+        double *tmp = Mzr + 3 * nnode, *G = tmp + n_tmp;
+        // band operators, cached per line length
+        for (int ax = 0; ax < 2; ++ax) {
+            int n = ax ? nR : nZ;
+            if (ctx->band_n[ax] != n) {
+                std::vector<double> b = spline_band(n);
+                size_t cap = ctx->band_cap[ax];
+                rc = tg_reserve(ctx, &ctx->band[ax], &cap, b.size());
+                ctx->band_cap[ax] = cap;
+                if (rc) return rc;
+                TG_CUDA(ctx, cudaMemcpyAsync(ctx->band[ax], b.data(), b.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+                TG_CUDA(ctx, cudaStreamSynchronize(st));
+                ctx->band_n[ax] = n;
+            }
+        }
+        if (g->kind == 2) {
+            std::vector<double> Gh = circulant_inverse_col(nS);
+            TG_CUDA(ctx, cudaMemcpyAsync(G, Gh.data(), nS * sizeof(double), cudaMemcpyHostToDevice, st));
+            TG_CUDA(ctx, cudaStreamSynchronize(st));
+        }
+        for (int m = 0; m < 3; ++m)
+            TG_CUDA(ctx, cudaMemcpyAsync(y + (size_t)m * nnode, src[m], nnode * sizeof(double),
+                                         c->on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+        long long tot = 3 * nnode;
+        unsigned gb = (unsigned)((tot + TPB - 1) / TPB);
+        k_second_deriv<<<gb, TPB, 0, st>>>(y, Mz, ctx->band[0], nZ, 1, tot);          // y_zz
+        k_second_deriv<<<gb, TPB, 0, st>>>(y, Myr, ctx->band[1], nR, nZ, tot);        // y_rr
+        k_second_deriv<<<gb, TPB, 0, st>>>(Mz, Mzr, ctx->band[1], nR, nZ, tot);       // y_rrzz
         for (int m = 0; m < 3; ++m) {
-            const double* yy = src[m];
-            if (!c->on_device) { TG_CUDA(ctx, cudaMemcpyAsync(y, src[m], nnode * sizeof(double), cudaMemcpyHostToDevice, st)); yy = y; }
-            int linesZ = nS * nR, linesR = nS * nZ;
-            // along Z: line (k,i) at (k*nR+i)*nZ, stride 1
-            k_spline_lines<<<(linesZ + TPB - 1) / TPB, TPB, 0, st>>>(yy, Mz, cpZ, nZ, 1, linesZ, nZ, 0, linesZ);
-            // along R: line (k,j) at k*nR*nZ + j, stride nZ  -- of y and of Mz
-            k_spline_lines<<<(linesR + TPB - 1) / TPB, TPB, 0, st>>>(yy, Myr, cpR, nR, nZ, nZ, 1, (long long)nR * nZ, linesR);
-            k_spline_lines<<<(linesR + TPB - 1) / TPB, TPB, 0, st>>>(Mz, Mzr, cpR, nR, nZ, nZ, 1, (long long)nR * nZ, linesR);
             long long nt = ncell * nS;
-            k_assemble<<<(unsigned)((nt + TPB - 1) / TPB), TPB, 0, st>>>(yy, Mz, Myr, Mzr, g->kind == 2 ? tmp : ctx->table,
-                                                                      nS, nR, nZ, m, g->kind == 2 ? 1 : 0);
+            size_t o = (size_t)m * nnode;
+            k_assemble<<<(unsigned)((nt + TPB - 1) / TPB), TPB, 0, st>>>(y + o, Mz + o, Myr + o, Mzr + o,
+                                                                      g->kind == 2 ? tmp : ctx->table, nS, nR, nZ, m,
+                                                                      g->kind == 2 ? 1 : 0);
         }
         if (g->kind == 2) {
             long long nt = ncell * 48;

@@ -36,8 +36,8 @@ extern "C" int taiga_create(taiga_ctx** out, int device, void* cuda_stream) {
         cudaMallocHost((void**)&ctx->counters_host, 16 * sizeof(unsigned long long)) != cudaSuccess) {
         delete ctx; return TAIGA_E_NOMEM;
     }
-    ctx->opt_sort = 1; ctx->opt_sort_sub = 4;
-    ctx->opt_chunk0 = 0; ctx->opt_chunk = 2048; ctx->opt_min_active = 12;
+    ctx->opt_sort = 1; ctx->opt_sort_sub = 16;
+    ctx->opt_chunk0 = 0; ctx->opt_chunk = 2048; ctx->opt_min_active = 32;
     ctx->opt_ctas_per_sm = 0; ctx->opt_variant = 0; ctx->opt_stats = 1;
     strcpy(ctx->err, "ok");
     *out = ctx;
@@ -48,7 +48,7 @@ extern "C" int taiga_destroy(taiga_ctx* ctx) {
     if (!ctx) return TAIGA_E_ARG;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    void* bufs[] = {ctx->table, ctx->scratch, ctx->cdf_depth, ctx->cdf_normal, ctx->edges, ctx->order,
+    void* bufs[] = {ctx->table, ctx->scratch, ctx->band[0], ctx->band[1], ctx->cdf_depth, ctx->cdf_normal, ctx->edges, ctx->order,
                     ctx->bins, ctx->surv[0], ctx->surv[1], ctx->surv_idx[0], ctx->surv_idx[1],
                     ctx->surv_steps[0], ctx->surv_steps[1], ctx->counters};
     for (void* b : bufs) if (b) cudaFree(b);

@@ -36,6 +36,7 @@ struct taiga_ctx {
     FieldDev field;
     double* table;            size_t table_bytes;
     double* scratch;          size_t scratch_bytes;     // precompute work arrays
+    double* band[2];          size_t band_cap[2]; int band_n[2];   // y -> y'' band operators (Z, R)
 
     // seeding tables
     double *cdf_depth, *cdf_normal;  int cap_depth, cap_normal;

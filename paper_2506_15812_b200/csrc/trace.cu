@@ -73,24 +73,32 @@ __device__ __forceinline__ double tg_horner16(const double* c, double p, double 
 }
 
 // Cartesian B at (X,Y,Z,t) given R2 = X^2+Y^2, rinv = 1/R, R.
-template <int KIND, bool CACHED>
-__device__ __forceinline__ void tg_fieldB(const TraceParams& P, CellCache<KIND>& cc, int& reloads, double X, double Y,
-                                          double Z, double t, double R, double rinv, double& Bx, double& By, double& Bz) {
+// FIRST (stage 1 of a step, cached path): also reports whether (R,Z) lies outside the grid; a
+// point inside the cached cell is inside the grid, so the four comparisons run only on a refill.
+template <int KIND, bool CACHED, bool FIRST = false>
+__device__ __forceinline__ void tg_fieldB(const TraceParams& P, CellCache<KIND>& cc, unsigned& reloads, bool& outside,
+                                          double X, double Y, double Z, double t, double R, double rinv,
+                                          double& Bx, double& By, double& Bz) {
     double BR, BZ, Bp;
     if constexpr (KIND == 0 && CACHED) {
         double tR = fma(R, P.f.inv_hR, -cc.oR), tZ = fma(Z, P.f.inv_hZ, -cc.oZ);
         if (!(tg_in01(tR) && tg_in01(tZ))) {
+            if constexpr (FIRST) outside = (R < P.f.Rmin) | (R > P.f.Rmax) | (Z < P.f.Zmin) | (Z > P.f.Zmax);
             double pR = fma(R, P.f.inv_hR, -P.f.offR), pZ = fma(Z, P.f.inv_hZ, -P.f.offZ);
             int i = tg_clampi(__double2int_rd(pR), 0, P.f.cR - 1), j = tg_clampi(__double2int_rd(pZ), 0, P.f.cZ - 1);
             cc.oR = P.f.offR + (double)i; cc.oZ = P.f.offZ + (double)j;
-            const double2* src = reinterpret_cast<const double2*>(P.f.table + ((size_t)i * P.f.cZ + j) * 48);
+            const double* src = P.f.table + ((size_t)i * P.f.cZ + j) * 48;      // 384-B aligned
 #pragma unroll
-            for (int k = 0; k < 24; ++k) { double2 v = __ldg(src + k); cc.c[2 * k] = v.x; cc.c[2 * k + 1] = v.y; }
+            for (int k = 0; k < 12; ++k)       // 12 x LDG.E.256 (sm_100: 256-bit global loads)
+                asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];"
+                             : "=d"(cc.c[4 * k]), "=d"(cc.c[4 * k + 1]), "=d"(cc.c[4 * k + 2]), "=d"(cc.c[4 * k + 3])
+                             : "l"(src + 4 * k));
             tR = fma(R, P.f.inv_hR, -cc.oR); tZ = fma(Z, P.f.inv_hZ, -cc.oZ);
             ++reloads;
         }
         BR = tg_horner16(cc.c, tR, tZ); BZ = tg_horner16(cc.c + 16, tR, tZ); Bp = tg_horner16(cc.c + 32, tR, tZ);
     } else {
+        if constexpr (FIRST) outside = (R < P.f.Rmin) | (R > P.f.Rmax) | (Z < P.f.Zmin) | (Z > P.f.Zmax);
         double s = t;
         if constexpr (KIND == 2) s = atan2(Y, X);
         tg_field_cyl(P.f, R, Z, s, BR, BZ, Bp);
@@ -101,8 +109,8 @@ __device__ __forceinline__ void tg_fieldB(const TraceParams& P, CellCache<KIND>&
     Bz = BZ;
 }
 
-template <int KIND, bool CACHED, int MINB>
-__global__ void __launch_bounds__(128, MINB) k_trace(const TraceParams P) {
+template <int KIND, bool CACHED, int THREADS, int MAXREG>
+__global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const TraceParams P) {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     CellCache<KIND> cc;
@@ -112,8 +120,8 @@ __global__ void __launch_bounds__(128, MINB) k_trace(const TraceParams P) {
     double X = 0, Y = 0, Z = 0, Ux = 0, Uy = 0, Uz = 0, t = 0, s0 = -1.0;
     uint32_t idx = 0, nst = 0;
     bool alive = false, exhausted = false;
-    int reloads = 0;
-    unsigned long long warp_steps = 0, ion_steps = 0;
+    unsigned reloads = 0, ion_steps = 0;       // per lane; < 2^32 for any run the queue allows
+    unsigned long long warp_steps = 0;
 
     while (true) {
         unsigned freem = __ballot_sync(FULL, !alive);
@@ -142,9 +150,11 @@ __global__ void __launch_bounds__(128, MINB) k_trace(const TraceParams P) {
         if (!__any_sync(FULL, alive)) { if (exhausted) break; else continue; }
         ++warp_steps;
         if (alive) {
-            // ---- stage 1 at (r, u); R of r also serves the out-of-grid test of the previous step
+            // ---- stage 1 at (r, u); its grid test is the out-of-grid test of the previous step (O4)
             double R2 = fma(X, X, Y * Y), rinv = tg_rsqrt(R2), R = R2 * rinv;
-            bool outside = (R < P.f.Rmin) | (R > P.f.Rmax) | (Z < P.f.Zmin) | (Z > P.f.Zmax);
+            double Bx, By, Bz;
+            bool outside = false, dummy = false;
+            tg_fieldB<KIND, CACHED, true>(P, cc, reloads, outside, X, Y, Z, t, R, rinv, Bx, By, Bz);
             if (outside || nst == P.max_steps) {
                 uint8_t fl = 0;
                 if (outside && (fabs(R - P.f.Rmin) < TG_GRAZE || fabs(R - P.f.Rmax) < TG_GRAZE ||
@@ -154,21 +164,19 @@ __global__ void __launch_bounds__(128, MINB) k_trace(const TraceParams P) {
                 P.steps[idx] = nst; P.flags[idx] = fl;
                 alive = false;
             } else {
-                double Bx, By, Bz;
-                tg_fieldB<KIND, CACHED>(P, cc, reloads, X, Y, Z, t, R, rinv, Bx, By, Bz);
                 double k1x = fma(Uy, Bz, -(Uz * By)), k1y = fma(Uz, Bx, -(Ux * Bz)), k1z = fma(Ux, By, -(Uy * Bx));
                 // ---- stage 2 (and 3, classical: same position)
                 double Xm = fma(k1x, P.a2, fma(Ux, P.a1, X)), Ym = fma(k1y, P.a2, fma(Uy, P.a1, Y)), Zm = fma(k1z, P.a2, fma(Uz, P.a1, Z));
                 double ux = fma(k1x, P.b1, Ux), uy = fma(k1y, P.b1, Uy), uz = fma(k1z, P.b1, Uz);
                 double tm = t + 0.5 * P.dt;
                 R2 = fma(Xm, Xm, Ym * Ym); rinv = tg_rsqrt(R2); R = R2 * rinv;
-                tg_fieldB<KIND, CACHED>(P, cc, reloads, Xm, Ym, Zm, tm, R, rinv, Bx, By, Bz);
+                tg_fieldB<KIND, CACHED>(P, cc, reloads, dummy, Xm, Ym, Zm, tm, R, rinv, Bx, By, Bz);
                 double k2x = fma(uy, Bz, -(uz * By)), k2y = fma(uz, Bx, -(ux * Bz)), k2z = fma(ux, By, -(uy * Bx));
                 ux = fma(k2x, P.b1, Ux); uy = fma(k2y, P.b1, Uy); uz = fma(k2z, P.b1, Uz);
                 if (P.variant) {               // printed Eq. 6: k3 position increment from k2
                     Xm = fma(k2x, P.a2, fma(Ux, P.a1, X)); Ym = fma(k2y, P.a2, fma(Uy, P.a1, Y)); Zm = fma(k2z, P.a2, fma(Uz, P.a1, Z));
                     R2 = fma(Xm, Xm, Ym * Ym); rinv = tg_rsqrt(R2); R = R2 * rinv;
-                    tg_fieldB<KIND, false>(P, cc, reloads, Xm, Ym, Zm, tm, R, rinv, Bx, By, Bz);
+                    tg_fieldB<KIND, false>(P, cc, reloads, dummy, Xm, Ym, Zm, tm, R, rinv, Bx, By, Bz);
                 }
                 double k3x = fma(uy, Bz, -(uz * By)), k3y = fma(uz, Bx, -(ux * Bz)), k3z = fma(ux, By, -(uy * Bx));
                 // ---- stage 4
@@ -176,7 +184,7 @@ __global__ void __launch_bounds__(128, MINB) k_trace(const TraceParams P) {
                        Ze = fma(k3z, 4.0 * P.a2, fma(Uz, 2.0 * P.a1, Z));
                 ux = fma(k3x, 2.0 * P.b1, Ux); uy = fma(k3y, 2.0 * P.b1, Uy); uz = fma(k3z, 2.0 * P.b1, Uz);
                 R2 = fma(Xe, Xe, Ye * Ye); rinv = tg_rsqrt(R2); R = R2 * rinv;
-                tg_fieldB<KIND, CACHED>(P, cc, reloads, Xe, Ye, Ze, t + P.dt, R, rinv, Bx, By, Bz);
+                tg_fieldB<KIND, CACHED>(P, cc, reloads, dummy, Xe, Ye, Ze, t + P.dt, R, rinv, Bx, By, Bz);
                 double k4x = fma(uy, Bz, -(uz * By)), k4y = fma(uz, Bx, -(ux * Bz)), k4z = fma(ux, By, -(uy * Bx));
                 // ---- Eq. 5
                 double Tx = k2x + k3x, Ty = k2y + k3y, Tz = k2z + k3z;
@@ -203,15 +211,15 @@ __global__ void __launch_bounds__(128, MINB) k_trace(const TraceParams P) {
         }
     }
     // per-warp statistics
-    unsigned long long ws = warp_steps;
+    unsigned long long rl = reloads, is = ion_steps;
     for (int o = 16; o > 0; o >>= 1) {
-        reloads += __shfl_down_sync(FULL, reloads, o);
-        ion_steps += __shfl_down_sync(FULL, ion_steps, o);
+        rl += __shfl_down_sync(FULL, rl, o);
+        is += __shfl_down_sync(FULL, is, o);
     }
     if (lane == 0) {
-        atomicAdd(&P.counters[1], ws);
-        atomicAdd(&P.counters[2], (unsigned long long)reloads);
-        atomicAdd(&P.counters[3], ion_steps);
+        atomicAdd(&P.counters[1], warp_steps);
+        atomicAdd(&P.counters[2], rl);
+        atomicAdd(&P.counters[3], is);
     }
 }
 
@@ -363,22 +371,24 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         launches += 5;
     }
     TG_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, 8 * sizeof(unsigned long long), st));
-    // kernel variants (option "variant"): 0 = register cell cache, 2 CTAs/SM (kind 0 only);
-    // 1 = uncached, 2 CTAs/SM; 2 = uncached, 4 CTAs/SM; 3 = cached, 3 CTAs/SM
+    // kernel variants (option "variant"), kind 0 with the classical RKN:
+    //   0: register cell cache, 2 x 128 threads/SM (254 regs)   3: cache, 3 x 128 (168 regs)
+    //   1: no cache, 2 x 128   2: no cache, 4 x 128 (128 regs)   (the only ones for kinds 1, 2)
     int kv = ctx->opt_variant;
-    if (ctx->field.kind != 0 || variant != 0) { if (kv == 0) kv = 1; if (kv == 3) kv = 2; }
+    if (ctx->field.kind != 0 || variant != 0) kv = (kv == 2 || kv == 3) ? 2 : 1;
+    const int threads = 128;
     int per_sm = ctx->opt_ctas_per_sm > 0 ? ctx->opt_ctas_per_sm : (kv == 2 ? 4 : (kv == 3 ? 3 : 2));
     unsigned grid = (unsigned)(ctx->sm_count * per_sm);
-    unsigned need = (unsigned)((ions->n + 127) / 128);
+    unsigned need = (unsigned)((ions->n + threads - 1) / threads);
     if (grid > need) grid = need;
-#define TG_LAUNCH(K, C, B) k_trace<K, C, B><<<grid, 128, 0, st>>>(P)
+#define TG_LAUNCH(K, C, T, B) k_trace<K, C, T, B><<<grid, T, 0, st>>>(P)
     switch (ctx->field.kind) {
     case 0:
-        if (kv == 0) TG_LAUNCH(0, true, 2); else if (kv == 3) TG_LAUNCH(0, true, 3);
-        else if (kv == 2) TG_LAUNCH(0, false, 4); else TG_LAUNCH(0, false, 2);
+        if (kv == 0) TG_LAUNCH(0, true, 128, 255); else if (kv == 3) TG_LAUNCH(0, true, 128, 168);
+        else if (kv == 2) TG_LAUNCH(0, false, 128, 128); else TG_LAUNCH(0, false, 128, 255);
         break;
-    case 1: if (kv == 2) TG_LAUNCH(1, false, 4); else TG_LAUNCH(1, false, 2); break;
-    default: if (kv == 2) TG_LAUNCH(2, false, 4); else TG_LAUNCH(2, false, 2); break;
+    case 1: if (kv == 2) TG_LAUNCH(1, false, 128, 128); else TG_LAUNCH(1, false, 128, 255); break;
+    default: if (kv == 2) TG_LAUNCH(2, false, 128, 128); else TG_LAUNCH(2, false, 128, 255); break;
     }
 #undef TG_LAUNCH
     ++launches;
