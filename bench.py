@@ -127,11 +127,10 @@ def main_ours(args):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    from paper_2506_15812_b200 import taiga, workloads as wl
+    from paper_2506_15812_b200 import sharding, taiga, workloads as wl
     dev = "cuda:%d" % local
-    cfg = wl.config(args.config, n_override=args.ions or None)
-    for g in cfg.groups:                        # weak scaling: every rank traces its own ions
-        g.first_index += rank << 40
+    # weak scaling: every rank traces its own cfg.n_ions ions (disjoint Philox counters)
+    cfg = sharding.shard_config(wl.config(args.config, n_override=args.ions or None), rank, world, "weak")
     grid, nodal = cfg.field_builder()
     nodal_dev = [torch.from_numpy(np.ascontiguousarray(c)).to(dev) for c in nodal]
     nodal_pin = [torch.from_numpy(np.ascontiguousarray(c)).pin_memory() for c in nodal]
@@ -178,8 +177,7 @@ def main_ours(args):
         else:
             for v, g in spans:
                 tg.detector_histogram(v, g.detector, cfg.n_hist, counts, summary)
-        if world > 1:
-            dist.all_reduce(counts); dist.all_reduce(summary)                            # exchange step: <= 0.5 MB
+        sharding.allreduce_counters(dist, counts, summary)                               # exchange step: <= 0.5 MB
         if host:
             counts_pin.copy_(counts, non_blocking=True); summary_pin.copy_(summary, non_blocking=True)
         if record:

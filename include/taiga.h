@@ -8,9 +8,11 @@
  *  - "dev" pointers are CUDA device pointers owned by the caller (e.g. torch tensors);
  *    "host" pointers are ordinary host memory, read during the call only.  The ctx owns only
  *    its internal tables / scratch and frees them in taiga_destroy.
- *  - All kernels are enqueued on the ctx's stream.  taiga_load_field, taiga_seed_beam and
- *    taiga_detector_histogram return without synchronising; taiga_trace synchronises the
- *    stream internally between compaction passes (it reads back one survivor counter).
+ *  - All kernels are enqueued on the ctx's stream and the caller synchronises.  Exceptions:
+ *    taiga_load_field synchronises once the first time it sees a new grid line length (it
+ *    uploads a host-built band operator); taiga_trace synchronises at its end only while the
+ *    "stats" option is on (default; it reads the counters back), taiga_field_table and
+ *    taiga_measure_fp64_peak always do.
  *  - Coordinates: right-handed Cartesian (X,Y,Z), Z vertical, torus axis = Z,
  *    R = sqrt(X^2+Y^2); (R,phi,Z) right-handed; SI units.
  *  - There is no CPU fallback: every entry point needs an sm_100 device.
@@ -146,12 +148,14 @@ int taiga_detector_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga
                              unsigned long long* summary_dev);
 
 /* ---- tuning / measurement hooks (not part of the method) */
-/* integer options: "sort" (1: order ions by birth cell before tracing, default 1),
- * "chunk0", "chunk" (steps per compaction pass), "min_active" (spill threshold),
- * "ctas_per_sm", "variant" (kernel variant), "stats" (collect counters). */
+/* integer options: "sort" (1: order the ion queue by birth cell before tracing, default 1),
+ * "sort_sub" (sort bins per grid cell and axis, default 16), "min_active" (a warp refills its
+ * free lanes from the queue when at least this many are free; 32 = whole tiles, default),
+ * "ctas_per_sm", "variant" (kernel variant: 0 register cell cache 8 warps/SM, 3 the same at
+ * 12 warps/SM, 1 / 2 no cache at 8 / 16 warps/SM), "stats" (1: read counters back, default). */
 int taiga_set_option(taiga_ctx* ctx, const char* key, long long value);
-/* counters of the last taiga_trace: [0] ion-steps, [1] warp-steps*32 (lane slots issued),
- * [2] passes, [3] kernel launches, [4] cell reloads, [5] survivors after pass 0. */
+/* counters of the last taiga_trace (valid with "stats" on): [0] ion-steps, [1] warp-steps*32
+ * (lane slots issued), [2] 1, [3] kernel launches, [4] cell refills, [5..7] 0. */
 int taiga_get_stats(taiga_ctx* ctx, unsigned long long stats_host[8]);
 /* register-resident DFMA microkernel: measured FP64 FMA instructions per second (thread-level,
  * i.e. lanes x instr) over ~`ms` milliseconds; the roofline denominator. */

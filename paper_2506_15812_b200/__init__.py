@@ -12,4 +12,4 @@ taiga     : thin ctypes binding of the C ABI in ``include/taiga.h`` (``libtaiga.
 Nothing is imported eagerly so that ``workloads`` can be used without the CUDA library.
 """
 
-__all__ = ["workloads", "taiga"]
+__all__ = ["workloads", "sharding", "taiga"]
