@@ -24,6 +24,9 @@ sys.path.insert(0, ROOT)
 # FP64-pipe instructions per ion-step of the classical RKN step on a 2-D bicubic field
 # (3 field evaluations x 61 + 4 cross products x 6 + stage/Eq.5/plane 45).
 ALG_FP64_INSTR_PER_ION_STEP = {0: 252.0, 1: 402.0, 2: 840.0}
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_trace launch on config 2, from the
+# `ncu --set full` capture summarised in profiles/r1c_trace_ncu.md (per launch; None elsewhere)
+NCU_DRAM_BYTES_PER_LAUNCH = {2: 233.7e6}
 
 
 def parse():
@@ -241,7 +244,8 @@ def main_ours(args):
         "gpu_launches": launches_per_step(cfg, kind) * args.steps,
         "roofline": {"bound": "alu", "achieved": 2e-12 * achieved, "peak": 2e-12 * peak_dfma,
                      "unit": "TFLOP/s (FP64 pipe; every FP64 instruction counted as one FMA = 2 flop)",
-                     "frac": achieved / peak_dfma, "traffic": None,
+                     "frac": achieved / peak_dfma,
+                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.config) if not args.ions else None,
                      "kernel": "k_trace", "alg_fp64_instr_per_ion_step": alg,
                      "peak_source": "measured live: register-resident DFMA microkernel (taiga_measure_fp64_peak); "
                                     "nominal 148 SM x 64 lanes x 1.965 GHz = 18.6e12 instr/s"},
