@@ -151,8 +151,10 @@ int taiga_detector_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga
 /* integer options: "sort" (1: order the ion queue by birth cell before tracing, default 1),
  * "sort_sub" (sort bins per grid cell and axis, default 16), "min_active" (a warp refills its
  * free lanes from the queue when at least this many are free; 32 = whole tiles, default),
- * "ctas_per_sm", "variant" (kernel variant: 0 register cell cache 8 warps/SM, 3 the same at
- * 12 warps/SM, 1 / 2 no cache at 8 / 16 warps/SM), "stats" (1: read counters back, default). */
+ * "ctas_per_sm", "variant" (kernel variant: 0 register cell cache with rolling predictive refill,
+ * 8 warps/SM (default); 4 predictive refill after each evaluation; 5 refill on demand only; 3 the
+ * same at 12 warps/SM; 1 / 2 no cache at 8 / 16 warps/SM), "stats" (1: read counters back,
+ * default). */
 int taiga_set_option(taiga_ctx* ctx, const char* key, long long value);
 /* counters of the last taiga_trace (valid with "stats" on): [0] ion-steps, [1] warp-steps*32
  * (lane slots issued), [2] 1, [3] kernel launches, [4] cell refills, [5..7] 0. */

@@ -28,6 +28,7 @@ struct TraceParams {
     double a1, a2, b1;                // dt/(2 qm), dt^2/8, qm dt/2   (stage 2/3)
     double c6, d6, dtq;               // dt^2/6, qm dt/6, dt/qm
     double qm, dt;
+    double pa1R, pa1Z;                // a1/hR, a1/hZ: half-step displacement in cells per unit u (predictive refill)
     uint32_t max_steps, n;
     int variant, refill_min;
     const double *x, *y, *z, *vx, *vy, *vz, *t0;
@@ -72,29 +73,69 @@ __device__ __forceinline__ double tg_horner16(const double* c, double p, double 
     return fma(fma(fma(r3, p, r2), p, r1), p, r0);
 }
 
-// Cartesian B at (X,Y,Z,t) given R2 = X^2+Y^2, rinv = 1/R, R.
+// Re-read the register cache for the cell that contains the global cell coordinates (pR, pZ)
+// (clamped to the grid: outside it the boundary cell extrapolates, reading A12).
+__device__ __forceinline__ void tg_refill(const TraceParams& P, CellCache<0>& cc, unsigned& reloads, double pR, double pZ) {
+    int i = tg_clampi(__double2int_rd(pR), 0, P.f.cR - 1), j = tg_clampi(__double2int_rd(pZ), 0, P.f.cZ - 1);
+    cc.oR = P.f.offR + (double)i; cc.oZ = P.f.offZ + (double)j;
+    const double* src = P.f.table + ((size_t)i * P.f.cZ + j) * 48;      // 384-B aligned
+#pragma unroll
+    for (int k = 0; k < 12; ++k)       // 12 x LDG.E.256 (sm_100: 256-bit global loads)
+        asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];"
+                     : "+d"(cc.c[4 * k]), "+d"(cc.c[4 * k + 1]), "+d"(cc.c[4 * k + 2]), "+d"(cc.c[4 * k + 3])
+                     : "l"(src + 4 * k));
+    ++reloads;
+}
+
+// (B_R, B_Z, B_phi) at (X,Y,Z,t) given R = sqrt(X^2+Y^2); cached path also returns the in-cell
+// coordinates (tR, tZ) relative to the cached cell.
 // FIRST (stage 1 of a step, cached path): also reports whether (R,Z) lies outside the grid; a
 // point inside the cached cell is inside the grid, so the four comparisons run only on a refill.
-template <int KIND, bool CACHED, bool FIRST = false>
-__device__ __forceinline__ void tg_fieldB(const TraceParams& P, CellCache<KIND>& cc, unsigned& reloads, bool& outside,
-                                          double X, double Y, double Z, double t, double R, double rinv,
-                                          double& Bx, double& By, double& Bz) {
-    double BR, BZ, Bp;
-    if constexpr (KIND == 0 && CACHED) {
-        double tR = fma(R, P.f.inv_hR, -cc.oR), tZ = fma(Z, P.f.inv_hZ, -cc.oZ);
+// 4 predicated 256-bit loads into 16 cached coefficients (rolling refill)
+__device__ __forceinline__ void tg_ldpred16(const double* src, int need, double* c) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+        asm volatile("{ .reg .pred p; setp.ne.s32 p, %5, 0; @p ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4]; }"
+                     : "+d"(c[4 * k]), "+d"(c[4 * k + 1]), "+d"(c[4 * k + 2]), "+d"(c[4 * k + 3])
+                     : "l"(src + 4 * k), "r"(need));
+}
+
+template <int KIND, bool CACHED, bool FIRST = false, bool ROLL = false>
+__device__ __forceinline__ void tg_fieldCyl(const TraceParams& P, CellCache<KIND>& cc, unsigned& reloads, bool& outside,
+                                            double X, double Y, double Z, double t, double R,
+                                            double& BR, double& BZ, double& Bp, double& tR, double& tZ,
+                                            double dR = 0.0, double dZ = 0.0) {
+    if constexpr (KIND == 0 && CACHED && ROLL) {
+        // Rolling predictive refill: the next stage's in-cell coordinates are predicted to ~1e-3
+        // cell (tRp, tZp); if they leave the cached cell, each part of the cache is re-read for
+        // the successor cell once this stage's Horner sums have consumed it, so the L2 round trip
+        // overlaps the rest of the stage.  Every stage still verifies its true coordinates
+        // against the cached cell first, so a wrong guess costs a second refill and nothing else.
+        tR = fma(R, P.f.inv_hR, -cc.oR); tZ = fma(Z, P.f.inv_hZ, -cc.oZ);
         if (!(tg_in01(tR) && tg_in01(tZ))) {
             if constexpr (FIRST) outside = (R < P.f.Rmin) | (R > P.f.Rmax) | (Z < P.f.Zmin) | (Z > P.f.Zmax);
-            double pR = fma(R, P.f.inv_hR, -P.f.offR), pZ = fma(Z, P.f.inv_hZ, -P.f.offZ);
-            int i = tg_clampi(__double2int_rd(pR), 0, P.f.cR - 1), j = tg_clampi(__double2int_rd(pZ), 0, P.f.cZ - 1);
-            cc.oR = P.f.offR + (double)i; cc.oZ = P.f.offZ + (double)j;
-            const double* src = P.f.table + ((size_t)i * P.f.cZ + j) * 48;      // 384-B aligned
-#pragma unroll
-            for (int k = 0; k < 12; ++k)       // 12 x LDG.E.256 (sm_100: 256-bit global loads)
-                asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];"
-                             : "=d"(cc.c[4 * k]), "=d"(cc.c[4 * k + 1]), "=d"(cc.c[4 * k + 2]), "=d"(cc.c[4 * k + 3])
-                             : "l"(src + 4 * k));
+            tg_refill(P, cc, reloads, fma(R, P.f.inv_hR, -P.f.offR), fma(Z, P.f.inv_hZ, -P.f.offZ));
             tR = fma(R, P.f.inv_hR, -cc.oR); tZ = fma(Z, P.f.inv_hZ, -cc.oZ);
+        }
+        double tRp = tR + dR, tZp = tZ + dZ;
+        int need = !(tg_in01(tRp) && tg_in01(tZp));
+        const double* src = P.f.table;
+        if (need) {
+            int i = tg_clampi(__double2int_rd(tRp + (cc.oR - P.f.offR)), 0, P.f.cR - 1);
+            int j = tg_clampi(__double2int_rd(tZp + (cc.oZ - P.f.offZ)), 0, P.f.cZ - 1);
+            cc.oR = P.f.offR + (double)i; cc.oZ = P.f.offZ + (double)j;
+            src += ((size_t)i * P.f.cZ + j) * 48;
             ++reloads;
+        }
+        BR = tg_horner16(cc.c, tR, tZ);      tg_ldpred16(src, need, cc.c);
+        BZ = tg_horner16(cc.c + 16, tR, tZ); tg_ldpred16(src + 16, need, cc.c + 16);
+        Bp = tg_horner16(cc.c + 32, tR, tZ); tg_ldpred16(src + 32, need, cc.c + 32);
+    } else if constexpr (KIND == 0 && CACHED) {
+        tR = fma(R, P.f.inv_hR, -cc.oR); tZ = fma(Z, P.f.inv_hZ, -cc.oZ);
+        if (!(tg_in01(tR) && tg_in01(tZ))) {
+            if constexpr (FIRST) outside = (R < P.f.Rmin) | (R > P.f.Rmax) | (Z < P.f.Zmin) | (Z > P.f.Zmax);
+            tg_refill(P, cc, reloads, fma(R, P.f.inv_hR, -P.f.offR), fma(Z, P.f.inv_hZ, -P.f.offZ));
+            tR = fma(R, P.f.inv_hR, -cc.oR); tZ = fma(Z, P.f.inv_hZ, -cc.oZ);
         }
         BR = tg_horner16(cc.c, tR, tZ); BZ = tg_horner16(cc.c + 16, tR, tZ); Bp = tg_horner16(cc.c + 32, tR, tZ);
     } else {
@@ -103,13 +144,29 @@ __device__ __forceinline__ void tg_fieldB(const TraceParams& P, CellCache<KIND>&
         if constexpr (KIND == 2) s = atan2(Y, X);
         tg_field_cyl(P.f, R, Z, s, BR, BZ, Bp);
     }
-    double c = X * rinv, s_ = Y * rinv;        // O0: B_X = B_R c - B_phi s, B_Y = B_R s + B_phi c
-    Bx = fma(BR, c, -(Bp * s_));
-    By = fma(BR, s_, Bp * c);
-    Bz = BZ;
 }
 
-template <int KIND, bool CACHED, int THREADS, int MAXREG>
+// Predictive refill (kind 0, cached): right after the Horner evaluation of one stage has read the
+// cached coefficients for the last time, the in-cell coordinates of the NEXT stage are predicted
+// to ~1e-3 cell (tRp, tZp); if they fall outside the cached cell its successor is loaded now, so
+// that the L2 round trip overlaps the rotation, cross product and 1/R chain in between.  The next
+// stage still tests its true coordinates against the cached cell, so a wrong guess costs a second
+// refill and nothing else.
+__device__ __forceinline__ void tg_predict(const TraceParams& P, CellCache<0>& cc, unsigned& reloads, double tRp, double tZp,
+                                           double BR, double BZ, double Bp) {
+    asm volatile("" ::"d"(BR), "d"(BZ), "d"(Bp));      // the stage's Horner sums are complete: the old coefficients are dead
+    if (!(tg_in01(tRp) && tg_in01(tZp)))
+        tg_refill(P, cc, reloads, tRp + (cc.oR - P.f.offR), tZp + (cc.oZ - P.f.offZ));
+}
+
+// O0: B_X = B_R c - B_phi s, B_Y = B_R s + B_phi c
+__device__ __forceinline__ void tg_rotate(double X, double Y, double rinv, double BR, double Bp, double& Bx, double& By) {
+    double c = X * rinv, s_ = Y * rinv;
+    Bx = fma(BR, c, -(Bp * s_));
+    By = fma(BR, s_, Bp * c);
+}
+
+template <int KIND, bool CACHED, int THREADS, int MAXREG, int PRED = 0>
 __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const TraceParams P) {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
@@ -124,9 +181,9 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
     unsigned long long warp_steps = 0;
 
     while (true) {
-        unsigned freem = __ballot_sync(FULL, !alive);
+        unsigned am = __ballot_sync(FULL, alive), freem = ~am;
         int nfree = __popc(freem);
-        if (!exhausted && (nfree >= P.refill_min || nfree == 32)) {
+        if (nfree >= P.refill_min && !exhausted) {
             unsigned long long base = 0;
             if (lane == 0) base = atomicAdd(&P.counters[0], (unsigned long long)nfree);
             base = __shfl_sync(FULL, base, 0);
@@ -146,15 +203,18 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                     alive = false;
                 }
             }
+            am = __ballot_sync(FULL, alive);
         }
-        if (!__any_sync(FULL, alive)) { if (exhausted) break; else continue; }
+        if (am == 0) { if (exhausted) break; else continue; }
         ++warp_steps;
         if (alive) {
             // ---- stage 1 at (r, u); its grid test is the out-of-grid test of the previous step (O4)
             double R2 = fma(X, X, Y * Y), rinv = tg_rsqrt(R2), R = R2 * rinv;
-            double Bx, By, Bz;
+            double Bx, By, Bz, BR, Bp, tR, tZ;
             bool outside = false, dummy = false;
-            tg_fieldB<KIND, CACHED, true>(P, cc, reloads, outside, X, Y, Z, t, R, rinv, Bx, By, Bz);
+            double dR = 0.0, dZ = 0.0;         // predicted half-step displacement in cells
+            if constexpr (PRED) { dR = (fma(X, Ux, Y * Uy) * rinv) * P.pa1R; dZ = Uz * P.pa1Z; }
+            tg_fieldCyl<KIND, CACHED, true, PRED == 2>(P, cc, reloads, outside, X, Y, Z, t, R, BR, Bz, Bp, tR, tZ, dR, dZ);
             if (outside || nst == P.max_steps) {
                 uint8_t fl = 0;
                 if (outside && (fabs(R - P.f.Rmin) < TG_GRAZE || fabs(R - P.f.Rmax) < TG_GRAZE ||
@@ -164,19 +224,24 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 P.steps[idx] = nst; P.flags[idx] = fl;
                 alive = false;
             } else {
+                if constexpr (PRED == 1) tg_predict(P, cc, reloads, tR + dR, tZ + dZ, BR, Bz, Bp);
+                tg_rotate(X, Y, rinv, BR, Bp, Bx, By);
                 double k1x = fma(Uy, Bz, -(Uz * By)), k1y = fma(Uz, Bx, -(Ux * Bz)), k1z = fma(Ux, By, -(Uy * Bx));
                 // ---- stage 2 (and 3, classical: same position)
                 double Xm = fma(k1x, P.a2, fma(Ux, P.a1, X)), Ym = fma(k1y, P.a2, fma(Uy, P.a1, Y)), Zm = fma(k1z, P.a2, fma(Uz, P.a1, Z));
                 double ux = fma(k1x, P.b1, Ux), uy = fma(k1y, P.b1, Uy), uz = fma(k1z, P.b1, Uz);
                 double tm = t + 0.5 * P.dt;
                 R2 = fma(Xm, Xm, Ym * Ym); rinv = tg_rsqrt(R2); R = R2 * rinv;
-                tg_fieldB<KIND, CACHED>(P, cc, reloads, dummy, Xm, Ym, Zm, tm, R, rinv, Bx, By, Bz);
+                tg_fieldCyl<KIND, CACHED, false, PRED == 2>(P, cc, reloads, dummy, Xm, Ym, Zm, tm, R, BR, Bz, Bp, tR, tZ, dR, dZ);
+                if constexpr (PRED == 1) tg_predict(P, cc, reloads, tR + dR, tZ + dZ, BR, Bz, Bp);
+                tg_rotate(Xm, Ym, rinv, BR, Bp, Bx, By);
                 double k2x = fma(uy, Bz, -(uz * By)), k2y = fma(uz, Bx, -(ux * Bz)), k2z = fma(ux, By, -(uy * Bx));
                 ux = fma(k2x, P.b1, Ux); uy = fma(k2y, P.b1, Uy); uz = fma(k2z, P.b1, Uz);
                 if (P.variant) {               // printed Eq. 6: k3 position increment from k2
                     Xm = fma(k2x, P.a2, fma(Ux, P.a1, X)); Ym = fma(k2y, P.a2, fma(Uy, P.a1, Y)); Zm = fma(k2z, P.a2, fma(Uz, P.a1, Z));
                     R2 = fma(Xm, Xm, Ym * Ym); rinv = tg_rsqrt(R2); R = R2 * rinv;
-                    tg_fieldB<KIND, false>(P, cc, reloads, dummy, Xm, Ym, Zm, tm, R, rinv, Bx, By, Bz);
+                    tg_fieldCyl<KIND, false>(P, cc, reloads, dummy, Xm, Ym, Zm, tm, R, BR, Bz, Bp, tR, tZ);
+                    tg_rotate(Xm, Ym, rinv, BR, Bp, Bx, By);
                 }
                 double k3x = fma(uy, Bz, -(uz * By)), k3y = fma(uz, Bx, -(ux * Bz)), k3z = fma(ux, By, -(uy * Bx));
                 // ---- stage 4
@@ -184,7 +249,8 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                        Ze = fma(k3z, 4.0 * P.a2, fma(Uz, 2.0 * P.a1, Z));
                 ux = fma(k3x, 2.0 * P.b1, Ux); uy = fma(k3y, 2.0 * P.b1, Uy); uz = fma(k3z, 2.0 * P.b1, Uz);
                 R2 = fma(Xe, Xe, Ye * Ye); rinv = tg_rsqrt(R2); R = R2 * rinv;
-                tg_fieldB<KIND, CACHED>(P, cc, reloads, dummy, Xe, Ye, Ze, t + P.dt, R, rinv, Bx, By, Bz);
+                tg_fieldCyl<KIND, CACHED>(P, cc, reloads, dummy, Xe, Ye, Ze, t + P.dt, R, BR, Bz, Bp, tR, tZ);
+                tg_rotate(Xe, Ye, rinv, BR, Bp, Bx, By);
                 double k4x = fma(uy, Bz, -(uz * By)), k4y = fma(uz, Bx, -(ux * Bz)), k4z = fma(ux, By, -(uy * Bx));
                 // ---- Eq. 5
                 double Tx = k2x + k3x, Ty = k2y + k3y, Tz = k2z + k3z;
@@ -357,6 +423,7 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     P.qm = qm; P.dt = dt;
     P.a1 = dt / (2.0 * qm); P.a2 = dt * dt / 8.0; P.b1 = qm * dt / 2.0;
     P.c6 = dt * dt / 6.0; P.d6 = qm * dt / 6.0; P.dtq = dt / qm;
+    P.pa1R = P.a1 * ctx->field.inv_hR; P.pa1Z = P.a1 * ctx->field.inv_hZ;
     P.max_steps = max_steps; P.n = (uint32_t)ions->n; P.variant = variant;
     P.refill_min = ctx->opt_min_active > 0 ? (ctx->opt_min_active > 32 ? 32 : ctx->opt_min_active) : 1;
     P.x = ions->x; P.y = ions->y; P.z = ions->z; P.vx = ions->vx; P.vy = ions->vy; P.vz = ions->vz; P.t0 = ions->t0;
@@ -372,19 +439,21 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     }
     TG_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, 8 * sizeof(unsigned long long), st));
     // kernel variants (option "variant"), kind 0 with the classical RKN:
-    //   0: register cell cache, 2 x 128 threads/SM (254 regs)   3: cache, 3 x 128 (168 regs)
+    //   0: register cell cache + rolling predictive refill, 2 x 128 threads/SM (254 regs)
+    //   4: cache + predictive refill after each Horner   5: cache, refill on demand only (r1c kernel)
+    //   3: cache on demand, 3 x 128 (168 regs)
     //   1: no cache, 2 x 128   2: no cache, 4 x 128 (128 regs)   (the only ones for kinds 1, 2)
     int kv = ctx->opt_variant;
-    if (ctx->field.kind != 0 || variant != 0) kv = (kv == 2 || kv == 3) ? 2 : 1;
+    if (ctx->field.kind != 0 || variant != 0) kv = (kv == 2 || kv == 3) ? 2 : 1;   // (the cached kernels assume k2 and k3 share their position)
     const int threads = 128;
     int per_sm = ctx->opt_ctas_per_sm > 0 ? ctx->opt_ctas_per_sm : (kv == 2 ? 4 : (kv == 3 ? 3 : 2));
     unsigned grid = (unsigned)(ctx->sm_count * per_sm);
     unsigned need = (unsigned)((ions->n + threads - 1) / threads);
     if (grid > need) grid = need;
-#define TG_LAUNCH(K, C, T, B) k_trace<K, C, T, B><<<grid, T, 0, st>>>(P)
+#define TG_LAUNCH(K, C, T, B, ...) k_trace<K, C, T, B, ##__VA_ARGS__><<<grid, T, 0, st>>>(P)
     switch (ctx->field.kind) {
     case 0:
-        if (kv == 0) TG_LAUNCH(0, true, 128, 255); else if (kv == 3) TG_LAUNCH(0, true, 128, 168);
+        if (kv == 0) TG_LAUNCH(0, true, 128, 255, 2); else if (kv == 4) TG_LAUNCH(0, true, 128, 255, 1); else if (kv == 5) TG_LAUNCH(0, true, 128, 255); else if (kv == 3) TG_LAUNCH(0, true, 128, 168);
         else if (kv == 2) TG_LAUNCH(0, false, 128, 128); else TG_LAUNCH(0, false, 128, 255);
         break;
     case 1: if (kv == 2) TG_LAUNCH(1, false, 128, 128); else TG_LAUNCH(1, false, 128, 255); break;
