@@ -4,18 +4,19 @@
 #pragma once
 #include "taiga_internal.h"
 
-__device__ __forceinline__ double2 tg_ld2(const double* p) {
-    return __ldg(reinterpret_cast<const double2*>(p));
+// 16 coefficients [a][b] at c (32-byte aligned: one 128-B line, four 256-bit loads): Horner in w
+// inside, in p outside.
+__device__ __forceinline__ void tg_ld4(const double* p, double& a, double& b, double& c, double& d) {
+    asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
 }
-
-// 16 coefficients [a][b] at c (16-byte aligned): Horner in w inside, in p outside.
 __device__ __forceinline__ double tg_bicubic(const double* __restrict__ c, double p, double w) {
-    double2 a0 = tg_ld2(c + 0), a1 = tg_ld2(c + 2), b0 = tg_ld2(c + 4), b1 = tg_ld2(c + 6);
-    double2 c0 = tg_ld2(c + 8), c1 = tg_ld2(c + 10), d0 = tg_ld2(c + 12), d1 = tg_ld2(c + 14);
-    double r0 = fma(fma(fma(a1.y, w, a1.x), w, a0.y), w, a0.x);
-    double r1 = fma(fma(fma(b1.y, w, b1.x), w, b0.y), w, b0.x);
-    double r2 = fma(fma(fma(c1.y, w, c1.x), w, c0.y), w, c0.x);
-    double r3 = fma(fma(fma(d1.y, w, d1.x), w, d0.y), w, d0.x);
+    double a0, a1, a2, a3, b0, b1, b2, b3, c0, c1, c2, c3, d0, d1, d2, d3;
+    tg_ld4(c, a0, a1, a2, a3); tg_ld4(c + 4, b0, b1, b2, b3);
+    tg_ld4(c + 8, c0, c1, c2, c3); tg_ld4(c + 12, d0, d1, d2, d3);
+    double r0 = fma(fma(fma(a3, w, a2), w, a1), w, a0);
+    double r1 = fma(fma(fma(b3, w, b2), w, b1), w, b0);
+    double r2 = fma(fma(fma(c3, w, c2), w, c1), w, c0);
+    double r3 = fma(fma(fma(d3, w, d2), w, d1), w, d0);
     return fma(fma(fma(r3, p, r2), p, r1), p, r0);
 }
 

@@ -302,7 +302,7 @@ struct SortParams {
     const double *x, *y, *z, *t0;
     uint32_t n;
     double Rmin, Zmin, minwR, minwZ, s0, inv_ds;
-    int n_major, nS;
+    int n_major, nS, kind;
     unsigned long long* bbox;          // [4]: min a, max a, min b, max b (bit patterns of doubles >= 0)
 };
 
@@ -339,9 +339,13 @@ __device__ __forceinline__ uint32_t sort_key(const SortParams& S, uint32_t i) {
     double wR = fmax((a1 - a0) / SORT_NBR, S.minwR), wZ = fmax((b1 - b0) / SORT_NBZ, S.minwZ);
     int bR = min(max((int)((a - a0) / wR), 0), SORT_NBR - 1), bZ = min(max((int)((b - b0) / wZ), 0), SORT_NBZ - 1);
     int m = 0;
-    if (S.n_major > 1 && S.t0) {
+    if (S.n_major > 1 && S.kind == 1) {             // time slices: major key = slice of birth
         int k = min(max((int)floor((S.t0[i] - S.s0) * S.inv_ds), 0), S.nS - 1);
         m = (int)(((long long)k * S.n_major) / S.nS);
+    } else if (S.n_major > 1) {                     // phi planes: major key = toroidal (sub-)cell of birth
+        double xs = (atan2(S.y[i], S.x[i]) - S.s0) * S.inv_ds;
+        xs -= (double)S.nS * floor(xs / (double)S.nS);
+        m = min(max((int)(xs * (double)S.n_major / (double)S.nS), 0), S.n_major - 1);
     }
     return (uint32_t)((m * SORT_NBR + bR) * SORT_NBZ + bZ);
 }
@@ -386,7 +390,7 @@ __global__ void k_sort_scatter(SortParams S, uint32_t* bins, const uint32_t* sum
 static int build_order(taiga_ctx* ctx, const taiga_ions* ions) {
     const FieldDev& f = ctx->field;
     uint32_t n = (uint32_t)ions->n;
-    int n_major = (f.kind == 1 && ions->t0) ? (f.nS < 64 ? f.nS : 64) : 1;
+    int n_major = (f.kind == 1 && ions->t0) ? (f.nS < 64 ? f.nS : 64) : (f.kind == 2 ? 64 : 1);
     uint32_t nb = (uint32_t)n_major * SORT_NBR * SORT_NBZ;
     uint32_t nblk = (nb + SCAN_TPB * SCAN_ITEMS - 1) / (SCAN_TPB * SCAN_ITEMS);   // <= 1024
     int rc = tg_reserve(ctx, &ctx->order, &ctx->cap_order, (size_t)n);
@@ -403,7 +407,7 @@ static int build_order(taiga_ctx* ctx, const taiga_ions* ions) {
     S.Rmin = f.Rmin; S.Zmin = f.Zmin;
     int sub = ctx->opt_sort_sub > 0 ? ctx->opt_sort_sub : 4;
     S.minwR = 1.0 / (f.inv_hR * sub); S.minwZ = 1.0 / (f.inv_hZ * sub);
-    S.s0 = f.s0; S.inv_ds = f.inv_ds; S.n_major = n_major; S.nS = f.nS;
+    S.s0 = f.s0; S.inv_ds = f.inv_ds; S.n_major = n_major; S.nS = f.nS; S.kind = f.kind;
     S.bbox = ctx->counters + 8;
     unsigned gb = (n + 255) / 256;
     k_sort_bbox<<<gb, 256, 0, st>>>(S);

@@ -297,3 +297,70 @@ def test_cfg2_full_size_bench_configuration(tg):
     # mean steps / structure of the workload (SURVEY 8(d) probe: ~1038 steps/ion, 96.3 % cross)
     assert 900 < st["ion_steps"] / cfg.n_ions < 1200
     assert 0.955 < (s[0] + s[1]) / cfg.n_ions < 0.97
+
+
+def _full_size_check(tg, icfg, windows, width, max_flag_frac=0.01):
+    """A BASELINE config at FULL size: invariants that hold at any size, plus windows of
+    consecutive ions per group re-seeded and re-traced one by one by the oracle."""
+    from paper_2506_15812_b200 import taiga
+    cfg = wl.config(icfg)
+    ions, counts, summary = taiga.run_config(tg, cfg)
+    torch.cuda.synchronize()
+    s = _np(summary)
+    assert s[:, :5].sum() == cfg.n_ions                                   # O5 counting invariant
+    assert np.array_equal(s[:, 0], _np(counts).reshape(cfg.n_hist, -1).sum(axis=1))
+    cell_all = ions.cell
+    assert int((cell_all >= 0).sum().item()) == int(s[:, 0].sum())
+    assert int((cell_all < -4).sum().item()) == 0
+    grid, nodal = cfg.field_builder()
+    f = orc.OracleField(grid, nodal)
+    cd, cn = wl.depth_cdf(), wl.normal_cdf()
+    rng = np.random.default_rng(100 + icfg)
+    off, n_cmp, n_flag, max_d = 0, 0, 0, 0.0
+    for g in cfg.groups:
+        det = cfg.detector or g.detector
+        for lo in sorted(rng.integers(0, g.n_ions - width, windows).tolist()) + [g.n_ions - width]:
+            v = ions.view(off + lo, off + lo + width)
+            seeds = orc.seed(g.beam, cd, cn, cfg.seed, g.first_index + lo, width)
+            state = [_np(v.a[k]) for k in ("x", "y", "z", "vx", "vy", "vz")]
+            for a, b in zip(state, seeds):
+                assert np.array_equal(a, b), (icfg, g.group, lo)
+            t0 = np.full(width, g.t0) if grid.kind == 1 else None
+            res = orc.trace(f, g.beam.charge_C / g.beam.mass_kg, state, t0, cfg.dt, cfg.max_steps, det)
+            orc.histogram(res, None, det, 1)
+            fl = (_np(v.flags) | res["flags"]) != 0
+            ok = ~fl
+            assert np.array_equal(_np(v.cell)[ok], res["cell"][ok]), (icfg, g.group, lo)
+            assert np.array_equal(_np(v.steps)[ok].astype(np.uint32), res["steps"][ok]), (icfg, g.group, lo)
+            assert np.all(_np(v.group) == g.group)
+            cr = ok & (res["status"] == 0)
+            if cr.any():
+                max_d = max(max_d, np.abs(_np(v.hit_u)[cr] - res["u"][cr]).max(), np.abs(_np(v.hit_w)[cr] - res["w"][cr]).max())
+            n_cmp += width
+            n_flag += int(fl.sum())
+        off += g.n_ions
+    assert max_d < TOL_UW, max_d
+    assert n_flag <= max(4, int(max_flag_frac * n_cmp))
+    return cfg, s
+
+
+def test_cfg3_full_size_energy_scan(tg):
+    """16,777,216 ions, four energies with their own detectors, 2 mrad divergence."""
+    cfg, s = _full_size_check(tg, 3, windows=3, width=96)
+    frac = (s[:, 0] + s[:, 1]) / (cfg.n_ions / 4)
+    # SURVEY 8(d) probe: crossers 69.5 / 90.6 / 96.3 / 98.1 %
+    assert np.all(np.abs(frac - np.array([0.695, 0.906, 0.963, 0.981])) < 0.02), frac
+
+
+def test_cfg4_full_size_time_slices(tg):
+    """2,097,152 Na+ ions over 64 time slices, one histogram per slice."""
+    cfg, s = _full_size_check(tg, 4, windows=1, width=64)
+    assert np.all(s[:, :5].sum(axis=1) == cfg.n_ions // 64)
+    assert 0.99 < (s[:, 0] + s[:, 1]).sum() / cfg.n_ions < 1.0
+
+
+def test_cfg5_full_size_ripple_3d(tg):
+    """67,108,864 ions in the periodic-tricubic (R, Z, phi) field: the largest configuration
+    (6.2 GB of ion state, 1.6 GB of tables)."""
+    cfg, s = _full_size_check(tg, 5, windows=2, width=64)
+    assert 0.95 < (s[0, 0] + s[0, 1]) / cfg.n_ions < 0.975
