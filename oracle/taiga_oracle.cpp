@@ -307,11 +307,83 @@ static inline void rkn_step(const orc_field* f, double qm, int variant, const do
     }
 }
 
+/* Eq. 4: the equation of motion as a first-order system in the generalised
+ * coordinate y = (r1,r2,r3,v1,v2,v3), dy/dt = f(y,t) with f_{1..3} = y_{4..6} and f_{4..6} =
+ * (q/m)(E + v x B); "solved by a fourth-order Runge-Kutta method" (L210): the classical RK4
+ *  K1=f(y,t); K2=f(y+K1 dt/2,t+dt/2); K3=f(y+K2 dt/2,t+dt/2); K4=f(y+K3 dt,t+dt);
+ *  y'=y+(K1+2K2+2K3+K4) dt/6.   (Reading R1 in DESIGN.md: L191 calls the solver "quadratic";
+ *  L210 and ref. [29] fix the fourth-order scheme.)                                          */
+static inline void rk4_f(const orc_field* f, double qm, const double y[6], double t, double dy[6]) {
+    dy[0] = y[3]; dy[1] = y[4]; dy[2] = y[5];
+    accel(f, qm, y, y + 3, t, dy + 3);
+}
+static inline void rk4_step(const orc_field* f, double qm, const double r[3], const double v[3],
+                            double t, double dt, double rn[3], double vn[3]) {
+    double y[6] = {r[0], r[1], r[2], v[0], v[1], v[2]}, ys[6], K1[6], K2[6], K3[6], K4[6];
+    rk4_f(f, qm, y, t, K1);
+    for (int c = 0; c < 6; ++c) ys[c] = y[c] + K1[c] * (dt / 2.0);
+    rk4_f(f, qm, ys, t + dt / 2.0, K2);
+    for (int c = 0; c < 6; ++c) ys[c] = y[c] + K2[c] * (dt / 2.0);
+    rk4_f(f, qm, ys, t + dt / 2.0, K3);
+    for (int c = 0; c < 6; ++c) ys[c] = y[c] + K3[c] * dt;
+    rk4_f(f, qm, ys, t + dt, K4);
+    for (int c = 0; c < 3; ++c) {
+        rn[c] = y[c] + (K1[c] + 2.0 * K2[c] + 2.0 * K3[c] + K4[c]) * (dt / 6.0);
+        vn[c] = y[c + 3] + (K1[c + 3] + 2.0 * K2[c + 3] + 2.0 * K3[c + 3] + K4[c + 3]) * (dt / 6.0);
+    }
+}
+
+static inline void cross3(const double a[3], const double b[3], double c[3]) {
+    c[0] = a[1] * b[2] - a[2] * b[1]; c[1] = a[2] * b[0] - a[0] * b[2]; c[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+/* Eq. 7: Boris push of the velocity over a step h, B and E taken at r, t:
+ *  v- = v + (q/m) E h/2;  t = (q/m) B h/2;  s = 2t/(1+t.t);  v* = v- + v- x t;
+ *  v+ = v- + v* x s;  v' = v+ + (q/m) E h/2   (first line of Eq. 8).                         */
+static inline void boris_velocity(const orc_field* f, double qm, const double r[3], const double v[3],
+                                  double t, double h, double vn[3]) {
+    double B[3], vm[3], tv[3], sv[3], vs[3], vp[3], c1[3], c2[3];
+    orc_field_B(f, r, t, B);
+    double tt = 0.0;
+    for (int c = 0; c < 3; ++c) { vm[c] = v[c] + qm * f->E[c] * (h / 2.0); tv[c] = qm * B[c] * (h / 2.0); tt += tv[c] * tv[c]; }
+    for (int c = 0; c < 3; ++c) sv[c] = 2.0 * tv[c] / (1.0 + tt);
+    cross3(vm, tv, c1);
+    for (int c = 0; c < 3; ++c) vs[c] = vm[c] + c1[c];
+    cross3(vs, sv, c2);
+    for (int c = 0; c < 3; ++c) { vp[c] = vm[c] + c2[c]; vn[c] = vp[c] + qm * f->E[c] * (h / 2.0); }
+}
+/* Eq. 8, second line (L266): position.  As printed, r(t0+dt) = r(t0) + v(t0) dt uses the OLD
+ * velocity: explicit Euler in r, first order, while the text calls the solver "a second-order
+ * Verlet solver with a Boris push" (L249).  Reading R2: solver 3 is the Verlet /
+ * leap-frog form of refs [32,33], r(t0+dt) = r(t0) + v' dt with the velocity living at half
+ * steps (boris_start below); solver 4 is Eq. 8 exactly as printed, no start correction.      */
+static inline void boris_step(const orc_field* f, double qm, bool printed, const double r[3], const double v[3],
+                              double t, double dt, double rn[3], double vn[3]) {
+    boris_velocity(f, qm, r, v, t, dt, vn);
+    for (int c = 0; c < 3; ++c) rn[c] = r[c] + (printed ? v[c] : vn[c]) * dt;
+}
+/* leap-frog start of solver 3: v(t0) -> v(t0 - dt/2) by a Boris push over -dt/2 at (r0, t0) */
+static inline void boris_start(const orc_field* f, double qm, const double r[3], double v[3], double t, double dt) {
+    double vb[3];
+    boris_velocity(f, qm, r, v, t, -dt / 2.0, vb);
+    for (int c = 0; c < 3; ++c) v[c] = vb[c];
+}
+
+/* solver codes: 0 RKN classical (A1), 1 RKN with the printed k3, 2 linearised RK4 (Eq. 4),
+ * 3 Boris-Verlet (Eq. 7-8, reading R2), 4 Boris with Eq. 8 as printed */
+static inline void solver_step(const orc_field* f, double qm, int solver, const double r[3], const double v[3],
+                               double t, double dt, double rn[3], double vn[3]) {
+    if (solver == 2) rk4_step(f, qm, r, v, t, dt, rn, vn);
+    else if (solver == 3 || solver == 4) boris_step(f, qm, solver == 4, r, v, t, dt, rn, vn);
+    else rkn_step(f, qm, solver, r, v, t, dt, rn, vn);
+}
+
 extern "C" void orc_rkn_advance(const orc_field* f, double qm, int variant, double r[3], double v[3],
                                 double* t, double dt, uint64_t nsteps) {
+    if (variant == 3) boris_start(f, qm, r, v, *t, dt);     /* every call is a fresh start */
     for (uint64_t s = 0; s < nsteps; ++s) {
         double rn[3], vn[3];
-        rkn_step(f, qm, variant, r, v, *t, dt, rn, vn);
+        solver_step(f, qm, variant, r, v, *t, dt, rn, vn);
         for (int c = 0; c < 3; ++c) { r[c] = rn[c]; v[c] = vn[c]; }
         *t = *t + dt;
     }
@@ -355,11 +427,12 @@ extern "C" void orc_trace(const orc_field* f, double qm, int variant, uint64_t n
         bool inside = in_grid(f, r, &gz);
         if (gz) fl |= 4;
         if (!(s0 < 0.0) || !inside) { status[i] = -4; steps[i] = 0; flags[i] = fl; continue; }
+        if (variant == 3) boris_start(f, qm, r, v, t, dt);
         int32_t st = -2;
         uint32_t nst = max_steps;
         for (uint32_t step = 1; step <= max_steps; ++step) {
             double rn[3], vn[3];
-            rkn_step(f, qm, variant, r, v, t, dt, rn, vn);
+            solver_step(f, qm, variant, r, v, t, dt, rn, vn);
             double s1 = det->normal[0] * (rn[0] - det->origin[0]) + det->normal[1] * (rn[1] - det->origin[1]) +
                         det->normal[2] * (rn[2] - det->origin[2]);
             if (std::fabs(s1) < GRAZE) fl |= 2;

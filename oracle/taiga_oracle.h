@@ -11,7 +11,9 @@
  * P5 kinetic-energy bound; P6 canonical momentum in axisymmetric fields; P7 step-halving
  * order; P8 magnetic moment / grad-B drift; P9 spline properties + scipy cross-check;
  * P10 CDF inversion exactness + statistics; P11 straight-line plane hit + brute-force
- * binning; P12 independent naive evaluator end to end.
+ * binning; P12 independent naive evaluator end to end; P13 RK4 (Eq. 4) amplification factor,
+ * order and agreement with RKN; P14 Boris (Eq. 7-8) exact |v|, rotation angle 2 atan(z/2),
+ * E x B drift, order of both position readings; P15 the three solvers agree as dt -> 0 (L294).
  * Parity unpinned: nothing in this file; the paper's own figures that cannot be pinned
  * (Fig. 10 loss rate, Table 1, Fig. 12 curves) are listed in DESIGN.md.
  *
@@ -37,7 +39,7 @@ typedef struct {
     double Rmin, Rmax, Zmin, Zmax, s0, ds;
     const double* coef[3];   /* BR, BZ, Bphi per-cell power-basis tables (orc_build_tables) */
     double par[8];           /* analytic-field parameters */
-    double E[3];             /* uniform electric field (pins P4 only; 0 otherwise)      */
+    double E[3];             /* uniform electric field (Eq. 3; L175 "parametric modeling")  */
 } orc_field;
 
 typedef struct {
@@ -77,8 +79,11 @@ void orc_field_B(const orc_field* f, const double r[3], double t, double B[3]);
 /* field components in the poloidal plane, (B_R,B_Z,B_phi), s = time or phi */
 void orc_field_cyl(const orc_field* f, double R, double Z, double s, double Bc[3]);
 
-/* O3  nsteps RKN steps of one ion, no termination tests (pins). variant 0 = classical
- *     Nystrom (A1 default), 1 = k3 position from k2 (the printed Eq. 6 k3). */
+/* O3  nsteps integrator steps of one ion, no termination tests (pins).  variant = solver code:
+ *     0 = classical Nystrom (Eq. 5-6, A1 default), 1 = k3 position from k2 (the printed Eq. 6 k3),
+ *     2 = linearised RK4 on y = (r, v) (Eq. 4), 3 = Boris-Verlet (Eq. 7-8 with r advanced by the
+ *     NEW velocity, reading R2), 4 = Boris with Eq. 8 as printed (r advanced by the old velocity).
+ *     f->E (uniform, "parametric" electric field, L175) enters every solver through Eq. 3. */
 void orc_rkn_advance(const orc_field* f, double qm, int variant, double r[3], double v[3],
                      double* t, double dt, uint64_t nsteps);
 
