@@ -130,13 +130,25 @@ typedef struct {
 
 /* ---- a3 + a4: integrator and termination (Eq. 3; Eq. 5-6 L218-235 with
  * readings A1-A3; L326 stop at the plane or at max_steps; L338 two-state storage and linear
- * interpolation to the plane; L318 error value).  E = 0.  charge_C/mass_kg of the LAST
+ * interpolation to the plane; L318 error value).  charge_C/mass_kg of the LAST
  * taiga_seed_beam call is NOT implied: q/m is passed explicitly.
  * Writes hit_u, hit_w, cell (TAIGA_CELL_MISS for every plane-crossing ion, or an error code),
- * steps, flags.  rkn_variant: 0 = classical Nystrom (default reading A1), 1 = k3 position
- * increment from k2 (Eq. 6 as printed). */
+ * steps, flags.
+ * solver: 0 = Runge-Kutta-Nystrom, classical stages (default reading A1; the production path),
+ *         1 = RKN with the k3 position increment from k2 (Eq. 6 as printed),
+ *         2 = linearised fourth-order Runge-Kutta on y = (r, v) (Eq. 4),
+ *         3 = Boris-Verlet (Eq. 7-8) in its leap-frog form: r(t0+dt) = r(t0) + v' dt,
+ *             v(t0) moved to t0 - dt/2 by one Boris push at the start (reading R2: "a
+ *             second-order Verlet solver"),
+ *         4 = Boris with Eq. 8 exactly as printed: r(t0+dt) = r(t0) + v(t0) dt (first order).
+ * E of Eq. 3 is the uniform field set by taiga_set_efield (default 0). */
 int taiga_trace(taiga_ctx* ctx, taiga_ions* ions, double q_over_m, double dt,
-                uint32_t max_steps, const taiga_detector* det, int rkn_variant);
+                uint32_t max_steps, const taiga_detector* det, int solver);
+
+/* Uniform electric field E [V/m] of Eq. 3 ("we can use parametric modeling
+ * for it"; verification scenarios 2 and 5, L279, L282).  Host pointer, copied.  Applies to all
+ * later taiga_trace calls of this ctx; (0,0,0) restores the E = 0 production kernels. */
+int taiga_set_efield(taiga_ctx* ctx, const double E_V_per_m[3]);
 
 /* ---- a5: binning + histogram (segment ID per ion; atomically summed
  * per-segment counters; only the compact counter array is returned).

@@ -146,12 +146,19 @@ extern "C" int taiga_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double d
     if (rc) return rc;
     rc = check_det(ctx, det, false);
     if (rc) return rc;
-    if (!(dt > 0) || !isfinite(qm) || qm == 0 || (variant != 0 && variant != 1)) { TG_SET_ERR(ctx, "trace: bad dt / q_over_m / variant"); return TAIGA_E_ARG; }
+    if (!(dt > 0) || !isfinite(qm) || qm == 0 || variant < 0 || variant > 4) { TG_SET_ERR(ctx, "trace: bad dt / q_over_m / solver"); return TAIGA_E_ARG; }
     if (ions->n == 0) return TAIGA_OK;
     TG_CUDA(ctx, cudaSetDevice(ctx->device));
     DetDev dd;
     for (int c = 0; c < 3; ++c) { dd.origin[c] = det->origin[c]; dd.normal[c] = det->normal[c]; dd.eu[c] = det->eu[c]; dd.ew[c] = det->ew[c]; }
     return tg_trace(ctx, ions, qm, dt, max_steps, dd, variant);
+}
+
+extern "C" int taiga_set_efield(taiga_ctx* ctx, const double E[3]) {
+    if (!ctx || !E) return TAIGA_E_ARG;
+    for (int c = 0; c < 3; ++c) if (!isfinite(E[c])) { TG_SET_ERR(ctx, "set_efield: non-finite component"); return TAIGA_E_ARG; }
+    for (int c = 0; c < 3; ++c) ctx->E[c] = E[c];
+    return TAIGA_OK;
 }
 
 extern "C" int taiga_detector_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,

@@ -38,6 +38,8 @@ struct taiga_ctx {
     double* scratch;          size_t scratch_bytes;     // precompute work arrays
     double* band[2];          size_t band_cap[2]; int band_n[2];   // y -> y'' band operators (Z, R)
 
+    double E[3];                                         // uniform electric field (taiga_set_efield), V/m
+
     // seeding tables
     double *cdf_depth, *cdf_normal;  int cap_depth, cap_normal;
 

@@ -28,6 +28,7 @@ struct TraceParams {
     double a1, a2, b1;                // dt/(2 qm), dt^2/8, qm dt/2   (stage 2/3)
     double c6, d6, dtq;               // dt^2/6, qm dt/6, dt/qm
     double qm, dt;
+    double qE[3], eh[3];              // (q/m) E [m/s^2];  (q/m)^2 E dt/2 (Boris half kick in u units)
     double pa1R, pa1Z;                // a1/hR, a1/hZ: half-step displacement in cells per unit u (predictive refill)
     uint32_t max_steps, n;
     int variant, refill_min;
@@ -166,7 +167,19 @@ __device__ __forceinline__ void tg_rotate(double X, double Y, double rinv, doubl
     By = fma(BR, s_, Bp * c);
 }
 
-template <int KIND, bool CACHED, int THREADS, int MAXREG, int PRED = 0>
+// Cartesian B at a stage point (on-demand cache refill / uncached gather); solvers other than RKN
+template <int KIND, bool CACHED>
+__device__ __forceinline__ void tg_fieldXYZ(const TraceParams& P, CellCache<KIND>& cc, unsigned& reloads,
+                                            double Xs, double Ys, double Zs, double ts, double& bx, double& by, double& bz) {
+    double r2 = fma(Xs, Xs, Ys * Ys), ri = tg_rsqrt(r2), Rs = r2 * ri, br, bp, tR, tZ;
+    bool dummy = false;
+    tg_fieldCyl<KIND, CACHED>(P, cc, reloads, dummy, Xs, Ys, Zs, ts, Rs, br, bz, bp, tR, tZ);
+    tg_rotate(Xs, Ys, ri, br, bp, bx, by);
+}
+
+// SOLVER: 0 Runge-Kutta-Nystrom (Eq. 5-6), 2 linearised RK4 (Eq. 4), 3 Boris (Eq. 7-8; P.variant 3 =
+// Verlet form with leap-frog start, 4 = Eq. 8 as printed).  HAS_E: uniform E of Eq. 3 added to every k.
+template <int KIND, bool CACHED, int THREADS, int MAXREG, int PRED = 0, int SOLVER = 0, bool HAS_E = false>
 __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const TraceParams P) {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
@@ -224,9 +237,12 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 P.steps[idx] = nst; P.flags[idx] = fl;
                 alive = false;
             } else {
+                double Xn, Yn, Zn;
+                if constexpr (SOLVER == 0) {
                 if constexpr (PRED == 1) tg_predict(P, cc, reloads, tR + dR, tZ + dZ, BR, Bz, Bp);
                 tg_rotate(X, Y, rinv, BR, Bp, Bx, By);
                 double k1x = fma(Uy, Bz, -(Uz * By)), k1y = fma(Uz, Bx, -(Ux * Bz)), k1z = fma(Ux, By, -(Uy * Bx));
+                if constexpr (HAS_E) { k1x += P.qE[0]; k1y += P.qE[1]; k1z += P.qE[2]; }
                 // ---- stage 2 (and 3, classical: same position)
                 double Xm = fma(k1x, P.a2, fma(Ux, P.a1, X)), Ym = fma(k1y, P.a2, fma(Uy, P.a1, Y)), Zm = fma(k1z, P.a2, fma(Uz, P.a1, Z));
                 double ux = fma(k1x, P.b1, Ux), uy = fma(k1y, P.b1, Uy), uz = fma(k1z, P.b1, Uz);
@@ -236,6 +252,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 if constexpr (PRED == 1) tg_predict(P, cc, reloads, tR + dR, tZ + dZ, BR, Bz, Bp);
                 tg_rotate(Xm, Ym, rinv, BR, Bp, Bx, By);
                 double k2x = fma(uy, Bz, -(uz * By)), k2y = fma(uz, Bx, -(ux * Bz)), k2z = fma(ux, By, -(uy * Bx));
+                if constexpr (HAS_E) { k2x += P.qE[0]; k2y += P.qE[1]; k2z += P.qE[2]; }
                 ux = fma(k2x, P.b1, Ux); uy = fma(k2y, P.b1, Uy); uz = fma(k2z, P.b1, Uz);
                 if (P.variant) {               // printed Eq. 6: k3 position increment from k2
                     Xm = fma(k2x, P.a2, fma(Ux, P.a1, X)); Ym = fma(k2y, P.a2, fma(Uy, P.a1, Y)); Zm = fma(k2z, P.a2, fma(Uz, P.a1, Z));
@@ -244,6 +261,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                     tg_rotate(Xm, Ym, rinv, BR, Bp, Bx, By);
                 }
                 double k3x = fma(uy, Bz, -(uz * By)), k3y = fma(uz, Bx, -(ux * Bz)), k3z = fma(ux, By, -(uy * Bx));
+                if constexpr (HAS_E) { k3x += P.qE[0]; k3y += P.qE[1]; k3z += P.qE[2]; }
                 // ---- stage 4
                 double Xe = fma(k3x, 4.0 * P.a2, fma(Ux, 2.0 * P.a1, X)), Ye = fma(k3y, 4.0 * P.a2, fma(Uy, 2.0 * P.a1, Y)),
                        Ze = fma(k3z, 4.0 * P.a2, fma(Uz, 2.0 * P.a1, Z));
@@ -252,13 +270,58 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 tg_fieldCyl<KIND, CACHED>(P, cc, reloads, dummy, Xe, Ye, Ze, t + P.dt, R, BR, Bz, Bp, tR, tZ);
                 tg_rotate(Xe, Ye, rinv, BR, Bp, Bx, By);
                 double k4x = fma(uy, Bz, -(uz * By)), k4y = fma(uz, Bx, -(ux * Bz)), k4z = fma(ux, By, -(uy * Bx));
+                if constexpr (HAS_E) { k4x += P.qE[0]; k4y += P.qE[1]; k4z += P.qE[2]; }
                 // ---- Eq. 5
                 double Tx = k2x + k3x, Ty = k2y + k3y, Tz = k2z + k3z;
-                double Xn = fma(k1x + Tx, P.c6, fma(Ux, P.dtq, X)), Yn = fma(k1y + Ty, P.c6, fma(Uy, P.dtq, Y)),
-                       Zn = fma(k1z + Tz, P.c6, fma(Uz, P.dtq, Z));
+                Xn = fma(k1x + Tx, P.c6, fma(Ux, P.dtq, X)); Yn = fma(k1y + Ty, P.c6, fma(Uy, P.dtq, Y));
+                Zn = fma(k1z + Tz, P.c6, fma(Uz, P.dtq, Z));
                 Ux = fma(fma(2.0, Tx, k1x + k4x), P.d6, Ux);
                 Uy = fma(fma(2.0, Ty, k1y + k4y), P.d6, Uy);
                 Uz = fma(fma(2.0, Tz, k1z + k4z), P.d6, Uz);
+                } else {
+                tg_rotate(X, Y, rinv, BR, Bp, Bx, By);
+                if constexpr (SOLVER == 2) {
+                    // ---- Eq. 4: classical RK4 on y = (r, v); with u = (q/m) v and k = dv/dt:
+                    //  r2 = r + v dt/2;            r3 = r + v dt/2 + k1 dt^2/4;   r4 = r + v dt + k2 dt^2/2
+                    //  r' = r + v dt + (k1+k2+k3) dt^2/6;   v' = v + (k1+2k2+2k3+k4) dt/6
+                    double k1x = fma(Uy, Bz, -(Uz * By)) + P.qE[0], k1y = fma(Uz, Bx, -(Ux * Bz)) + P.qE[1], k1z = fma(Ux, By, -(Uy * Bx)) + P.qE[2];
+                    double ux = fma(k1x, P.b1, Ux), uy = fma(k1y, P.b1, Uy), uz = fma(k1z, P.b1, Uz);
+                    tg_fieldXYZ<KIND, CACHED>(P, cc, reloads, fma(Ux, P.a1, X), fma(Uy, P.a1, Y), fma(Uz, P.a1, Z), t + 0.5 * P.dt, Bx, By, Bz);
+                    double k2x = fma(uy, Bz, -(uz * By)) + P.qE[0], k2y = fma(uz, Bx, -(ux * Bz)) + P.qE[1], k2z = fma(ux, By, -(uy * Bx)) + P.qE[2];
+                    ux = fma(k2x, P.b1, Ux); uy = fma(k2y, P.b1, Uy); uz = fma(k2z, P.b1, Uz);
+                    tg_fieldXYZ<KIND, CACHED>(P, cc, reloads, fma(k1x, 2.0 * P.a2, fma(Ux, P.a1, X)), fma(k1y, 2.0 * P.a2, fma(Uy, P.a1, Y)),
+                            fma(k1z, 2.0 * P.a2, fma(Uz, P.a1, Z)), t + 0.5 * P.dt, Bx, By, Bz);
+                    double k3x = fma(uy, Bz, -(uz * By)) + P.qE[0], k3y = fma(uz, Bx, -(ux * Bz)) + P.qE[1], k3z = fma(ux, By, -(uy * Bx)) + P.qE[2];
+                    ux = fma(k3x, 2.0 * P.b1, Ux); uy = fma(k3y, 2.0 * P.b1, Uy); uz = fma(k3z, 2.0 * P.b1, Uz);
+                    tg_fieldXYZ<KIND, CACHED>(P, cc, reloads, fma(k2x, 4.0 * P.a2, fma(Ux, 2.0 * P.a1, X)), fma(k2y, 4.0 * P.a2, fma(Uy, 2.0 * P.a1, Y)),
+                            fma(k2z, 4.0 * P.a2, fma(Uz, 2.0 * P.a1, Z)), t + P.dt, Bx, By, Bz);
+                    double k4x = fma(uy, Bz, -(uz * By)) + P.qE[0], k4y = fma(uz, Bx, -(ux * Bz)) + P.qE[1], k4z = fma(ux, By, -(uy * Bx)) + P.qE[2];
+                    double Tx = k2x + k3x, Ty = k2y + k3y, Tz = k2z + k3z;
+                    Xn = fma(k1x + Tx, P.c6, fma(Ux, P.dtq, X)); Yn = fma(k1y + Ty, P.c6, fma(Uy, P.dtq, Y));
+                    Zn = fma(k1z + Tz, P.c6, fma(Uz, P.dtq, Z));
+                    Ux = fma(fma(2.0, Tx, k1x + k4x), P.d6, Ux);
+                    Uy = fma(fma(2.0, Ty, k1y + k4y), P.d6, Uy);
+                    Uz = fma(fma(2.0, Tz, k1z + k4z), P.d6, Uz);
+                } else {
+                    // ---- Eq. 7-8: Boris push with B, E at r(t0).  In u = (q/m) v units:
+                    //  u- = u + eh;  t = B (q/m) h/2;  s = 2t/(1+t.t);  u* = u- + u- x t;  u+ = u- + u* x s;  u' = u+ + eh
+                    auto push = [&](double hb, double he) {      // hb = (q/m) h/2, he = h/dt
+                        double ax = fma(he, P.eh[0], Ux), ay = fma(he, P.eh[1], Uy), az = fma(he, P.eh[2], Uz);
+                        double tx = Bx * hb, ty = By * hb, tz = Bz * hb;
+                        double sc = 2.0 / (1.0 + fma(tx, tx, fma(ty, ty, tz * tz)));
+                        double bx = ax + fma(ay, tz, -(az * ty)), by = ay + fma(az, tx, -(ax * tz)), bz = az + fma(ax, ty, -(ay * tx));
+                        double sx = tx * sc, sy = ty * sc, sz = tz * sc;
+                        Ux = fma(he, P.eh[0], ax + fma(by, sz, -(bz * sy)));
+                        Uy = fma(he, P.eh[1], ay + fma(bz, sx, -(bx * sz)));
+                        Uz = fma(he, P.eh[2], az + fma(bx, sy, -(by * sx)));
+                    };
+                    if (nst == 0 && P.variant == 3) push(-0.5 * P.b1, -0.5);   // leap-frog start: v(t0) -> v(t0 - dt/2)
+                    double ox = Ux, oy = Uy, oz = Uz;
+                    push(P.b1, 1.0);
+                    if (P.variant == 4) { Xn = fma(ox, P.dtq, X); Yn = fma(oy, P.dtq, Y); Zn = fma(oz, P.dtq, Z); }   // Eq. 8 as printed
+                    else { Xn = fma(Ux, P.dtq, X); Yn = fma(Uy, P.dtq, Y); Zn = fma(Uz, P.dtq, Z); }
+                }
+                }
                 ++nst; ++ion_steps;
                 double s1 = fma(P.det.normal[0], Xn, fma(P.det.normal[1], Yn, fma(P.det.normal[2], Zn, -P.nrD)));
                 if (s1 >= 0.0) {               // O4: s0 < 0 <= s1 -> interpolate to the plane (L326, L338)
@@ -427,6 +490,8 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     P.qm = qm; P.dt = dt;
     P.a1 = dt / (2.0 * qm); P.a2 = dt * dt / 8.0; P.b1 = qm * dt / 2.0;
     P.c6 = dt * dt / 6.0; P.d6 = qm * dt / 6.0; P.dtq = dt / qm;
+    bool hasE = false;
+    for (int c = 0; c < 3; ++c) { P.qE[c] = qm * ctx->E[c]; P.eh[c] = qm * qm * ctx->E[c] * dt * 0.5; hasE |= ctx->E[c] != 0.0; }
     P.pa1R = P.a1 * ctx->field.inv_hR; P.pa1Z = P.a1 * ctx->field.inv_hZ;
     P.max_steps = max_steps; P.n = (uint32_t)ions->n; P.variant = variant;
     P.refill_min = ctx->opt_min_active > 0 ? (ctx->opt_min_active > 32 ? 32 : ctx->opt_min_active) : 1;
@@ -455,6 +520,7 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     unsigned need = (unsigned)((ions->n + threads - 1) / threads);
     if (grid > need) grid = need;
 #define TG_LAUNCH(K, C, T, B, ...) k_trace<K, C, T, B, ##__VA_ARGS__><<<grid, T, 0, st>>>(P)
+    if (variant <= 1 && !hasE) {           // the production path: RKN, E = 0
     switch (ctx->field.kind) {
     case 0:
         if (kv == 0) TG_LAUNCH(0, true, 128, 255, 2); else if (kv == 4) TG_LAUNCH(0, true, 128, 255, 1); else if (kv == 5) TG_LAUNCH(0, true, 128, 255); else if (kv == 3) TG_LAUNCH(0, true, 128, 168);
@@ -462,6 +528,21 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         break;
     case 1: if (kv == 2) TG_LAUNCH(1, false, 128, 128); else TG_LAUNCH(1, false, 128, 255); break;
     default: if (kv == 2) TG_LAUNCH(2, false, 128, 128); else TG_LAUNCH(2, false, 128, 255); break;
+    }
+    } else {                               // other solvers (Eq. 4, Eq. 7-8) and / or a uniform E: on-demand cache, 8 warps/SM
+        grid = (unsigned)(ctx->sm_count * 2); if (grid > need) grid = need;
+        const int S = variant <= 1 ? 0 : (variant == 2 ? 2 : 3);
+        const int kind = ctx->field.kind;
+        if (kind == 0 && variant == 1) TG_LAUNCH(0, false, 128, 255, 0, 0, true);
+        else if (kind == 0 && S == 0) TG_LAUNCH(0, true, 128, 255, 0, 0, true);
+        else if (kind == 0 && S == 2) TG_LAUNCH(0, true, 128, 255, 0, 2, true);
+        else if (kind == 0) TG_LAUNCH(0, true, 128, 255, 0, 3, true);
+        else if (kind == 1 && S == 0) TG_LAUNCH(1, false, 128, 255, 0, 0, true);
+        else if (kind == 1 && S == 2) TG_LAUNCH(1, false, 128, 255, 0, 2, true);
+        else if (kind == 1) TG_LAUNCH(1, false, 128, 255, 0, 3, true);
+        else if (S == 0) TG_LAUNCH(2, false, 128, 255, 0, 0, true);
+        else if (S == 2) TG_LAUNCH(2, false, 128, 255, 0, 2, true);
+        else TG_LAUNCH(2, false, 128, 255, 0, 3, true);
     }
 #undef TG_LAUNCH
     ++launches;

@@ -28,7 +28,7 @@ FLAG_EDGE, FLAG_PLANE, FLAG_GRID = 1, 2, 4
 
 EXPORTS = ["taiga_create", "taiga_destroy", "taiga_last_error", "taiga_load_field",
            "taiga_field_eval", "taiga_field_table", "taiga_seed_beam", "taiga_trace",
-           "taiga_detector_histogram", "taiga_set_option", "taiga_get_stats",
+           "taiga_detector_histogram", "taiga_set_efield", "taiga_set_option", "taiga_get_stats",
            "taiga_measure_fp64_peak"]
 
 
@@ -75,6 +75,7 @@ _lib.taiga_trace.argtypes = [C.c_void_p, C.POINTER(IonsS), C.c_double, C.c_doubl
                              C.POINTER(DetS), C.c_int]
 _lib.taiga_detector_histogram.argtypes = [C.c_void_p, C.POINTER(IonsS), C.POINTER(DetS), C.c_int,
                                           C.c_void_p, C.c_void_p]
+_lib.taiga_set_efield.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
 _lib.taiga_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_longlong]
 _lib.taiga_get_stats.argtypes = [C.c_void_p, C.POINTER(C.c_ulonglong * 8)]
 _lib.taiga_measure_fp64_peak.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
@@ -202,6 +203,9 @@ class Taiga:
         s = ions.struct()
         self._chk(_lib.taiga_trace(self.h, C.byref(s), q_over_m, dt, int(max_steps), C.byref(d),
                                    int(rkn_variant)))
+
+    def set_efield(self, E):
+        self._chk(_lib.taiga_set_efield(self.h, D3(*[float(e) for e in E])))
 
     def detector_histogram(self, ions, det, n_hist, counts, summary):
         d, keep = self._det(det)

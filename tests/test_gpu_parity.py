@@ -364,3 +364,48 @@ def test_cfg5_full_size_ripple_3d(tg):
     (6.2 GB of ion state, 1.6 GB of tables)."""
     cfg, s = _full_size_check(tg, 5, windows=2, width=64)
     assert 0.95 < (s[0, 0] + s[0, 1]) / cfg.n_ions < 0.975
+
+
+@pytest.mark.parametrize("icfg,n", [(1, 2048 + 19), (4, 128), (5, 1024 + 5)])
+@pytest.mark.parametrize("solver", [2, 3, 4])
+def test_other_solvers_parity(tg, icfg, n, solver):
+    """linearised RK4 (Eq. 4) and Boris (Eq. 7-8, both position readings)
+    on all three field kinds, same acceptance as the RKN path."""
+    from paper_2506_15812_b200 import taiga
+    cfg = wl.config(icfg, n_override=n)
+    ions, counts, summary = taiga.run_config(tg, cfg, rkn_variant=solver)
+    torch.cuda.synchronize()
+    ref = orc.run_config(cfg, variant=solver)
+    st = compare_groups(ions, ref, "%s solver %d" % (cfg.name, solver))
+    check_histogram(cfg, ions, counts, summary, ref)
+    assert st["flagged"] <= max(8, st["n"] // 200)
+    # the solver switch is live: Boris at the production step lands micrometres-millimetres from RKN
+    if solver >= 3:
+        ref0 = orc.run_config(cfg, field=ref["field"], variant=0)
+        g, g0 = ref["groups"][0], ref0["groups"][0]
+        cr = (g["status"] == 0) & (g0["status"] == 0)
+        assert np.abs(g["w"][cr] - g0["w"][cr]).max() > 1e-7
+
+
+@pytest.mark.parametrize("solver", [0, 1, 2, 3])
+def test_uniform_E_field_parity(tg, solver):
+    """Eq. 3 with a uniform ("parametric", L175) electric field, through every solver; an
+    E of 50 kV/m moves the hits by far more than the tolerance, so the term is live."""
+    from paper_2506_15812_b200 import taiga
+    E = (3.0e4, -2.0e4, 5.0e4)
+    cfg = wl.config(1, n_override=1500)
+    grid, nodal = cfg.field_builder()
+    try:
+        tg.set_efield(E)
+        ions, counts, summary = taiga.run_config(tg, cfg, rkn_variant=solver)
+        torch.cuda.synchronize()
+    finally:
+        tg.set_efield((0.0, 0.0, 0.0))
+    fE = orc.OracleField(grid, nodal, E=E)
+    ref = orc.run_config(cfg, field=fE, variant=solver)
+    compare_groups(ions, ref, "cfg1 E solver %d" % solver)
+    check_histogram(cfg, ions, counts, summary, ref)
+    ref0 = orc.run_config(cfg, variant=solver)
+    g, g0 = ref["groups"][0], ref0["groups"][0]
+    cr = (g["status"] == 0) & (g0["status"] == 0)
+    assert np.abs(g["w"][cr] - g0["w"][cr]).max() > 1e-5
