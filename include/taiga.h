@@ -166,7 +166,10 @@ int taiga_detector_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga
  * "ctas_per_sm", "variant" (kernel variant: 0 register cell cache with rolling predictive refill,
  * 8 warps/SM (default); 4 predictive refill after each evaluation; 5 refill on demand only; 3 the
  * same at 12 warps/SM; 1 / 2 no cache at 8 / 16 warps/SM), "stats" (1: read counters back,
- * default). */
+ * default), "precision" (64 default; 32 = the fp32 variant of BASELINE config 5: kind-2 fields
+ * with the RKN solver only, tricubic evaluation and its table in fp32, cell location and the ion
+ * state in fp64; hit coordinates then agree with fp64 to 1e-5 m, integer outputs are not
+ * bit-exact; taiga_trace returns TAIGA_E_ARG for other kinds / solvers). */
 int taiga_set_option(taiga_ctx* ctx, const char* key, long long value);
 /* counters of the last taiga_trace (valid with "stats" on): [0] ion-steps, [1] warp-steps*32
  * (lane slots issued), [2] 1, [3] kernel launches, [4] cell refills, [5..7] 0. */

@@ -22,6 +22,17 @@ __device__ __forceinline__ double tg_bicubic(const double* __restrict__ c, doubl
 
 __device__ __forceinline__ int tg_clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
 
+// fp32 variant (BASELINE config 5 "fp64 and fp32 variants"): 16 fp32 coefficients, two 256-bit loads
+__device__ __forceinline__ float tg_bicubic32(const float* __restrict__ c, float p, float w) {
+    float4 a0 = __ldg(reinterpret_cast<const float4*>(c)), a1 = __ldg(reinterpret_cast<const float4*>(c + 4));
+    float4 a2 = __ldg(reinterpret_cast<const float4*>(c + 8)), a3 = __ldg(reinterpret_cast<const float4*>(c + 12));
+    float r0 = fmaf(fmaf(fmaf(a0.w, w, a0.z), w, a0.y), w, a0.x);
+    float r1 = fmaf(fmaf(fmaf(a1.w, w, a1.z), w, a1.y), w, a1.x);
+    float r2 = fmaf(fmaf(fmaf(a2.w, w, a2.z), w, a2.y), w, a2.x);
+    float r3 = fmaf(fmaf(fmaf(a3.w, w, a3.z), w, a3.y), w, a3.x);
+    return fmaf(fmaf(fmaf(r3, p, r2), p, r1), p, r0);
+}
+
 // cell index and in-cell coordinate along one axis; outside the grid the boundary cell
 // extrapolates (reading A12).
 __device__ __forceinline__ int tg_locate(double x, double inv_h, double off, int ncell, double& frac) {
@@ -29,6 +40,29 @@ __device__ __forceinline__ int tg_locate(double x, double inv_h, double off, int
     int i = tg_clampi(__double2int_rd(pt), 0, ncell - 1);
     frac = pt - (double)i;
     return i;
+}
+
+// kind 2, fp32 variant: cell and in-cell coordinates located in fp64 (no cancellation), the 189 FMAs
+// of the tricubic evaluation and the table in fp32.
+__device__ __forceinline__ void tg_field_cyl32(const FieldDev& f, double R, double Z, double s,
+                                               double& BR, double& BZ, double& Bp) {
+    double p, w;
+    int i = tg_locate(R, f.inv_hR, f.offR, f.cR, p);
+    int j = tg_locate(Z, f.inv_hZ, f.offZ, f.cZ, w);
+    double xs = (s - f.s0) * f.inv_ds;
+    xs = xs - (double)f.nS * floor(xs / (double)f.nS);
+    int k = tg_clampi(__double2int_rd(xs), 0, f.nS - 1);
+    float pf = (float)p, wf = (float)w, qf = (float)(xs - (double)k);
+    const float* c = f.table32 + (((size_t)k * f.cR + i) * f.cZ + j) * 192;
+    float out[3];
+#pragma unroll
+    for (int m = 0; m < 3; ++m) {
+        const float* d = c + m * 64;
+        float e0 = tg_bicubic32(d, pf, wf), e1 = tg_bicubic32(d + 16, pf, wf);
+        float e2 = tg_bicubic32(d + 32, pf, wf), e3 = tg_bicubic32(d + 48, pf, wf);
+        out[m] = fmaf(fmaf(fmaf(e3, qf, e2), qf, e1), qf, e0);
+    }
+    BR = (double)out[0]; BZ = (double)out[1]; Bp = (double)out[2];
 }
 
 // (B_R, B_Z, B_phi) at (R, Z, s); s = time (kind 1) or phi (kind 2).

@@ -254,7 +254,7 @@ int tg_precompute(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c) {
     f.inv_hR = 1.0 / hR; f.inv_hZ = 1.0 / hZ;
     f.offR = g->Rmin / hR; f.offZ = g->Zmin / hZ;
     f.s0 = g->s0; f.inv_ds = (g->kind == 0) ? 0.0 : 1.0 / g->ds;
-    f.table = ctx->table;
+    f.table = ctx->table; f.table32 = nullptr;
     return TAIGA_OK;
 }
 

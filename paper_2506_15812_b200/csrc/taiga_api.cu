@@ -38,7 +38,7 @@ extern "C" int taiga_create(taiga_ctx** out, int device, void* cuda_stream) {
     }
     ctx->opt_sort = 1; ctx->opt_sort_sub = 16;
     ctx->opt_chunk0 = 0; ctx->opt_chunk = 2048; ctx->opt_min_active = 32;
-    ctx->opt_ctas_per_sm = 0; ctx->opt_variant = 0; ctx->opt_stats = 1;
+    ctx->opt_ctas_per_sm = 0; ctx->opt_variant = 0; ctx->opt_stats = 1; ctx->opt_precision = 64;
     strcpy(ctx->err, "ok");
     *out = ctx;
     return TAIGA_OK;
@@ -50,7 +50,7 @@ extern "C" int taiga_destroy(taiga_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     void* bufs[] = {ctx->table, ctx->scratch, ctx->band[0], ctx->band[1], ctx->cdf_depth, ctx->cdf_normal, ctx->edges, ctx->order,
                     ctx->bins, ctx->surv[0], ctx->surv[1], ctx->surv_idx[0], ctx->surv_idx[1],
-                    ctx->surv_steps[0], ctx->surv_steps[1], ctx->counters};
+                    ctx->surv_steps[0], ctx->surv_steps[1], ctx->counters, ctx->table32};
     for (void* b : bufs) if (b) cudaFree(b);
     if (ctx->counters_host) cudaFreeHost(ctx->counters_host);
     delete ctx;
@@ -69,7 +69,7 @@ extern "C" int taiga_load_field(taiga_ctx* ctx, const taiga_grid* g, const taiga
         return TAIGA_E_ARG;
     }
     TG_CUDA(ctx, cudaSetDevice(ctx->device));
-    ctx->field_loaded = false;
+    ctx->field_loaded = false; ctx->table32_valid = false;
     int rc = tg_precompute(ctx, g, c);
     if (rc == TAIGA_OK) ctx->field_loaded = true;
     return rc;
@@ -178,7 +178,7 @@ extern "C" int taiga_set_option(taiga_ctx* ctx, const char* key, long long v) {
     if (!ctx || !key) return TAIGA_E_ARG;
     struct { const char* k; int* p; } tab[] = {
         {"sort", &ctx->opt_sort}, {"sort_sub", &ctx->opt_sort_sub}, {"chunk0", &ctx->opt_chunk0},
-        {"chunk", &ctx->opt_chunk}, {"min_active", &ctx->opt_min_active},
+        {"chunk", &ctx->opt_chunk}, {"precision", &ctx->opt_precision}, {"min_active", &ctx->opt_min_active},
         {"ctas_per_sm", &ctx->opt_ctas_per_sm}, {"variant", &ctx->opt_variant}, {"stats", &ctx->opt_stats}};
     for (auto& t : tab) if (!strcmp(key, t.k)) { *t.p = (int)v; return TAIGA_OK; }
     TG_SET_ERR(ctx, "set_option: unknown key '%s'", key);

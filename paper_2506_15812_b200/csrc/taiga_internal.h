@@ -19,6 +19,7 @@ struct FieldDev {
     // kind 1: [iR][iZ][slice][comp][16]     (the two slices of a cell are adjacent)
     // kind 2: [iphi][iR][iZ][comp][64]
     const double* table;
+    const float* table32;            // kind 2, "precision" = 32: the same table rounded to fp32 (else null)
 };
 
 struct DetDev {
@@ -36,6 +37,7 @@ struct taiga_ctx {
     FieldDev field;
     double* table;            size_t table_bytes;
     double* scratch;          size_t scratch_bytes;     // precompute work arrays
+    float* table32;           size_t cap_table32;  bool table32_valid;   // fp32 copy of a kind-2 table
     double* band[2];          size_t band_cap[2]; int band_n[2];   // y -> y'' band operators (Z, R)
 
     double E[3];                                         // uniform electric field (taiga_set_efield), V/m
@@ -58,7 +60,7 @@ struct taiga_ctx {
 
     // options
     int opt_sort, opt_chunk0, opt_chunk, opt_min_active, opt_ctas_per_sm, opt_variant, opt_stats;
-    int opt_sort_sub;
+    int opt_sort_sub, opt_precision;
 };
 
 #define TG_SET_ERR(ctx, ...) snprintf((ctx)->err, sizeof((ctx)->err), __VA_ARGS__)

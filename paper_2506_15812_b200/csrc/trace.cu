@@ -143,7 +143,8 @@ __device__ __forceinline__ void tg_fieldCyl(const TraceParams& P, CellCache<KIND
         if constexpr (FIRST) outside = (R < P.f.Rmin) | (R > P.f.Rmax) | (Z < P.f.Zmin) | (Z > P.f.Zmax);
         double s = t;
         if constexpr (KIND == 2) s = atan2(Y, X);
-        tg_field_cyl(P.f, R, Z, s, BR, BZ, Bp);
+        if (KIND == 2 && P.f.table32) tg_field_cyl32(P.f, R, Z, s, BR, BZ, Bp);
+        else tg_field_cyl(P.f, R, Z, s, BR, BZ, Bp);
     }
 }
 
@@ -450,6 +451,11 @@ __global__ void k_sort_scatter(SortParams S, uint32_t* bins, const uint32_t* sum
     order[pos] = i;
 }
 
+__global__ void k_table_to_f32(const double* __restrict__ src, float* __restrict__ dst, size_t n) {
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x, stride = (size_t)gridDim.x * blockDim.x;
+    for (; i < n; i += stride) dst[i] = (float)src[i];
+}
+
 static int build_order(taiga_ctx* ctx, const taiga_ions* ions) {
     const FieldDev& f = ctx->field;
     uint32_t n = (uint32_t)ions->n;
@@ -486,6 +492,24 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     cudaStream_t st = ctx->stream;
     TraceParams P;
     P.f = ctx->field; P.det = det;
+    if (ctx->opt_precision == 32) {            // fp32 field evaluation (BASELINE config 5 "fp32 variant")
+        if (ctx->field.kind != 2 || variant > 1) {
+            TG_SET_ERR(ctx, "precision=32 is offered for kind-2 (R,Z,phi) fields with the RKN solver only");
+            return TAIGA_E_ARG;
+        }
+        if (!ctx->table32_valid) {
+            size_t n = (size_t)ctx->field.nS * ctx->field.cR * ctx->field.cZ * 192;
+            int rc = tg_reserve(ctx, &ctx->table32, &ctx->cap_table32, n);
+            if (rc) return rc;
+            k_table_to_f32<<<ctx->sm_count * 8, 256, 0, st>>>(ctx->table, ctx->table32, n);
+            TG_CUDA(ctx, cudaGetLastError());
+            ctx->table32_valid = true;
+        }
+        P.f.table32 = ctx->table32;
+    } else if (ctx->opt_precision != 64) {
+        TG_SET_ERR(ctx, "option precision must be 64 or 32");
+        return TAIGA_E_ARG;
+    }
     P.nrD = det.normal[0] * det.origin[0] + det.normal[1] * det.origin[1] + det.normal[2] * det.origin[2];
     P.qm = qm; P.dt = dt;
     P.a1 = dt / (2.0 * qm); P.a2 = dt * dt / 8.0; P.b1 = qm * dt / 2.0;
