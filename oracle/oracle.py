@@ -236,3 +236,69 @@ def run_config(cfg, field: OracleField | None = None, nthreads=0, variant=0):
         res["group"] = grp
         per_group.append(res)
     return dict(counts=counts, summary=summary, groups=per_group, field=field)
+
+
+# ---- secondary-ionisation loss (Eq. 2) -----------------
+class LossS(C.Structure):
+    _fields_ = [("psi_coef", _dp), ("n", C.c_int), ("psi0", C.c_double), ("dpsi", C.c_double),
+                ("rate", _dp)]
+
+
+_lib.orc_mcwhirter_rate.restype = C.c_double
+_lib.orc_mcwhirter_rate.argtypes = [C.c_double, C.c_double, C.c_double]
+
+
+def mcwhirter_rate(ne, Te, E12):
+    """Eq. 2: per-ion secondary ionisation rate [1/s]; scalars or arrays."""
+    ne, Te = np.broadcast_arrays(np.asarray(ne, dtype=np.float64), np.asarray(Te, dtype=np.float64))
+    out = np.array([_lib.orc_mcwhirter_rate(float(a), float(b), float(E12)) for a, b in zip(ne.ravel(), Te.ravel())])
+    return out.reshape(ne.shape) if ne.shape else float(out[0])
+
+
+class OracleLoss:
+    """psi(R,Z) spline table on the field's (R,Z) grid + rate profile nu(psi0 + k dpsi)."""
+
+    def __init__(self, grid, psi_nodal, psi0, dpsi, rate):
+        nod = np.ascontiguousarray(psi_nodal, dtype=np.float64).reshape(1, grid.nR, grid.nZ)
+        self.table = np.empty((1, grid.nR - 1, grid.nZ - 1, 16))
+        rc = _lib.orc_build_tables(C.c_int(0), C.c_int(grid.nR), C.c_int(grid.nZ), C.c_int(1), _p(nod), _p(self.table))
+        assert rc == 0
+        self.rate = np.ascontiguousarray(rate, dtype=np.float64)
+        self.s = LossS(_p(self.table), len(self.rate), float(psi0), float(dpsi), _p(self.rate))
+
+
+def trace_loss(field: OracleField, loss: OracleLoss, qm, state, t0, dt, max_steps, det, variant=0, nthreads=0):
+    x, y, z, vx, vy, vz = [np.ascontiguousarray(a, dtype=np.float64) for a in state]
+    n = len(x)
+    d, keep = _det_struct(det)
+    status = np.empty(n, dtype=np.int32)
+    u, w, weight = np.empty(n), np.empty(n), np.empty(n)
+    steps = np.empty(n, dtype=np.uint32)
+    flags = np.empty(n, dtype=np.uint8)
+    t0a = None if t0 is None else np.ascontiguousarray(t0, dtype=np.float64)
+    _lib.orc_trace_loss(C.byref(field.s), C.byref(loss.s), C.c_double(qm), C.c_int(variant), C.c_uint64(n),
+                        _p(x), _p(y), _p(z), _p(vx), _p(vy), _p(vz),
+                        _p(t0a) if t0a is not None else None,
+                        C.c_double(dt), C.c_uint32(max_steps), C.byref(d),
+                        status.ctypes.data_as(C.c_void_p), _p(u), _p(w),
+                        steps.ctypes.data_as(C.c_void_p), flags.ctypes.data_as(C.c_void_p), _p(weight),
+                        C.c_int(nthreads))
+    return dict(status=status, u=u, w=w, steps=steps, flags=flags, weight=weight)
+
+
+def histogram_weighted(res, group, det, n_hist, wcounts=None, wsummary=None):
+    """32.32 fixed-point weighted counters of res (after histogram(): needs res['cell'])."""
+    n = len(res["cell"])
+    d, keep = _det_struct(det)
+    if wcounts is None:
+        wcounts = np.zeros((n_hist, det.nw, det.nu), dtype=np.uint64)
+    if wsummary is None:
+        wsummary = np.zeros((n_hist, 4), dtype=np.uint64)
+    grp = None if group is None else np.ascontiguousarray(group, dtype=np.uint16)
+    cell = np.ascontiguousarray(res["cell"], dtype=np.int32)
+    wt = np.ascontiguousarray(res["weight"], dtype=np.float64)
+    _lib.orc_histogram_weighted(C.c_uint64(n), cell.ctypes.data_as(C.c_void_p), _p(wt),
+                                grp.ctypes.data_as(C.c_void_p) if grp is not None else None,
+                                C.byref(d), C.c_int(n_hist), wcounts.ctypes.data_as(C.c_void_p),
+                                wsummary.ctypes.data_as(C.c_void_p))
+    return wcounts, wsummary

@@ -458,6 +458,109 @@ extern "C" void orc_trace(const orc_field* f, double qm, int variant, uint64_t n
     }
 }
 
+/* ---- secondary-ionisation loss ------------------------------------- */
+
+/* Eq. 2: McWhirter's rate of Li+ -> Li2+ (Na+ -> Na2+) per ion,
+ *   nu = n_e * sqrt(t_e) exp(-1/t_e) / ((E12/1 eV)^{3/2} (6 + t_e)) * 1e-11 m^3/s,  t_e = T_e/E12,
+ * n_e in m^-3, T_e and E12 in eV; result in 1/s.  T_e <= 0 gives 0 (the limit).               */
+extern "C" double orc_mcwhirter_rate(double ne, double Te, double E12) {
+    if (!(Te > 0.0)) return 0.0;
+    double te = Te / E12;
+    return ne * (std::sqrt(te) * std::exp(-1.0 / te) / (std::pow(E12, 1.5) * (6.0 + te))) * 1e-11;
+}
+
+/* L177: "These coordinates are mapped to a poloidal cross-section plane in each iteration step.
+ * That is how ... the poloidal flux coordinate is determined.  The loss due to the secondary
+ * ionization that is described by Equation 2 is numerically integrated with every step using the
+ * one-dimensional secondary ionization profile."
+ * psi(R,Z): bicubic spline table on the field's (R,Z) grid (same cell rule, boundary cell
+ * extrapolates); nu(psi): table of n entries at psi0 + k dpsi, linear in between, held constant
+ * outside (reading L1 in DESIGN.md).                                                          */
+static inline double loss_rate(const orc_field* f, const orc_loss* L, const double r[3]) {
+    const int cZ = f->nZ - 1;
+    double hR = (f->Rmax - f->Rmin) / (double)(f->nR - 1), hZ = (f->Zmax - f->Zmin) / (double)cZ;
+    double R = std::sqrt(r[0] * r[0] + r[1] * r[1]), p, w;
+    int i = cell_index(R, f->Rmin, hR, f->nR, &p);
+    int j = cell_index(r[2], f->Zmin, hZ, f->nZ, &w);
+    double psi = bicubic(L->psi_coef + ((size_t)i * cZ + j) * 16, p, w);
+    double x = (psi - L->psi0) / L->dpsi;
+    if (!(x > 0.0)) return L->rate[0];
+    if (x >= (double)(L->n - 1)) return L->rate[L->n - 1];
+    int k = (int)std::floor(x);
+    double fr = x - (double)k;
+    return L->rate[k] + fr * (L->rate[k + 1] - L->rate[k]);
+}
+
+/* O4 with the loss integral.  "integrated with every step" (L177) is read as the trapezoidal rule
+ * over the step end points (reading L2): Lam += dt (nu(r_n) + nu(r_{n+1}))/2; on the crossing step
+ * only the fraction lam up to the plane counts, with nu interpolated linearly to the hit point:
+ * Lam += lam dt (nu_n + nu_hit)/2, nu_hit = nu_n + lam (nu_{n+1} - nu_n).  weight = exp(-Lam): the
+ * surviving fraction of singly ionised ions (dn1/dt = -nu n1).  Ions that do not cross get the
+ * weight accumulated up to their last step.  Everything else is orc_trace, unchanged.         */
+extern "C" void orc_trace_loss(const orc_field* f, const orc_loss* L, double qm, int variant, uint64_t n,
+                               const double* x, const double* y, const double* z,
+                               const double* vx, const double* vy, const double* vz, const double* t0,
+                               double dt, uint32_t max_steps, const orc_detector* det,
+                               int32_t* status, double* hit_u, double* hit_w,
+                               uint32_t* steps, uint8_t* flags, double* weight, int nthreads) {
+    orc_trace(f, qm, variant, n, x, y, z, vx, vy, vz, t0, dt, max_steps, det, status, hit_u, hit_w, nullptr,
+              steps, flags, nthreads);
+#ifdef _OPENMP
+    if (nthreads <= 0) nthreads = omp_get_max_threads();
+#pragma omp parallel for schedule(dynamic, 16) num_threads(nthreads)
+#endif
+    for (int64_t ii = 0; ii < (int64_t)n; ++ii) {
+        uint64_t i = (uint64_t)ii;
+        double r[3] = {x[i], y[i], z[i]}, v[3] = {vx[i], vy[i], vz[i]};
+        double t = t0 ? t0[i] : 0.0, Lam = 0.0;
+        if (status[i] == -4) { weight[i] = 1.0; continue; }
+        if (variant == 3) boris_start(f, qm, r, v, t, dt);
+        double s0 = det->normal[0] * (r[0] - det->origin[0]) + det->normal[1] * (r[1] - det->origin[1]) +
+                    det->normal[2] * (r[2] - det->origin[2]);
+        double nu0 = loss_rate(f, L, r);
+        for (uint32_t step = 1; step <= steps[i]; ++step) {      /* the same steps orc_trace took */
+            double rn[3], vn[3];
+            solver_step(f, qm, variant, r, v, t, dt, rn, vn);
+            double nu1 = loss_rate(f, L, rn);
+            if (step == steps[i] && status[i] == 0) {
+                double s1 = det->normal[0] * (rn[0] - det->origin[0]) + det->normal[1] * (rn[1] - det->origin[1]) +
+                            det->normal[2] * (rn[2] - det->origin[2]);
+                double lam = s0 / (s0 - s1);
+                double nuh = nu0 + lam * (nu1 - nu0);
+                Lam += lam * dt * (nu0 + nuh) / 2.0;
+                break;
+            }
+            if (step == steps[i] && status[i] == -3) break;      /* left the grid: the last step is not counted */
+            Lam += dt * (nu0 + nu1) / 2.0;
+            for (int c = 0; c < 3; ++c) { r[c] = rn[c]; v[c] = vn[c]; }
+            t = t + dt;
+            s0 = det->normal[0] * (r[0] - det->origin[0]) + det->normal[1] * (r[1] - det->origin[1]) +
+                 det->normal[2] * (r[2] - det->origin[2]);
+            nu0 = nu1;
+        }
+        weight[i] = std::exp(-Lam);
+    }
+}
+
+/* Weighted counters (L350: "weight ... by the secondary loss"): every plane-crossing ion adds its
+ * weight in 32.32 fixed point, q = floor(w 2^32 + 1/2), so that sums are integers and independent
+ * of the order of accumulation.  wcounts[n_hist][nw][nu] by segment; wsummary[n_hist][4] =
+ * {sum q in segments, sum q of crossers outside the segments, sum floor(q^2 / 2^32) over all
+ * crossers, number of crossers}.  cell[] as written by orc_histogram.                          */
+extern "C" void orc_histogram_weighted(uint64_t n, const int32_t* cell, const double* weight, const uint16_t* group,
+                                       const orc_detector* det, int n_hist, uint64_t* wcounts, uint64_t* wsummary) {
+    const size_t ncell = (size_t)det->nu * det->nw;
+    for (uint64_t i = 0; i < n; ++i) {
+        int g = group ? (int)group[i] : 0;
+        if (g >= n_hist || cell[i] < -1) continue;
+        uint64_t q = (uint64_t)std::floor(weight[i] * 4294967296.0 + 0.5);
+        if (cell[i] >= 0) { wcounts[(size_t)g * ncell + (size_t)cell[i]] += q; wsummary[g * 4 + 0] += q; }
+        else wsummary[g * 4 + 1] += q;
+        wsummary[g * 4 + 2] += (uint64_t)(((unsigned __int128)q * q) >> 32);
+        wsummary[g * 4 + 3] += 1;
+    }
+}
+
 /* O5  PAPER.md L330 (segments with optional non-uniform size and gaps on a perpendicular
  * grid), L344-350 (segment ID or error indicator per ion; atomically summed counters).
  * Brute-force linear scan over all segments; half-open [lo,hi) (A11).                      */

@@ -13,7 +13,9 @@
  * P10 CDF inversion exactness + statistics; P11 straight-line plane hit + brute-force
  * binning; P12 independent naive evaluator end to end; P13 RK4 (Eq. 4) amplification factor,
  * order and agreement with RKN; P14 Boris (Eq. 7-8) exact |v|, rotation angle 2 atan(z/2),
- * E x B drift, order of both position readings; P15 the three solvers agree as dt -> 0 (L294).
+ * E x B drift, order of both position readings; P15 the three solvers agree as dt -> 0 (L294);
+ * P16 Eq. 2 values and limits; P17 loss integral: constant rate -> exp(-nu t_hit) exactly,
+ * order 2 under step halving, agreement with an independent quadrature; fixed-point counters.
  * Parity unpinned: nothing in this file; the paper's own figures that cannot be pinned
  * (Fig. 10 loss rate, Table 1, Fig. 12 curves) are listed in DESIGN.md.
  *
@@ -41,6 +43,14 @@ typedef struct {
     double par[8];           /* analytic-field parameters */
     double E[3];             /* uniform electric field (Eq. 3; L175 "parametric modeling")  */
 } orc_field;
+
+/* secondary-ionisation loss inputs (Eq. 2): psi spline table of ONE component in
+ * the kind-0 layout [nR-1][nZ-1][16] (orc_build_tables), rate profile nu(psi0 + k dpsi) in 1/s */
+typedef struct {
+    const double* psi_coef;
+    int n; double psi0, dpsi;
+    const double* rate;
+} orc_loss;
 
 typedef struct {
     double origin[3], normal[3], eu[3], ew[3];
@@ -101,6 +111,18 @@ void orc_trace(const orc_field* f, double qm, int variant, uint64_t n,
 void orc_histogram(uint64_t n, int32_t* cell_io, const double* hit_u, const double* hit_w,
                    const uint16_t* group, uint8_t* flags, const orc_detector* det, int n_hist,
                    uint64_t* counts, uint64_t* summary);
+
+/* NEXT-1: Eq. 2 rate; O4 + loss integral (trapezoid over step end points, reading L2); weighted
+ * counters in 32.32 fixed point. */
+double orc_mcwhirter_rate(double ne_m3, double Te_eV, double E12_eV);
+void orc_trace_loss(const orc_field* f, const orc_loss* L, double qm, int variant, uint64_t n,
+                    const double* x, const double* y, const double* z,
+                    const double* vx, const double* vy, const double* vz, const double* t0,
+                    double dt, uint32_t max_steps, const orc_detector* det,
+                    int32_t* status, double* hit_u, double* hit_w,
+                    uint32_t* steps, uint8_t* flags, double* weight, int nthreads);
+void orc_histogram_weighted(uint64_t n, const int32_t* cell, const double* weight, const uint16_t* group,
+                            const orc_detector* det, int n_hist, uint64_t* wcounts, uint64_t* wsummary);
 
 int orc_max_threads(void);
 #ifdef __cplusplus

@@ -44,9 +44,40 @@ DETECTOR_X = 0.82
 
 
 def solovev_psi(R, Z):
-    """Poloidal flux of the synthetic equilibrium (A15); used by oracle pin P6 only."""
+    """Poloidal flux of the synthetic equilibrium (A15)."""
     return PSI_A * (((R * R - R0 * R0) / (2.0 * R0 * A_MINOR)) ** 2
                     + (R * Z / (R0 * KAPPA * A_MINOR)) ** 2)
+
+
+# synthetic plasma profiles for the secondary-ionisation loss (NEXT-1; stand in for the COMPASS
+# Thomson profiles of PAPER.md L71-81): n_e, T_e against normalised flux psi_N = psi / PSI_A
+E12_LI, E12_NA = 75.6400937, 47.28636          # second ionisation energies [eV]
+NE0, TE0 = 6.0e19, 900.0                      # core density [m^-3] and temperature [eV]
+LOSS_K, LOSS_PSIN_MAX = 257, 1.6              # profile table: psi_N = 0 .. 1.6
+
+
+def plasma_profiles(psin):
+    """H-mode-like profiles: parabolic core, exponential scrape-off layer beyond psi_N = 1."""
+    psin = np.asarray(psin, dtype=np.float64)
+    core = np.clip(1.0 - psin, 0.0, 1.0)
+    sol = np.exp(-np.clip(psin - 1.0, 0.0, None) / 0.05)
+    ne = NE0 * (0.08 * sol + 0.92 * core ** 0.6 * (psin < 1.0))
+    te = TE0 * (0.04 * sol + 0.96 * core ** 1.2 * (psin < 1.0))
+    return ne, te
+
+
+def loss_profile_inputs():
+    """(psi0, dpsi, n_e[k], T_e[k]) tabulated on psi = psi0 + k dpsi, k < LOSS_K."""
+    psin = np.linspace(0.0, LOSS_PSIN_MAX, LOSS_K)
+    ne, te = plasma_profiles(psin)
+    return 0.0, PSI_A * LOSS_PSIN_MAX / (LOSS_K - 1), ne, te
+
+
+def nodal_psi(grid):
+    """Nodal poloidal flux [Wb/rad] on a grid's (R, Z) nodes."""
+    R = np.linspace(grid.Rmin, grid.Rmax, grid.nR)[:, None]
+    Z = np.linspace(grid.Zmin, grid.Zmax, grid.nZ)[None, :]
+    return np.ascontiguousarray(solovev_psi(R, Z + 0.0 * R))
 
 
 def solovev_B(R, Z):
