@@ -92,6 +92,8 @@ typedef struct {
     uint8_t *flags;                      /* TAIGA_FLAG_*                                       */
     uint16_t *group;                     /* histogram index (energy / time slice)              */
     double *t0;                          /* birth time [s] (kind-1 fields)                     */
+    double *weight;                      /* surviving fraction after secondary ionisation, written
+                                            by taiga_trace when a loss model is loaded; may be null */
     uint64_t n;                          /* < 2^32                                             */
 } taiga_ions;
 
@@ -158,6 +160,35 @@ int taiga_set_efield(taiga_ctx* ctx, const double E_V_per_m[3]);
 int taiga_detector_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det,
                              int n_hist, unsigned long long* counts_dev,
                              unsigned long long* summary_dev);
+
+/* ---- secondary-ionisation loss (PAPER.md III.C, Eq. 2; L177: "numerically integrated with
+ * every step using the one-dimensional secondary ionization profile"; L350 weighting).
+ * taiga_load_loss builds (i) the bicubic spline table of the poloidal flux psi(R,Z) from nodal values
+ * [nR][nZ] on the (R,Z) grid of the field loaded before (any kind; psi is static and axisymmetric),
+ * (ii) the rate profile nu_k = n_e,k sqrt(t) exp(-1/t) / (E12^1.5 (6+t)) 1e-11 [1/s], t = T_e,k/E12
+ * (Eq. 2) at psi0 + k dpsi, k < n; nu(psi) is linear in between and held constant outside.
+ * While a loss model is loaded and ions->weight is not null, taiga_trace (RKN solvers, E = 0)
+ * also writes weight = exp(-integral of nu dt), the integral taken by the trapezoidal rule over
+ * the step end points, the crossing step counted up to the plane with nu interpolated linearly
+ * (reading L2); ions that do not cross keep the weight of their completed steps (1 for bad starts).
+ * psi_nodal = NULL unloads the model.  ne / Te: host pointers; psi_nodal host or dev. */
+typedef struct {
+    int n;                               /* >= 2 profile points                                   */
+    double psi0, dpsi;                   /* psi of point 0 and spacing (dpsi > 0), same unit as psi_nodal */
+    const double *ne_m3, *Te_eV;         /* electron density [m^-3] and temperature [eV]          */
+    double E12_eV;                       /* second ionisation energy of the beam species           */
+} taiga_loss_profile;
+int taiga_load_loss(taiga_ctx* ctx, const double* psi_nodal, int psi_on_device,
+                    const taiga_loss_profile* profile);
+
+/* Weighted counters (L350): every plane-crossing ion adds q = floor(weight 2^32 + 1/2) (32.32 fixed
+ * point: integer sums, independent of the order of the atomics) to wcounts_dev[n_hist][nw][nu] at
+ * its segment; wsummary_dev[n_hist][4] = {sum q in segments, sum q of crossers outside the
+ * segments, sum floor(q^2 / 2^32) over crossers, number of crossers}.  Both are ACCUMULATED into.
+ * Call after taiga_detector_histogram (uses ions->cell); needs ions->weight. */
+int taiga_detector_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det,
+                                      int n_hist, unsigned long long* wcounts_dev,
+                                      unsigned long long* wsummary_dev);
 
 /* ---- tuning / measurement hooks (not part of the method) */
 /* integer options: "sort" (1: order the ion queue by birth cell before tracing, default 1),

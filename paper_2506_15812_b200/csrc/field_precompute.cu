@@ -258,6 +258,63 @@ int tg_precompute(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c) {
     return TAIGA_OK;
 }
 
+// Eq. 2: nu = n_e sqrt(t) exp(-1/t) / (E12^1.5 (6 + t)) 1e-11 m^3/s, t = T_e / E12
+__global__ void k_mcwhirter(const double* __restrict__ ne, const double* __restrict__ Te, double E12, int n, double* __restrict__ rate) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    double T = Te[k], r = 0.0;
+    if (T > 0.0) {
+        double t = T / E12;
+        r = ne[k] * (sqrt(t) * exp(-1.0 / t) / (E12 * sqrt(E12) * (6.0 + t))) * 1e-11;
+    }
+    rate[k] = r;
+}
+
+// psi(R,Z): the a1 spline machinery on one more scalar (same band operators, kind-0 cell layout).
+int tg_load_loss(taiga_ctx* ctx, const double* psi_nodal, int on_device, const taiga_loss_profile* prof) {
+    const FieldDev& f = ctx->field;
+    const int nR = f.nR, nZ = f.nZ;
+    const long long nnode = (long long)nR * nZ, ncell = (long long)f.cR * f.cZ;
+    cudaStream_t st = ctx->stream;
+    const int TPB = 128;
+    int rc = tg_reserve(ctx, &ctx->psi_table, &ctx->cap_psi, (size_t)ncell * 48);
+    if (rc) return rc;
+    rc = tg_reserve(ctx, &ctx->loss_rate, &ctx->cap_rate, (size_t)prof->n);
+    if (rc) return rc;
+    size_t need = 4 * (size_t)nnode + 2 * (size_t)prof->n, scap = ctx->scratch_bytes / sizeof(double);
+    rc = tg_reserve(ctx, &ctx->scratch, &scap, need);
+    ctx->scratch_bytes = scap * sizeof(double);
+    if (rc) return rc;
+    double *y = ctx->scratch, *Mz = y + nnode, *Myr = Mz + nnode, *Mzr = Myr + nnode, *pne = Mzr + nnode, *pte = pne + prof->n;
+    for (int ax = 0; ax < 2; ++ax) {                 // band operators (normally cached by load_field)
+        int n = ax ? nR : nZ;
+        if (ctx->band_n[ax] != n) {
+            std::vector<double> b = spline_band(n);
+            size_t cap = ctx->band_cap[ax];
+            rc = tg_reserve(ctx, &ctx->band[ax], &cap, b.size());
+            ctx->band_cap[ax] = cap;
+            if (rc) return rc;
+            TG_CUDA(ctx, cudaMemcpyAsync(ctx->band[ax], b.data(), b.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+            TG_CUDA(ctx, cudaStreamSynchronize(st));
+            ctx->band_n[ax] = n;
+        }
+    }
+    TG_CUDA(ctx, cudaMemcpyAsync(y, psi_nodal, nnode * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+    TG_CUDA(ctx, cudaMemcpyAsync(pne, prof->ne_m3, prof->n * sizeof(double), cudaMemcpyHostToDevice, st));
+    TG_CUDA(ctx, cudaMemcpyAsync(pte, prof->Te_eV, prof->n * sizeof(double), cudaMemcpyHostToDevice, st));
+    unsigned gb = (unsigned)((nnode + TPB - 1) / TPB);
+    k_second_deriv<<<gb, TPB, 0, st>>>(y, Mz, ctx->band[0], nZ, 1, nnode);
+    k_second_deriv<<<gb, TPB, 0, st>>>(y, Myr, ctx->band[1], nR, nZ, nnode);
+    k_second_deriv<<<gb, TPB, 0, st>>>(Mz, Mzr, ctx->band[1], nR, nZ, nnode);
+    k_assemble<<<(unsigned)((ncell + TPB - 1) / TPB), TPB, 0, st>>>(y, Mz, Myr, Mzr, ctx->psi_table, 1, nR, nZ, 0, 0);
+    k_mcwhirter<<<(prof->n + TPB - 1) / TPB, TPB, 0, st>>>(pne, pte, prof->E12_eV, prof->n, ctx->loss_rate);
+    TG_CUDA(ctx, cudaGetLastError());
+    TG_CUDA(ctx, cudaStreamSynchronize(st));          // host profile arrays may be freed by the caller
+    ctx->loss.psi = ctx->psi_table; ctx->loss.rate = ctx->loss_rate; ctx->loss.n = prof->n;
+    ctx->loss.psi0 = prof->psi0; ctx->loss.inv_dpsi = 1.0 / prof->dpsi;
+    return TAIGA_OK;
+}
+
 int tg_field_eval(taiga_ctx* ctx, uint64_t n, const double* R, const double* Z, const double* s, double* BR, double* BZ, double* Bp) {
     k_field_eval<<<(unsigned)((n + 127) / 128), 128, 0, ctx->stream>>>(ctx->field, n, R, Z, s, BR, BZ, Bp);
     TG_CUDA(ctx, cudaGetLastError());

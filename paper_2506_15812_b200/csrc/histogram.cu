@@ -130,3 +130,29 @@ int tg_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* d
     TG_CUDA(ctx, cudaGetLastError());
     return TAIGA_OK;
 }
+
+// ------------------------------------------------------------------------------------------
+// Weighted counters: q = floor(w 2^32 + 1/2) per plane-crossing ion, 64-bit
+// integer atomics, so the sums do not depend on the order of accumulation.
+__global__ void k_histogram_weighted(const int32_t* __restrict__ cell, const double* __restrict__ weight,
+                                     const uint16_t* __restrict__ group, uint32_t n, int n_hist, int ncell,
+                                     unsigned long long* __restrict__ wcounts, unsigned long long* __restrict__ wsummary) {
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int g = group ? (int)group[i] : 0, c = cell[i];
+    if (g >= n_hist || c < TAIGA_CELL_MISS) return;
+    unsigned long long q = (unsigned long long)floor(fma(weight[i], 4294967296.0, 0.5));
+    if (c >= 0) { atomicAdd(&wcounts[(size_t)g * ncell + c], q); atomicAdd(&wsummary[g * 4 + 0], q); }
+    else atomicAdd(&wsummary[g * 4 + 1], q);
+    atomicAdd(&wsummary[g * 4 + 2], __umul64hi(q, q) << 32 | (q * q) >> 32);
+    atomicAdd(&wsummary[g * 4 + 3], 1ull);
+}
+
+int tg_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
+                          unsigned long long* wcounts, unsigned long long* wsummary) {
+    uint32_t n = (uint32_t)ions->n;
+    k_histogram_weighted<<<(n + 255) / 256, 256, 0, ctx->stream>>>(ions->cell, ions->weight, ions->group, n, n_hist,
+                                                                   det->nu * det->nw, wcounts, wsummary);
+    TG_CUDA(ctx, cudaGetLastError());
+    return TAIGA_OK;
+}

@@ -50,7 +50,7 @@ extern "C" int taiga_destroy(taiga_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     void* bufs[] = {ctx->table, ctx->scratch, ctx->band[0], ctx->band[1], ctx->cdf_depth, ctx->cdf_normal, ctx->edges, ctx->order,
                     ctx->bins, ctx->surv[0], ctx->surv[1], ctx->surv_idx[0], ctx->surv_idx[1],
-                    ctx->surv_steps[0], ctx->surv_steps[1], ctx->counters, ctx->table32};
+                    ctx->surv_steps[0], ctx->surv_steps[1], ctx->counters, ctx->table32, ctx->psi_table, ctx->loss_rate};
     for (void* b : bufs) if (b) cudaFree(b);
     if (ctx->counters_host) cudaFreeHost(ctx->counters_host);
     delete ctx;
@@ -69,7 +69,7 @@ extern "C" int taiga_load_field(taiga_ctx* ctx, const taiga_grid* g, const taiga
         return TAIGA_E_ARG;
     }
     TG_CUDA(ctx, cudaSetDevice(ctx->device));
-    ctx->field_loaded = false; ctx->table32_valid = false;
+    ctx->field_loaded = false; ctx->table32_valid = false; ctx->loss.psi = nullptr;   // a new grid invalidates psi
     int rc = tg_precompute(ctx, g, c);
     if (rc == TAIGA_OK) ctx->field_loaded = true;
     return rc;
@@ -152,6 +152,32 @@ extern "C" int taiga_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double d
     DetDev dd;
     for (int c = 0; c < 3; ++c) { dd.origin[c] = det->origin[c]; dd.normal[c] = det->normal[c]; dd.eu[c] = det->eu[c]; dd.ew[c] = det->ew[c]; }
     return tg_trace(ctx, ions, qm, dt, max_steps, dd, variant);
+}
+
+extern "C" int taiga_load_loss(taiga_ctx* ctx, const double* psi_nodal, int on_device, const taiga_loss_profile* prof) {
+    if (!ctx) return TAIGA_E_ARG;
+    if (!psi_nodal) { ctx->loss.psi = nullptr; return TAIGA_OK; }
+    if (!ctx->field_loaded) { TG_SET_ERR(ctx, "load_loss before load_field (psi lives on the field's (R,Z) grid)"); return TAIGA_E_STATE; }
+    if (!prof || prof->n < 2 || prof->n > (1 << 20) || !prof->ne_m3 || !prof->Te_eV || !(prof->dpsi > 0) || !isfinite(prof->psi0) ||
+        !(prof->E12_eV > 0)) { TG_SET_ERR(ctx, "load_loss: bad profile"); return TAIGA_E_ARG; }
+    for (int k = 0; k < prof->n; ++k)
+        if (!(prof->ne_m3[k] >= 0) || !isfinite(prof->ne_m3[k]) || !isfinite(prof->Te_eV[k])) { TG_SET_ERR(ctx, "load_loss: negative / non-finite profile value"); return TAIGA_E_ARG; }
+    TG_CUDA(ctx, cudaSetDevice(ctx->device));
+    return tg_load_loss(ctx, psi_nodal, on_device, prof);
+}
+
+extern "C" int taiga_detector_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
+                                                 unsigned long long* wcounts, unsigned long long* wsummary) {
+    if (!ctx) return TAIGA_E_ARG;
+    int rc = check_ions(ctx, ions, true);
+    if (rc) return rc;
+    rc = check_det(ctx, det, true);
+    if (rc) return rc;
+    if (n_hist < 1 || n_hist > 65536 || !wcounts || !wsummary) { TG_SET_ERR(ctx, "histogram_weighted: bad n_hist / null output"); return TAIGA_E_ARG; }
+    if (ions->n == 0) return TAIGA_OK;
+    if (!ions->weight) { TG_SET_ERR(ctx, "histogram_weighted: ions->weight is null"); return TAIGA_E_ARG; }
+    TG_CUDA(ctx, cudaSetDevice(ctx->device));
+    return tg_histogram_weighted(ctx, ions, det, n_hist, wcounts, wsummary);
 }
 
 extern "C" int taiga_set_efield(taiga_ctx* ctx, const double E[3]) {

@@ -22,6 +22,14 @@ struct FieldDev {
     const float* table32;            // kind 2, "precision" = 32: the same table rounded to fp32 (else null)
 };
 
+// secondary-ionisation loss model (taiga_load_loss); psi == nullptr: none
+struct LossDev {
+    const double* psi;               // [iR][iZ][48]: 16 coefficients used (kind-0 cell layout)
+    const double* rate;              // nu_k [1/s]
+    int n;
+    double psi0, inv_dpsi;
+};
+
 struct DetDev {
     double origin[3], normal[3], eu[3], ew[3];
 };
@@ -41,6 +49,11 @@ struct taiga_ctx {
     double* band[2];          size_t band_cap[2]; int band_n[2];   // y -> y'' band operators (Z, R)
 
     double E[3];                                         // uniform electric field (taiga_set_efield), V/m
+
+    // loss model
+    LossDev loss;
+    double* psi_table;        size_t cap_psi;
+    double* loss_rate;        size_t cap_rate;
 
     // seeding tables
     double *cdf_depth, *cdf_normal;  int cap_depth, cap_normal;
@@ -96,4 +109,7 @@ int tg_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* d
 int tg_field_eval(taiga_ctx* ctx, uint64_t n, const double* R, const double* Z, const double* s,
                   double* BR, double* BZ, double* Bp);
 int tg_field_table(taiga_ctx* ctx, int comp, double* host);
+int tg_load_loss(taiga_ctx* ctx, const double* psi_nodal, int on_device, const taiga_loss_profile* prof);
+int tg_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
+                          unsigned long long* wcounts, unsigned long long* wsummary);
 int tg_fp64_peak(taiga_ctx* ctx, double ms, double* rate);

@@ -24,6 +24,9 @@
 struct TraceParams {
     FieldDev f;
     DetDev det;
+    LossDev loss;                     // secondary-ionisation loss model (LOSS kernels)
+    double hdt;                       // dt/2
+    double* weight;
     double nrD;                       // normal . origin
     double a1, a2, b1;                // dt/(2 qm), dt^2/8, qm dt/2   (stage 2/3)
     double c6, d6, dtq;               // dt^2/6, qm dt/6, dt/qm
@@ -168,6 +171,21 @@ __device__ __forceinline__ void tg_rotate(double X, double Y, double rinv, doubl
     By = fma(BR, s_, Bp * c);
 }
 
+// nu(psi(R,Z)): psi from its bicubic table (boundary cell extrapolates), the rate
+// profile linear in psi between its points, held constant outside.
+__device__ __forceinline__ double tg_loss_rate(const TraceParams& P, double R, double Z) {
+    double p, w;
+    int i = tg_locate(R, P.f.inv_hR, P.f.offR, P.f.cR, p);
+    int j = tg_locate(Z, P.f.inv_hZ, P.f.offZ, P.f.cZ, w);
+    double psi = tg_bicubic(P.loss.psi + ((size_t)i * P.f.cZ + j) * 48, p, w);
+    double x = (psi - P.loss.psi0) * P.loss.inv_dpsi;
+    if (!(x > 0.0)) return __ldg(P.loss.rate);
+    if (x >= (double)(P.loss.n - 1)) return __ldg(P.loss.rate + P.loss.n - 1);
+    int k = __double2int_rd(x);
+    double r0 = __ldg(P.loss.rate + k), r1 = __ldg(P.loss.rate + k + 1);
+    return fma(x - (double)k, r1 - r0, r0);
+}
+
 // Cartesian B at a stage point (on-demand cache refill / uncached gather); solvers other than RKN
 template <int KIND, bool CACHED>
 __device__ __forceinline__ void tg_fieldXYZ(const TraceParams& P, CellCache<KIND>& cc, unsigned& reloads,
@@ -180,7 +198,8 @@ __device__ __forceinline__ void tg_fieldXYZ(const TraceParams& P, CellCache<KIND
 
 // SOLVER: 0 Runge-Kutta-Nystrom (Eq. 5-6), 2 linearised RK4 (Eq. 4), 3 Boris (Eq. 7-8; P.variant 3 =
 // Verlet form with leap-frog start, 4 = Eq. 8 as printed).  HAS_E: uniform E of Eq. 3 added to every k.
-template <int KIND, bool CACHED, int THREADS, int MAXREG, int PRED = 0, int SOLVER = 0, bool HAS_E = false>
+// LOSS: integrate Eq. 2 along the trajectory (trapezoid over step end points) and write exp(-integral).
+template <int KIND, bool CACHED, int THREADS, int MAXREG, int PRED = 0, int SOLVER = 0, bool HAS_E = false, bool LOSS = false>
 __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const TraceParams P) {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
@@ -189,6 +208,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
 #pragma unroll
         for (int k = 0; k < 48; ++k) cc.c[k] = 0.0; }
     double X = 0, Y = 0, Z = 0, Ux = 0, Uy = 0, Uz = 0, t = 0, s0 = -1.0;
+    double Lam = 0.0, nu0 = 0.0;               // LOSS: integral of nu dt, nu at the last step end point
     uint32_t idx = 0, nst = 0;
     bool alive = false, exhausted = false;
     unsigned reloads = 0, ion_steps = 0;       // per lane; < 2^32 for any run the queue allows
@@ -209,11 +229,13 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 Ux = P.qm * P.vx[idx]; Uy = P.qm * P.vy[idx]; Uz = P.qm * P.vz[idx];
                 t = P.t0 ? P.t0[idx] : 0.0;
                 nst = 0;
+                if constexpr (LOSS) Lam = 0.0;
                 s0 = fma(P.det.normal[0], X, fma(P.det.normal[1], Y, fma(P.det.normal[2], Z, -P.nrD)));
                 alive = true;
                 if (!(s0 < 0.0)) {             // O4: must start in front of the plane
                     P.hit_u[idx] = 0.0; P.hit_w[idx] = 0.0; P.cell[idx] = TAIGA_CELL_BADSTART; P.steps[idx] = 0;
                     P.flags[idx] = (fabs(s0) < TG_GRAZE) ? TAIGA_FLAG_PLANE : 0;
+                    if constexpr (LOSS) P.weight[idx] = 1.0;
                     alive = false;
                 }
             }
@@ -229,8 +251,14 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
             double dR = 0.0, dZ = 0.0;         // predicted half-step displacement in cells
             if constexpr (PRED) { dR = (fma(X, Ux, Y * Uy) * rinv) * P.pa1R; dZ = Uz * P.pa1Z; }
             tg_fieldCyl<KIND, CACHED, true, PRED == 2>(P, cc, reloads, outside, X, Y, Z, t, R, BR, Bz, Bp, tR, tZ, dR, dZ);
+            double nu1 = 0.0;
+            if constexpr (LOSS) {                  // trapezoid of the step that ended at this point (not of a step that left the grid)
+                nu1 = tg_loss_rate(P, R, Z);
+                if (nst > 0 && !outside) Lam = fma(P.hdt, nu0 + nu1, Lam);
+            }
             if (outside || nst == P.max_steps) {
                 uint8_t fl = 0;
+                if constexpr (LOSS) P.weight[idx] = (outside && nst == 0) ? 1.0 : exp(-Lam);
                 if (outside && (fabs(R - P.f.Rmin) < TG_GRAZE || fabs(R - P.f.Rmax) < TG_GRAZE ||
                                 fabs(Z - P.f.Zmin) < TG_GRAZE || fabs(Z - P.f.Zmax) < TG_GRAZE)) fl = TAIGA_FLAG_GRID;
                 P.hit_u[idx] = 0.0; P.hit_w[idx] = 0.0;
@@ -332,11 +360,17 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                     P.hit_u[idx] = fma(px, P.det.eu[0], fma(py, P.det.eu[1], pz * P.det.eu[2]));
                     P.hit_w[idx] = fma(px, P.det.ew[0], fma(py, P.det.ew[1], pz * P.det.ew[2]));
                     P.cell[idx] = TAIGA_CELL_MISS;      // segment assigned by the histogram kernel (a5)
+                    if constexpr (LOSS) {               // crossing step: up to the plane, nu interpolated linearly (reading L2)
+                        double nun = tg_loss_rate(P, sqrt(fma(Xn, Xn, Yn * Yn)), Zn);
+                        double nuh = fma(lam, nun - nu1, nu1);
+                        P.weight[idx] = exp(-fma(lam * P.hdt, nu1 + nuh, Lam));
+                    }
                     P.steps[idx] = nst;
                     P.flags[idx] = (fabs(s0) < TG_GRAZE || fabs(s1) < TG_GRAZE) ? TAIGA_FLAG_PLANE : 0;
                     alive = false;
                 }
                 X = Xn; Y = Yn; Z = Zn; t += P.dt; s0 = s1;
+                if constexpr (LOSS) nu0 = nu1;
             }
         }
     }
@@ -492,6 +526,8 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     cudaStream_t st = ctx->stream;
     TraceParams P;
     P.f = ctx->field; P.det = det;
+    P.loss = ctx->loss; P.hdt = 0.5 * dt; P.weight = ions->weight;
+    const bool loss = ctx->loss.psi != nullptr && ions->weight != nullptr;
     if (ctx->opt_precision == 32) {            // fp32 field evaluation (BASELINE config 5 "fp32 variant")
         if (ctx->field.kind != 2 || variant > 1) {
             TG_SET_ERR(ctx, "precision=32 is offered for kind-2 (R,Z,phi) fields with the RKN solver only");
@@ -544,7 +580,18 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     unsigned need = (unsigned)((ions->n + threads - 1) / threads);
     if (grid > need) grid = need;
 #define TG_LAUNCH(K, C, T, B, ...) k_trace<K, C, T, B, ##__VA_ARGS__><<<grid, T, 0, st>>>(P)
-    if (variant <= 1 && !hasE) {           // the production path: RKN, E = 0
+    if (loss) {                            // RKN + Eq. 2 loss integral: on-demand cache (kind 0) / uncached gathers
+        if (variant > 1 || hasE || ctx->opt_precision == 32) {
+            TG_SET_ERR(ctx, "the loss model is offered with the RKN solvers, E = 0, fp64");
+            return TAIGA_E_ARG;
+        }
+        grid = (unsigned)(ctx->sm_count * 2); if (grid > need) grid = need;
+        const int kind = ctx->field.kind;
+        if (kind == 0 && variant == 0) TG_LAUNCH(0, true, 128, 255, 0, 0, false, true);
+        else if (kind == 0) TG_LAUNCH(0, false, 128, 255, 0, 0, false, true);
+        else if (kind == 1) TG_LAUNCH(1, false, 128, 255, 0, 0, false, true);
+        else TG_LAUNCH(2, false, 128, 255, 0, 0, false, true);
+    } else if (variant <= 1 && !hasE) {           // the production path: RKN, E = 0
     switch (ctx->field.kind) {
     case 0:
         if (kv == 0) TG_LAUNCH(0, true, 128, 255, 2); else if (kv == 4) TG_LAUNCH(0, true, 128, 255, 1); else if (kv == 5) TG_LAUNCH(0, true, 128, 255); else if (kv == 3) TG_LAUNCH(0, true, 128, 168);

@@ -26,7 +26,8 @@ OK, E_ARG, E_STATE, E_CUDA, E_NOMEM = 0, -1, -2, -3, -4
 CELL_MISS, CELL_MAXSTEPS, CELL_OUT, CELL_BADSTART = -1, -2, -3, -4
 FLAG_EDGE, FLAG_PLANE, FLAG_GRID = 1, 2, 4
 
-EXPORTS = ["taiga_create", "taiga_destroy", "taiga_last_error", "taiga_load_field",
+EXPORTS = ["taiga_create", "taiga_destroy", "taiga_last_error", "taiga_load_field", "taiga_load_loss",
+           "taiga_detector_histogram_weighted",
            "taiga_field_eval", "taiga_field_table", "taiga_seed_beam", "taiga_trace",
            "taiga_detector_histogram", "taiga_set_efield", "taiga_set_option", "taiga_get_stats",
            "taiga_measure_fp64_peak"]
@@ -54,7 +55,12 @@ class BeamS(C.Structure):
 
 class IonsS(C.Structure):
     _fields_ = [(k, C.c_void_p) for k in ("x", "y", "z", "vx", "vy", "vz", "hit_u", "hit_w",
-                                          "cell", "steps", "flags", "group", "t0")] + [("n", C.c_uint64)]
+                                          "cell", "steps", "flags", "group", "t0", "weight")] + [("n", C.c_uint64)]
+
+
+class LossProfileS(C.Structure):
+    _fields_ = [("n", C.c_int), ("psi0", C.c_double), ("dpsi", C.c_double), ("ne", C.c_void_p),
+                ("Te", C.c_void_p), ("E12", C.c_double)]
 
 
 class DetS(C.Structure):
@@ -75,6 +81,9 @@ _lib.taiga_trace.argtypes = [C.c_void_p, C.POINTER(IonsS), C.c_double, C.c_doubl
                              C.POINTER(DetS), C.c_int]
 _lib.taiga_detector_histogram.argtypes = [C.c_void_p, C.POINTER(IonsS), C.POINTER(DetS), C.c_int,
                                           C.c_void_p, C.c_void_p]
+_lib.taiga_load_loss.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(LossProfileS)]
+_lib.taiga_detector_histogram_weighted.argtypes = [C.c_void_p, C.POINTER(IonsS), C.POINTER(DetS), C.c_int,
+                                                   C.c_void_p, C.c_void_p]
 _lib.taiga_set_efield.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
 _lib.taiga_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_longlong]
 _lib.taiga_get_stats.argtypes = [C.c_void_p, C.POINTER(C.c_ulonglong * 8)]
@@ -93,7 +102,7 @@ class Ions:
               ("vx", torch.float64), ("vy", torch.float64), ("vz", torch.float64),
               ("hit_u", torch.float64), ("hit_w", torch.float64), ("cell", torch.int32),
               ("steps", torch.int32), ("flags", torch.uint8), ("group", torch.int16),
-              ("t0", torch.float64))
+              ("t0", torch.float64), ("weight", torch.float64))
 
     def __init__(self, n, device="cuda:0", _arrays=None):
         self.n = int(n)
@@ -203,6 +212,29 @@ class Taiga:
         s = ions.struct()
         self._chk(_lib.taiga_trace(self.h, C.byref(s), q_over_m, dt, int(max_steps), C.byref(d),
                                    int(rkn_variant)))
+
+    def load_loss(self, psi_nodal, psi0=0.0, dpsi=1.0, ne=None, Te=None, E12=1.0):
+        """psi_nodal: [nR][nZ] numpy (host) or CUDA tensor, or None to unload; ne / Te: host arrays."""
+        if psi_nodal is None:
+            self._chk(_lib.taiga_load_loss(self.h, None, 0, None))
+            return
+        ne, Te = _host(ne), _host(Te)
+        assert len(ne) == len(Te)
+        prof = LossProfileS(len(ne), float(psi0), float(dpsi), ne.ctypes.data, Te.ctypes.data, float(E12))
+        if isinstance(psi_nodal, torch.Tensor):
+            assert psi_nodal.is_cuda and psi_nodal.dtype == torch.float64 and psi_nodal.is_contiguous()
+            self._chk(_lib.taiga_load_loss(self.h, psi_nodal.data_ptr(), 1, C.byref(prof)))
+        else:
+            a = _host(psi_nodal)
+            self._chk(_lib.taiga_load_loss(self.h, a.ctypes.data, 0, C.byref(prof)))
+
+    def detector_histogram_weighted(self, ions, det, n_hist, wcounts, wsummary):
+        d, keep = self._det(det)
+        s = ions.struct()
+        assert wcounts.dtype == torch.int64 and wsummary.dtype == torch.int64
+        assert wcounts.numel() == n_hist * d.nu * d.nw and wsummary.numel() == n_hist * 4
+        self._chk(_lib.taiga_detector_histogram_weighted(self.h, C.byref(s), C.byref(d), int(n_hist),
+                                                         wcounts.data_ptr(), wsummary.data_ptr()))
 
     def set_efield(self, E):
         self._chk(_lib.taiga_set_efield(self.h, D3(*[float(e) for e in E])))
