@@ -200,7 +200,10 @@ int taiga_detector_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, co
  * default), "precision" (64 default; 32 = the fp32 variant of BASELINE config 5: kind-2 fields
  * with the RKN solver only, tricubic evaluation and its table in fp32, cell location and the ion
  * state in fp64; hit coordinates then agree with fp64 to 1e-5 m, integer outputs are not
- * bit-exact; taiga_trace returns TAIGA_E_ARG for other kinds / solvers). */
+ * bit-exact; taiga_trace returns TAIGA_E_ARG for other kinds / solvers), "plane_interp" (0 default:
+ * linear interpolation to the detector plane; 1: quadratic Bezier through r_n, r_n+1 with the
+ * control point at the mean of r_n + v_n dt/2 and r_n+1 - v_n+1 dt/2, reading Z1;
+ * RKN solvers, E = 0, no loss model). */
 int taiga_set_option(taiga_ctx* ctx, const char* key, long long value);
 /* counters of the last taiga_trace (valid with "stats" on): [0] ion-steps, [1] warp-steps*32
  * (lane slots issued), [2] 1, [3] kernel launches, [4] cell refills, [5..7] 0. */

@@ -171,7 +171,7 @@ def seed(beam, cdf_depth, cdf_normal, seed_value, first_index, n):
 
 
 def trace(field: OracleField, qm, state, t0, dt, max_steps, det, variant=0, nthreads=0,
-          want_xyz=False):
+          want_xyz=False, interp=0):
     x, y, z, vx, vy, vz = [np.ascontiguousarray(a, dtype=np.float64) for a in state]
     n = len(x)
     d, keep = _det_struct(det)
@@ -181,7 +181,7 @@ def trace(field: OracleField, qm, state, t0, dt, max_steps, det, variant=0, nthr
     flags = np.empty(n, dtype=np.uint8)
     xyz = np.empty((n, 3)) if want_xyz else None
     t0a = None if t0 is None else np.ascontiguousarray(t0, dtype=np.float64)
-    _lib.orc_trace(C.byref(field.s), C.c_double(qm), C.c_int(variant), C.c_uint64(n),
+    _lib.orc_trace_interp(C.byref(field.s), C.c_double(qm), C.c_int(variant), C.c_int(interp), C.c_uint64(n),
                    _p(x), _p(y), _p(z), _p(vx), _p(vy), _p(vz),
                    _p(t0a) if t0a is not None else None,
                    C.c_double(dt), C.c_uint32(max_steps), C.byref(d),
@@ -213,7 +213,7 @@ def histogram(res, group, det, n_hist, counts=None, summary=None):
     return counts, summary
 
 
-def run_config(cfg, field: OracleField | None = None, nthreads=0, variant=0):
+def run_config(cfg, field: OracleField | None = None, nthreads=0, variant=0, interp=0):
     """Whole hot path (a1-a5) of one workloads.Config on the CPU oracle."""
     from paper_2506_15812_b200 import workloads as wl
     if field is None:
@@ -229,7 +229,7 @@ def run_config(cfg, field: OracleField | None = None, nthreads=0, variant=0):
         st = seed(g.beam, cd, cn, cfg.seed, g.first_index, g.n_ions)
         qm = g.beam.charge_C / g.beam.mass_kg
         t0 = np.full(g.n_ions, g.t0)
-        res = trace(field, qm, st, t0, cfg.dt, cfg.max_steps, det, variant, nthreads)
+        res = trace(field, qm, st, t0, cfg.dt, cfg.max_steps, det, variant, nthreads, interp=interp)
         grp = np.full(g.n_ions, g.group, dtype=np.uint16)
         histogram(res, grp, det, cfg.n_hist, counts, summary)
         res["state0"] = st

@@ -403,7 +403,48 @@ static inline bool in_grid(const orc_field* f, const double r[3], bool* graze) {
  * maximum number of iterations ... an interpolation is applied to the detector plane using
  * coordinates from the previous iteration step"), L318 (error value), L338 (two-state
  * storage, linear interpolation), L330 (coordinate transformation to the plane).          */
+/* L338: "We can use linear interpolation or quadratic Bezier interpolation to get the impact
+ * coordinates", from "the position and velocity coordinates of the current and previous iteration
+ * steps".  interp = 0: linear (O4 above).  interp = 1 (reading Z1 in DESIGN.md): the quadratic
+ * Bezier curve B(tau) = (1-tau)^2 P0 + 2 (1-tau) tau P1 + tau^2 P2 with P0 = r_n, P2 = r_{n+1}
+ * and the control point at the mean of the two tangent estimates,
+ * P1 = [(r_n + v_n dt/2) + (r_{n+1} - v_{n+1} dt/2)] / 2; the hit is B(tau*) where the signed
+ * plane distance s(tau) = (1-tau)^2 s0 + 2 (1-tau) tau sc + tau^2 s1 vanishes in [0,1]
+ * (sc = n.(P1 - r_D)); tau* = 2 s0 / (2 s0 - 2 sc - sqrt(4 sc^2 - 4 s0 s1))... written below in
+ * the cancellation-free form.  Exact for uniformly accelerated motion.                       */
+static inline void bezier_hit(const double r[3], const double v[3], const double rn[3], const double vn[3],
+                              double dt, double s0, double s1, const orc_detector* det, double p[3]) {
+    double P1[3], sc = 0.0;
+    for (int c = 0; c < 3; ++c) {
+        P1[c] = 0.5 * ((r[c] + v[c] * (dt / 2.0)) + (rn[c] - vn[c] * (dt / 2.0)));
+        sc += det->normal[c] * (P1[c] - det->origin[c]);
+    }
+    /* a tau^2 + b tau + c = 0, a = s0 - 2 sc + s1, b = 2 (sc - s0), c = s0 < 0 <= s1 */
+    double a = s0 - 2.0 * sc + s1, b = 2.0 * (sc - s0), c = s0;
+    double disc = b * b - 4.0 * a * c;
+    double tau;
+    if (!(disc >= 0.0)) tau = s0 / (s0 - s1);               /* no real root (cannot happen with s0<0<=s1): linear */
+    else {
+        double sq = std::sqrt(disc);
+        tau = (b >= 0.0) ? (-2.0 * c) / (b + sq) : (-b + sq) / (2.0 * a);
+    }
+    if (!(tau >= 0.0)) tau = 0.0;
+    if (tau > 1.0) tau = 1.0;
+    double w0 = (1.0 - tau) * (1.0 - tau), w1 = 2.0 * (1.0 - tau) * tau, w2 = tau * tau;
+    for (int k = 0; k < 3; ++k) p[k] = w0 * r[k] + w1 * P1[k] + w2 * rn[k];
+}
+
 extern "C" void orc_trace(const orc_field* f, double qm, int variant, uint64_t n,
+                          const double* x, const double* y, const double* z,
+                          const double* vx, const double* vy, const double* vz, const double* t0,
+                          double dt, uint32_t max_steps, const orc_detector* det,
+                          int32_t* status, double* hit_u, double* hit_w, double* hit_xyz,
+                          uint32_t* steps, uint8_t* flags, int nthreads) {
+    orc_trace_interp(f, qm, variant, 0, n, x, y, z, vx, vy, vz, t0, dt, max_steps, det, status, hit_u, hit_w, hit_xyz,
+                     steps, flags, nthreads);
+}
+
+extern "C" void orc_trace_interp(const orc_field* f, double qm, int variant, int interp, uint64_t n,
                           const double* x, const double* y, const double* z,
                           const double* vx, const double* vy, const double* vz, const double* t0,
                           double dt, uint32_t max_steps, const orc_detector* det,
@@ -440,6 +481,7 @@ extern "C" void orc_trace(const orc_field* f, double qm, int variant, uint64_t n
                 double lam = s0 / (s0 - s1);
                 double p[3];
                 for (int c = 0; c < 3; ++c) p[c] = r[c] + lam * (rn[c] - r[c]);
+                if (interp == 1) bezier_hit(r, v, rn, vn, dt, s0, s1, det, p);
                 hit_u[i] = (p[0] - det->origin[0]) * det->eu[0] + (p[1] - det->origin[1]) * det->eu[1] + (p[2] - det->origin[2]) * det->eu[2];
                 hit_w[i] = (p[0] - det->origin[0]) * det->ew[0] + (p[1] - det->origin[1]) * det->ew[1] + (p[2] - det->origin[2]) * det->ew[2];
                 if (hit_xyz) { hit_xyz[3 * i] = p[0]; hit_xyz[3 * i + 1] = p[1]; hit_xyz[3 * i + 2] = p[2]; }

@@ -106,6 +106,15 @@ void orc_trace(const orc_field* f, double qm, int variant, uint64_t n,
                int32_t* status, double* hit_u, double* hit_w, double* hit_xyz /*[n][3] or 0*/,
                uint32_t* steps, uint8_t* flags, int nthreads);
 
+/* O4 with the choice of plane interpolation (L338): interp 0 = linear, 1 = quadratic Bezier
+ * (reading Z1); orc_trace is interp = 0. */
+void orc_trace_interp(const orc_field* f, double qm, int variant, int interp, uint64_t n,
+               const double* x, const double* y, const double* z,
+               const double* vx, const double* vy, const double* vz, const double* t0,
+               double dt, uint32_t max_steps, const orc_detector* det,
+               int32_t* status, double* hit_u, double* hit_w, double* hit_xyz,
+               uint32_t* steps, uint8_t* flags, int nthreads);
+
 /* O5  binning + counting.  cell_io in: status from orc_trace; out: cell / -1 / error.
  *     counts[n_hist][nw][nu] and summary[n_hist][6] are accumulated into. */
 void orc_histogram(uint64_t n, int32_t* cell_io, const double* hit_u, const double* hit_w,

@@ -73,7 +73,7 @@ struct taiga_ctx {
 
     // options
     int opt_sort, opt_chunk0, opt_chunk, opt_min_active, opt_ctas_per_sm, opt_variant, opt_stats;
-    int opt_sort_sub, opt_precision;
+    int opt_sort_sub, opt_precision, opt_plane_interp;
 };
 
 #define TG_SET_ERR(ctx, ...) snprintf((ctx)->err, sizeof((ctx)->err), __VA_ARGS__)

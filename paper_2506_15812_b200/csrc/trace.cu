@@ -199,7 +199,9 @@ __device__ __forceinline__ void tg_fieldXYZ(const TraceParams& P, CellCache<KIND
 // SOLVER: 0 Runge-Kutta-Nystrom (Eq. 5-6), 2 linearised RK4 (Eq. 4), 3 Boris (Eq. 7-8; P.variant 3 =
 // Verlet form with leap-frog start, 4 = Eq. 8 as printed).  HAS_E: uniform E of Eq. 3 added to every k.
 // LOSS: integrate Eq. 2 along the trajectory (trapezoid over step end points) and write exp(-integral).
-template <int KIND, bool CACHED, int THREADS, int MAXREG, int PRED = 0, int SOLVER = 0, bool HAS_E = false, bool LOSS = false>
+// BEZ: quadratic Bezier instead of linear interpolation to the plane (reading Z1).
+template <int KIND, bool CACHED, int THREADS, int MAXREG, int PRED = 0, int SOLVER = 0, bool HAS_E = false, bool LOSS = false,
+          bool BEZ = false>
 __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const TraceParams P) {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
@@ -267,6 +269,8 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 alive = false;
             } else {
                 double Xn, Yn, Zn;
+                double c1x = 0.0, c1y = 0.0, c1z = 0.0;      // BEZ: r_n + v_n dt/2
+                if constexpr (BEZ) { c1x = fma(Ux, P.a1, X); c1y = fma(Uy, P.a1, Y); c1z = fma(Uz, P.a1, Z); }
                 if constexpr (SOLVER == 0) {
                 if constexpr (PRED == 1) tg_predict(P, cc, reloads, tR + dR, tZ + dZ, BR, Bz, Bp);
                 tg_rotate(X, Y, rinv, BR, Bp, Bx, By);
@@ -357,6 +361,22 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                     double lam = s0 / (s0 - s1);
                     double px = fma(lam, Xn - X, X) - P.det.origin[0], py = fma(lam, Yn - Y, Y) - P.det.origin[1],
                            pz = fma(lam, Zn - Z, Z) - P.det.origin[2];
+                    if constexpr (BEZ) {
+                        // control point = mean of r_n + v_n dt/2 and r_n+1 - v_n+1 dt/2; root of the plane distance
+                        // (1-tau)^2 s0 + 2 (1-tau) tau sc + tau^2 s1 in [0,1], cancellation-free form
+                        double qx = 0.5 * (c1x + fma(-Ux, P.a1, Xn)), qy = 0.5 * (c1y + fma(-Uy, P.a1, Yn)), qz = 0.5 * (c1z + fma(-Uz, P.a1, Zn));
+                        double sc = fma(P.det.normal[0], qx, fma(P.det.normal[1], qy, fma(P.det.normal[2], qz, -P.nrD)));
+                        double qa = s0 - 2.0 * sc + s1, qb = 2.0 * (sc - s0), disc = fma(qb, qb, -4.0 * qa * s0), tau = lam;
+                        if (disc >= 0.0) {
+                            double sq = sqrt(disc);
+                            tau = (qb >= 0.0) ? (-2.0 * s0) / (qb + sq) : (sq - qb) / (2.0 * qa);
+                        }
+                        tau = fmin(fmax(tau, 0.0), 1.0);
+                        double w0 = (1.0 - tau) * (1.0 - tau), w1 = 2.0 * (1.0 - tau) * tau, w2 = tau * tau;
+                        px = fma(w0, X, fma(w1, qx, w2 * Xn)) - P.det.origin[0];
+                        py = fma(w0, Y, fma(w1, qy, w2 * Yn)) - P.det.origin[1];
+                        pz = fma(w0, Z, fma(w1, qz, w2 * Zn)) - P.det.origin[2];
+                    }
                     P.hit_u[idx] = fma(px, P.det.eu[0], fma(py, P.det.eu[1], pz * P.det.eu[2]));
                     P.hit_w[idx] = fma(px, P.det.ew[0], fma(py, P.det.ew[1], pz * P.det.ew[2]));
                     P.cell[idx] = TAIGA_CELL_MISS;      // segment assigned by the histogram kernel (a5)
@@ -580,7 +600,18 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     unsigned need = (unsigned)((ions->n + threads - 1) / threads);
     if (grid > need) grid = need;
 #define TG_LAUNCH(K, C, T, B, ...) k_trace<K, C, T, B, ##__VA_ARGS__><<<grid, T, 0, st>>>(P)
-    if (loss) {                            // RKN + Eq. 2 loss integral: on-demand cache (kind 0) / uncached gathers
+    if (ctx->opt_plane_interp == 1) {      // quadratic Bezier interpolation to the plane
+        if (variant > 1 || hasE || loss || ctx->opt_precision == 32) {
+            TG_SET_ERR(ctx, "plane_interp=1 (Bezier) is offered with the RKN solvers, E = 0, no loss model, fp64");
+            return TAIGA_E_ARG;
+        }
+        grid = (unsigned)(ctx->sm_count * 2); if (grid > need) grid = need;
+        const int kind = ctx->field.kind;
+        if (kind == 0 && variant == 0) TG_LAUNCH(0, true, 128, 255, 0, 0, false, false, true);
+        else if (kind == 0) TG_LAUNCH(0, false, 128, 255, 0, 0, false, false, true);
+        else if (kind == 1) TG_LAUNCH(1, false, 128, 255, 0, 0, false, false, true);
+        else TG_LAUNCH(2, false, 128, 255, 0, 0, false, false, true);
+    } else if (loss) {                     // RKN + Eq. 2 loss integral: on-demand cache (kind 0) / uncached gathers
         if (variant > 1 || hasE || ctx->opt_precision == 32) {
             TG_SET_ERR(ctx, "the loss model is offered with the RKN solvers, E = 0, fp64");
             return TAIGA_E_ARG;

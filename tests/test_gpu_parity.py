@@ -525,3 +525,24 @@ def test_secondary_ionisation_loss_parity(tg, icfg, n, species):
     taiga.run_config(tg, wl.config(icfg, n_override=64), field_loaded=True, ions=ions.view(0, 64 * len(cfg.groups)))
     torch.cuda.synchronize()
     assert float(ions.weight[:64].min()) == 7.0
+
+
+@pytest.mark.parametrize("icfg,n", [(1, 4096), (4, 128), (5, 1024 + 3)])
+def test_bezier_plane_interpolation_parity(tg, icfg, n):
+    """quadratic Bezier interpolation to the detector plane."""
+    from paper_2506_15812_b200 import taiga
+    cfg = wl.config(icfg, n_override=n)
+    try:
+        tg.set_option("plane_interp", 1)
+        ions, counts, summary = taiga.run_config(tg, cfg)
+        torch.cuda.synchronize()
+    finally:
+        tg.set_option("plane_interp", 0)
+    ref = orc.run_config(cfg, interp=1)
+    compare_groups(ions, ref, "%s bezier" % cfg.name)
+    check_histogram(cfg, ions, counts, summary, ref)
+    lin = orc.run_config(cfg, field=ref["field"], interp=0)
+    g, g0 = ref["groups"][0], lin["groups"][0]
+    cr = (g["status"] == 0) & (g0["status"] == 0)
+    d = np.hypot(g["u"][cr] - g0["u"][cr], g["w"][cr] - g0["w"][cr]).max()
+    assert 1e-8 < d < 1e-3                    # micrometres (more at grazing incidence): the switch is live
