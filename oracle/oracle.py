@@ -170,6 +170,22 @@ def seed(beam, cdf_depth, cdf_normal, seed_value, first_index, n):
     return out
 
 
+def seed_grid(beam, cdf_depth, cdf_normal, nd, nT, nZ, z_lim, first_index, n):
+    """Deterministic weighted-grid initialisation (L314, reading D1): returns (state6, w0)."""
+    b = BeamS()
+    b.v0 = beam_v0(beam)
+    b.origin, b.axis, b.eT, b.eZ = D3(*beam.origin), D3(*beam.axis), D3(*beam.eT), D3(*beam.eZ)
+    cd = np.ascontiguousarray(cdf_depth, dtype=np.float64)
+    cn = np.ascontiguousarray(cdf_normal, dtype=np.float64)
+    b.cdf_depth, b.n_depth, b.depth_max = _p(cd), len(cd) - 1, beam.depth_max
+    b.cdf_normal, b.n_normal, b.z_max = _p(cn), len(cn) - 1, beam.z_max
+    b.sigma_pos, b.sigma_ang = beam.sigma_pos_m, 0.0
+    out = [np.empty(n) for _ in range(7)]
+    _lib.orc_seed_grid(C.byref(b), C.c_int(nd), C.c_int(nT), C.c_int(nZ), C.c_double(z_lim),
+                       C.c_uint64(first_index), C.c_uint64(n), *[_p(a) for a in out])
+    return out[:6], out[6]
+
+
 def trace(field: OracleField, qm, state, t0, dt, max_steps, det, variant=0, nthreads=0,
           want_xyz=False, interp=0):
     x, y, z, vx, vy, vz = [np.ascontiguousarray(a, dtype=np.float64) for a in state]
@@ -267,7 +283,7 @@ class OracleLoss:
         self.s = LossS(_p(self.table), len(self.rate), float(psi0), float(dpsi), _p(self.rate))
 
 
-def trace_loss(field: OracleField, loss: OracleLoss, qm, state, t0, dt, max_steps, det, variant=0, nthreads=0):
+def trace_loss(field: OracleField, loss: OracleLoss, qm, state, t0, dt, max_steps, det, variant=0, nthreads=0, w0=None):
     x, y, z, vx, vy, vz = [np.ascontiguousarray(a, dtype=np.float64) for a in state]
     n = len(x)
     d, keep = _det_struct(det)
@@ -281,7 +297,8 @@ def trace_loss(field: OracleField, loss: OracleLoss, qm, state, t0, dt, max_step
                         _p(t0a) if t0a is not None else None,
                         C.c_double(dt), C.c_uint32(max_steps), C.byref(d),
                         status.ctypes.data_as(C.c_void_p), _p(u), _p(w),
-                        steps.ctypes.data_as(C.c_void_p), flags.ctypes.data_as(C.c_void_p), _p(weight),
+                        steps.ctypes.data_as(C.c_void_p), flags.ctypes.data_as(C.c_void_p),
+                        _p(np.ascontiguousarray(w0, dtype=np.float64)) if w0 is not None else None, _p(weight),
                         C.c_int(nthreads))
     return dict(status=status, u=u, w=w, steps=steps, flags=flags, weight=weight)
 

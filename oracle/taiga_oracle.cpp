@@ -86,6 +86,44 @@ extern "C" void orc_seed(const orc_beam* b, uint64_t seed, uint64_t first_index,
     }
 }
 
+/* Deterministic initialisation ("we define a grid with representative ions along
+ * the beam, and each virtual ion gets a weight according to the ionization density function").
+ * Reading D1: nd x nT x nZ cells; depth cell k = depth_max [k, k+1]/nd, cross-section
+ * cells a, b = -z_lim + 2 z_lim [a, a+1]/nT (in units of sigma_pos) and likewise for nZ; the
+ * representative ion sits at the cell centre, flies along the beam axis, and carries the weight
+ * w0 = (F_d(hi) - F_d(lo)) (Phi(hi_T) - Phi(lo_T)) (Phi(hi_Z) - Phi(lo_Z)), the tabulated CDFs taken
+ * linear between their points (the same tables the stochastic mode inverts).  Ion index
+ * i = (k nT + a) nZ + b.                                                                      */
+static inline double cdf_value(const double* F, int K, double x_max, double x) {
+    double t = x / (x_max / (double)K);
+    if (!(t > 0.0)) return F[0];
+    if (t >= (double)K) return F[K];
+    int j = (int)std::floor(t);
+    return std::fma(t - (double)j, F[j + 1] - F[j], F[j]);
+}
+extern "C" void orc_seed_grid(const orc_beam* b, int nd, int nT, int nZ, double z_lim, uint64_t first_index, uint64_t n,
+                              double* x, double* y, double* z, double* vx, double* vy, double* vz, double* w0) {
+    for (uint64_t j = 0; j < n; ++j) {
+        uint64_t i = first_index + j;
+        uint64_t ib = i % (uint64_t)nZ, ia = (i / (uint64_t)nZ) % (uint64_t)nT, k = i / ((uint64_t)nZ * (uint64_t)nT);
+        double dd = b->depth_max / (double)nd, dT = 2.0 * z_lim / (double)nT, dZ = 2.0 * z_lim / (double)nZ;
+        double d_lo = (double)k * dd, d_hi = (double)(k + 1) * dd, d = ((double)k + 0.5) * dd;
+        double a_lo = (double)ia * dT - z_lim, a_hi = (double)(ia + 1) * dT - z_lim, za = ((double)ia + 0.5) * dT - z_lim;
+        double b_lo = (double)ib * dZ - z_lim, b_hi = (double)(ib + 1) * dZ - z_lim, zb = ((double)ib + 0.5) * dZ - z_lim;
+        double wd = cdf_value(b->cdf_depth, b->n_depth, b->depth_max, d_hi) - cdf_value(b->cdf_depth, b->n_depth, b->depth_max, d_lo);
+        double wT = cdf_value(b->cdf_normal, b->n_normal, 2.0 * b->z_max, a_hi + b->z_max) -
+                    cdf_value(b->cdf_normal, b->n_normal, 2.0 * b->z_max, a_lo + b->z_max);
+        double wZ = cdf_value(b->cdf_normal, b->n_normal, 2.0 * b->z_max, b_hi + b->z_max) -
+                    cdf_value(b->cdf_normal, b->n_normal, 2.0 * b->z_max, b_lo + b->z_max);
+        double r[3];
+        for (int c = 0; c < 3; ++c)
+            r[c] = (b->origin[c] + d * b->axis[c]) + b->sigma_pos * (za * b->eT[c] + zb * b->eZ[c]);
+        x[j] = r[0]; y[j] = r[1]; z[j] = r[2];
+        vx[j] = b->v0 * b->axis[0]; vy[j] = b->v0 * b->axis[1]; vz[j] = b->v0 * b->axis[2];
+        w0[j] = (wd * wT) * wZ;
+    }
+}
+
 /* ------------------------------------------------------------------------------------ */
 /* O1  dense Gaussian elimination with partial pivoting, m right-hand sides (columns of B) */
 static int solve_dense(int n, std::vector<double>& A, int m, double* B /*[n][m]*/) {
@@ -544,7 +582,7 @@ extern "C" void orc_trace_loss(const orc_field* f, const orc_loss* L, double qm,
                                const double* vx, const double* vy, const double* vz, const double* t0,
                                double dt, uint32_t max_steps, const orc_detector* det,
                                int32_t* status, double* hit_u, double* hit_w,
-                               uint32_t* steps, uint8_t* flags, double* weight, int nthreads) {
+                               uint32_t* steps, uint8_t* flags, const double* w0, double* weight, int nthreads) {
     orc_trace(f, qm, variant, n, x, y, z, vx, vy, vz, t0, dt, max_steps, det, status, hit_u, hit_w, nullptr,
               steps, flags, nthreads);
 #ifdef _OPENMP
@@ -555,7 +593,8 @@ extern "C" void orc_trace_loss(const orc_field* f, const orc_loss* L, double qm,
         uint64_t i = (uint64_t)ii;
         double r[3] = {x[i], y[i], z[i]}, v[3] = {vx[i], vy[i], vz[i]};
         double t = t0 ? t0[i] : 0.0, Lam = 0.0;
-        if (status[i] == -4) { weight[i] = 1.0; continue; }
+        const double wi = w0 ? w0[i] : 1.0;                       /* initial statistical weight (deterministic mode) */
+        if (status[i] == -4) { weight[i] = wi; continue; }
         if (variant == 3) boris_start(f, qm, r, v, t, dt);
         double s0 = det->normal[0] * (r[0] - det->origin[0]) + det->normal[1] * (r[1] - det->origin[1]) +
                     det->normal[2] * (r[2] - det->origin[2]);
@@ -580,7 +619,7 @@ extern "C" void orc_trace_loss(const orc_field* f, const orc_loss* L, double qm,
                  det->normal[2] * (r[2] - det->origin[2]);
             nu0 = nu1;
         }
-        weight[i] = std::exp(-Lam);
+        weight[i] = wi * std::exp(-Lam);
     }
 }
 

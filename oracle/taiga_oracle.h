@@ -15,7 +15,9 @@
  * order and agreement with RKN; P14 Boris (Eq. 7-8) exact |v|, rotation angle 2 atan(z/2),
  * E x B drift, order of both position readings; P15 the three solvers agree as dt -> 0 (L294);
  * P16 Eq. 2 values and limits; P17 loss integral: constant rate -> exp(-nu t_hit) exactly,
- * order 2 under step halving, agreement with an independent quadrature; fixed-point counters.
+ * order 2 under step halving, agreement with an independent quadrature; fixed-point counters;
+ * P18 Bezier plane interpolation: exact on parabolas, order 3; P19 weighted-grid seeding:
+ * weights sum to 1, marginals = CDF increments, weighted detector image = stochastic image.
  * Parity unpinned: nothing in this file; the paper's own figures that cannot be pinned
  * (Fig. 10 loss rate, Table 1, Fig. 12 curves) are listed in DESIGN.md.
  *
@@ -76,6 +78,11 @@ double orc_cdf_invert(const double* F, int K, double x_max, double U);
 void orc_seed(const orc_beam* b, uint64_t seed, uint64_t first_index, uint64_t n,
               double* x, double* y, double* z, double* vx, double* vy, double* vz);
 
+/* L314 deterministic initialisation (reading D1): weighted grid of nd x nT x nZ representative
+ * ions, cross-section spanning +-z_lim sigma_pos; ion index i = (k nT + a) nZ + b */
+void orc_seed_grid(const orc_beam* b, int nd, int nT, int nZ, double z_lim, uint64_t first_index, uint64_t n,
+                   double* x, double* y, double* z, double* vx, double* vy, double* vz, double* w0);
+
 /* O1  1-D splines on a unit-spaced grid: per-interval power coefficients c[i][0..3],
  *     S(i+p) = c0 + c1 p + c2 p^2 + c3 p^3.  not-a-knot: n>=4 nodes, n-1 intervals;
  *     periodic: n>=3 nodes, n intervals, y[n]==y[0] implied. */
@@ -129,7 +136,7 @@ void orc_trace_loss(const orc_field* f, const orc_loss* L, double qm, int varian
                     const double* vx, const double* vy, const double* vz, const double* t0,
                     double dt, uint32_t max_steps, const orc_detector* det,
                     int32_t* status, double* hit_u, double* hit_w,
-                    uint32_t* steps, uint8_t* flags, double* weight, int nthreads);
+                    uint32_t* steps, uint8_t* flags, const double* w0 /* or 0 */, double* weight, int nthreads);
 void orc_histogram_weighted(uint64_t n, const int32_t* cell, const double* weight, const uint16_t* group,
                             const orc_detector* det, int n_hist, uint64_t* wcounts, uint64_t* wsummary);
 

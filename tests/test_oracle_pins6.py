@@ -61,3 +61,67 @@ def test_p18_bezier_third_order_in_the_tokamak_field():
             e.append(np.hypot(r["u"][ok] - ref["u"][ok], r["w"][ok] - ref["w"][ok]).max())
         assert abs(math.log2(e[0] / e[2]) / 2 - order) < 0.35, (interp, e)
         assert 0.5 < e[1] / e1 < 2.0, (interp, e)
+
+
+# ---- P19: deterministic weighted-grid initialisation (L314, reading D1) ----------------------
+def _li_beam():
+    return wl.config(1).groups[0].beam
+
+
+def test_p19_grid_weights_sum_to_one_and_marginals_are_cdf_increments():
+    beam = _li_beam()
+    cd, cn = wl.depth_cdf(), wl.normal_cdf()
+    nd, nT, nZ = 50, 7, 9
+    st, w0 = orc.seed_grid(beam, cd, cn, nd, nT, nZ, beam.z_max, 0, nd * nT * nZ)
+    assert abs(w0.sum() - 1.0) < 1e-13 and np.all(w0 >= 0)
+    W = w0.reshape(nd, nT, nZ)
+    # depth marginal = increments of the tabulated CDF at the cell edges (linear between table points)
+    edges = np.linspace(0.0, beam.depth_max, nd + 1)
+    F = np.interp(edges, np.linspace(0.0, beam.depth_max, len(cd)), cd)
+    assert np.abs(W.sum(axis=(1, 2)) - np.diff(F)).max() < 1e-15
+    zc = np.linspace(-beam.z_max, beam.z_max, len(cn))
+    PhiT = np.interp(np.linspace(-beam.z_max, beam.z_max, nT + 1), zc, cn)
+    assert np.abs(W.sum(axis=(0, 2)) - np.diff(PhiT)).max() < 1e-15
+    # truncated exponential with lambda = 2 cm: the first cell holds (1 - e^{-dd/lam}) / (1 - e^{-dmax/lam})
+    dd = beam.depth_max / nd
+    assert abs(W.sum(axis=(1, 2))[0] - (1 - math.exp(-dd / 0.02)) / (1 - math.exp(-beam.depth_max / 0.02))) < 1e-6   # linear interpolation of the table between its points
+    # positions: cell centres on the beam frame; velocities along the axis; index i = (k nT + a) nZ + b
+    x, y, z, vx, vy, vz = st
+    k, a, b = 17, 3, 5
+    i = (k * nT + a) * nZ + b
+    assert abs(x[i] - (0.78 - (k + 0.5) * dd)) < 1e-15
+    assert abs(y[i] - beam.sigma_pos_m * ((a + 0.5) * 2 * beam.z_max / nT - beam.z_max)) < 1e-16
+    assert abs(z[i] - beam.sigma_pos_m * ((b + 0.5) * 2 * beam.z_max / nZ - beam.z_max)) < 1e-16
+    assert np.all(vx == -V0) and np.all(vy == 0) and np.all(vz == 0)
+    # sharding: a sub-range reproduces the same ions
+    st2, w2 = orc.seed_grid(beam, cd, cn, nd, nT, nZ, beam.z_max, 1000, 77)
+    assert np.array_equal(w2, w0[1000:1077]) and np.array_equal(st2[2], z[1000:1077])
+
+
+def test_p19_weighted_grid_image_agrees_with_the_stochastic_one():
+    """Both initialisations sample the same ionisation density (L314), so the weighted detector
+    image of the grid run agrees with the image of the stochastic run within sampling error."""
+    cfg = wl.config(1)
+    grid, nodal = cfg.field_builder()
+    f = orc.OracleField(grid, nodal)
+    g = cfg.groups[0]
+    cd, cn = wl.depth_cdf(), wl.normal_cdf()
+    n = 40000
+    st = orc.seed(g.beam, cd, cn, 123, 0, n)
+    rs = orc.trace(f, QM, st, None, cfg.dt, cfg.max_steps, cfg.detector)
+    cs = rs["status"] == 0
+    nd, nT, nZ = 200, 15, 15
+    sg, w0 = orc.seed_grid(g.beam, cd, cn, nd, nT, nZ, 4.0, 0, nd * nT * nZ)
+    rg = orc.trace(f, QM, sg, None, cfg.dt, cfg.max_steps, cfg.detector)
+    cg = rg["status"] == 0
+    W = w0[cg].sum()
+    # crossing fraction
+    p_s, p_g = cs.mean(), W / w0.sum()
+    assert abs(p_s - p_g) < 4 * math.sqrt(p_s * (1 - p_s) / n) + 2e-3
+    # first and second moments of the hit distribution on the plane
+    for key in ("u", "w"):
+        m_s, s_s = rs[key][cs].mean(), rs[key][cs].std()
+        m_g = (w0[cg] * rg[key][cg]).sum() / W
+        s_g = math.sqrt((w0[cg] * (rg[key][cg] - m_g) ** 2).sum() / W)
+        assert abs(m_s - m_g) < 4 * s_s / math.sqrt(cs.sum()) + 0.02 * s_s, (key, m_s, m_g)
+        assert abs(s_s / s_g - 1) < 0.05, (key, s_s, s_g)
