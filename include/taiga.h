@@ -92,8 +92,10 @@ typedef struct {
     uint8_t *flags;                      /* TAIGA_FLAG_*                                       */
     uint16_t *group;                     /* histogram index (energy / time slice)              */
     double *t0;                          /* birth time [s] (kind-1 fields)                     */
-    double *weight;                      /* surviving fraction after secondary ionisation, written
+    double *weight;                      /* w0 x surviving fraction after secondary ionisation, written
                                             by taiga_trace when a loss model is loaded; may be null */
+    double *w0;                          /* initial statistical weight (deterministic initialisation:
+                                            written by taiga_seed_beam_grid); null = 1             */
     uint64_t n;                          /* < 2^32                                             */
 } taiga_ions;
 
@@ -119,6 +121,18 @@ typedef struct {
 
 int taiga_seed_beam(taiga_ctx* ctx, const taiga_beam_params* params, uint64_t seed,
                     taiga_ions* ions);
+
+/* Deterministic initialisation ("we define a grid with representative ions along the
+ * beam, and each virtual ion gets a weight according to the ionization density function").
+ * Reading D1: nd x nT x nZ cells -- depth cell k = depth_max [k, k+1]/nd along `axis`, cross-section
+ * cells of width 2 z_lim/nT (2 z_lim/nZ) in units of sigma_pos spanning +-z_lim; the ion sits at the
+ * cell centre, flies along `axis` (sigma_ang ignored) and gets ions->w0 = product of the increments
+ * of the tabulated CDFs over the cell (linear between table points).  Ion j of the call is grid
+ * index i = first_index + j = (k nT + a) nZ + b; first_index + ions->n <= nd nT nZ.  ions->w0 must
+ * not be null.  No random numbers are drawn. */
+typedef struct { int nd, nT, nZ; double z_lim; } taiga_seed_grid;
+int taiga_seed_beam_grid(taiga_ctx* ctx, const taiga_beam_params* params, const taiga_seed_grid* grid,
+                         taiga_ions* ions);
 
 /* ---- detector (plane normal + perpendicular grid of segments with optional
  * non-uniform size and gaps; coordinate transformation to the plane).  u = (p-origin).eu,
@@ -168,7 +182,7 @@ int taiga_detector_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga
  * (ii) the rate profile nu_k = n_e,k sqrt(t) exp(-1/t) / (E12^1.5 (6+t)) 1e-11 [1/s], t = T_e,k/E12
  * (Eq. 2) at psi0 + k dpsi, k < n; nu(psi) is linear in between and held constant outside.
  * While a loss model is loaded and ions->weight is not null, taiga_trace (RKN solvers, E = 0)
- * also writes weight = exp(-integral of nu dt), the integral taken by the trapezoidal rule over
+ * also writes weight = w0 exp(-integral of nu dt) (w0 = 1 when ions->w0 is null), the integral taken by the trapezoidal rule over
  * the step end points, the crossing step counted up to the plane with nu interpolated linearly
  * (reading L2); ions that do not cross keep the weight of their completed steps (1 for bad starts).
  * psi_nodal = NULL unloads the model.  ne / Te: host pointers; psi_nodal host or dev. */
@@ -183,9 +197,9 @@ int taiga_load_loss(taiga_ctx* ctx, const double* psi_nodal, int psi_on_device,
 
 /* Weighted counters (L350): every plane-crossing ion adds q = floor(weight 2^32 + 1/2) (32.32 fixed
  * point: integer sums, independent of the order of the atomics) to wcounts_dev[n_hist][nw][nu] at
- * its segment; wsummary_dev[n_hist][4] = {sum q in segments, sum q of crossers outside the
+ * its segment (weight = ions->weight if not null, else ions->w0); wsummary_dev[n_hist][4] = {sum q in segments, sum q of crossers outside the
  * segments, sum floor(q^2 / 2^32) over crossers, number of crossers}.  Both are ACCUMULATED into.
- * Call after taiga_detector_histogram (uses ions->cell); needs ions->weight. */
+ * Call after taiga_detector_histogram (uses ions->cell); needs ions->weight or ions->w0. */
 int taiga_detector_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det,
                                       int n_hist, unsigned long long* wcounts_dev,
                                       unsigned long long* wsummary_dev);

@@ -87,7 +87,55 @@ __global__ void __launch_bounds__(256) k_beam_seed(SeedParams P, double* __restr
     if (t0) t0[j] = P.t0;
 }
 
-int tg_seed(taiga_ctx* ctx, const taiga_beam_params* p, uint64_t seed, taiga_ions* ions, double v0) {
+// Deterministic initialisation (a grid of representative ions along the beam, each
+// weighted by the ionisation density).  Reading D1: nd x nT x nZ cells, ion at the cell centre,
+// weight = product of the tabulated-CDF increments over the cell (CDFs linear between points).
+// Explicitly rounded intrinsics in a fixed operation order: bit-identical on any IEEE-754 machine.
+__device__ __forceinline__ double cdf_value(const double* __restrict__ F, int K, double x_max, double x) {
+    double t = __ddiv_rn(x, __ddiv_rn(x_max, (double)K));
+    if (!(t > 0.0)) return __ldg(F);
+    if (t >= (double)K) return __ldg(F + K);
+    int j = __double2int_rd(t);
+    double Fl = __ldg(F + j), Fh = __ldg(F + j + 1);
+    return __fma_rn(__dsub_rn(t, (double)j), __dsub_rn(Fh, Fl), Fl);
+}
+
+__global__ void __launch_bounds__(256) k_beam_seed_grid(SeedParams P, int nd, int nT, int nZ, double z_lim,
+                                                        double* __restrict__ x, double* __restrict__ y, double* __restrict__ z,
+                                                        double* __restrict__ vx, double* __restrict__ vy, double* __restrict__ vz,
+                                                        double* __restrict__ w0, unsigned short* __restrict__ group,
+                                                        double* __restrict__ t0) {
+    unsigned long long j = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= P.n) return;
+    unsigned long long i = P.first_index + j;
+    unsigned long long ib = i % (unsigned long long)nZ, ia = (i / (unsigned long long)nZ) % (unsigned long long)nT,
+                       k = i / ((unsigned long long)nZ * (unsigned long long)nT);
+    double dd = __ddiv_rn(P.depth_max, (double)nd), zl2 = __dmul_rn(2.0, z_lim), zw = __dmul_rn(2.0, P.z_max);
+    double dT = __ddiv_rn(zl2, (double)nT), dZ = __ddiv_rn(zl2, (double)nZ);
+    double d_lo = __dmul_rn((double)k, dd), d_hi = __dmul_rn((double)(k + 1), dd), d = __dmul_rn(__dadd_rn((double)k, 0.5), dd);
+    double a_lo = __dsub_rn(__dmul_rn((double)ia, dT), z_lim), a_hi = __dsub_rn(__dmul_rn((double)(ia + 1), dT), z_lim),
+           za = __dsub_rn(__dmul_rn(__dadd_rn((double)ia, 0.5), dT), z_lim);
+    double b_lo = __dsub_rn(__dmul_rn((double)ib, dZ), z_lim), b_hi = __dsub_rn(__dmul_rn((double)(ib + 1), dZ), z_lim),
+           zb = __dsub_rn(__dmul_rn(__dadd_rn((double)ib, 0.5), dZ), z_lim);
+    double wd = __dsub_rn(cdf_value(P.cdf_depth, P.n_depth, P.depth_max, d_hi), cdf_value(P.cdf_depth, P.n_depth, P.depth_max, d_lo));
+    double wT = __dsub_rn(cdf_value(P.cdf_normal, P.n_normal, zw, __dadd_rn(a_hi, P.z_max)),
+                          cdf_value(P.cdf_normal, P.n_normal, zw, __dadd_rn(a_lo, P.z_max)));
+    double wZ = __dsub_rn(cdf_value(P.cdf_normal, P.n_normal, zw, __dadd_rn(b_hi, P.z_max)),
+                          cdf_value(P.cdf_normal, P.n_normal, zw, __dadd_rn(b_lo, P.z_max)));
+    double r[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+        r[c] = __dadd_rn(__dadd_rn(P.origin[c], __dmul_rn(d, P.axis[c])),
+                         __dmul_rn(P.sigma_pos, __dadd_rn(__dmul_rn(za, P.eT[c]), __dmul_rn(zb, P.eZ[c]))));
+    x[j] = r[0]; y[j] = r[1]; z[j] = r[2];
+    vx[j] = __dmul_rn(P.v0, P.axis[0]); vy[j] = __dmul_rn(P.v0, P.axis[1]); vz[j] = __dmul_rn(P.v0, P.axis[2]);
+    w0[j] = __dmul_rn(__dmul_rn(wd, wT), wZ);
+    if (group) group[j] = P.group;
+    if (t0) t0[j] = P.t0;
+}
+
+int tg_seed(taiga_ctx* ctx, const taiga_beam_params* p, uint64_t seed, taiga_ions* ions, double v0,
+            const taiga_seed_grid* g) {
     size_t cd = ctx->cap_depth, cn = ctx->cap_normal;
     int rc = tg_reserve(ctx, &ctx->cdf_depth, &cd, (size_t)p->n_depth + 1);
     ctx->cap_depth = (int)cd;
@@ -107,7 +155,9 @@ int tg_seed(taiga_ctx* ctx, const taiga_beam_params* p, uint64_t seed, taiga_ion
     P.first_index = p->first_index; P.seed = seed; P.n = ions->n;
     P.group = p->group; P.t0 = p->t0;
     unsigned blocks = (unsigned)((ions->n + 255) / 256);
-    k_beam_seed<<<blocks, 256, 0, ctx->stream>>>(P, ions->x, ions->y, ions->z, ions->vx, ions->vy, ions->vz, ions->group, ions->t0);
+    if (g) k_beam_seed_grid<<<blocks, 256, 0, ctx->stream>>>(P, g->nd, g->nT, g->nZ, g->z_lim, ions->x, ions->y, ions->z, ions->vx,
+                                                             ions->vy, ions->vz, ions->w0, ions->group, ions->t0);
+    else k_beam_seed<<<blocks, 256, 0, ctx->stream>>>(P, ions->x, ions->y, ions->z, ions->vx, ions->vy, ions->vz, ions->group, ions->t0);
     TG_CUDA(ctx, cudaGetLastError());
     return TAIGA_OK;
 }

@@ -151,7 +151,7 @@ __global__ void k_histogram_weighted(const int32_t* __restrict__ cell, const dou
 int tg_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
                           unsigned long long* wcounts, unsigned long long* wsummary) {
     uint32_t n = (uint32_t)ions->n;
-    k_histogram_weighted<<<(n + 255) / 256, 256, 0, ctx->stream>>>(ions->cell, ions->weight, ions->group, n, n_hist,
+    k_histogram_weighted<<<(n + 255) / 256, 256, 0, ctx->stream>>>(ions->cell, ions->weight ? ions->weight : ions->w0, ions->group, n, n_hist,
                                                                    det->nu * det->nw, wcounts, wsummary);
     TG_CUDA(ctx, cudaGetLastError());
     return TAIGA_OK;

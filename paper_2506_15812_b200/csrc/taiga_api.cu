@@ -103,7 +103,7 @@ static int check_ions(taiga_ctx* ctx, const taiga_ions* ions, bool need_out) {
     return TAIGA_OK;
 }
 
-extern "C" int taiga_seed_beam(taiga_ctx* ctx, const taiga_beam_params* p, uint64_t seed, taiga_ions* ions) {
+static int seed_common(taiga_ctx* ctx, const taiga_beam_params* p, uint64_t seed, taiga_ions* ions, const taiga_seed_grid* g) {
     if (!ctx) return TAIGA_E_ARG;
     if (!p) { TG_SET_ERR(ctx, "seed_beam: null params"); return TAIGA_E_ARG; }
     int rc = check_ions(ctx, ions, false);
@@ -114,10 +114,26 @@ extern "C" int taiga_seed_beam(taiga_ctx* ctx, const taiga_beam_params* p, uint6
     if (!cdf_ok(p->cdf_depth, p->n_depth) || !cdf_ok(p->cdf_normal, p->n_normal)) {
         TG_SET_ERR(ctx, "seed_beam: CDF table must have F[0]=0, F[K]=1 and be non-decreasing"); return TAIGA_E_ARG;
     }
+    if (g) {
+        if (g->nd < 1 || g->nT < 1 || g->nZ < 1 || !(g->z_lim > 0) || !(g->z_lim <= p->z_max)) { TG_SET_ERR(ctx, "seed_beam_grid: bad grid (0 < z_lim <= z_max)"); return TAIGA_E_ARG; }
+        unsigned long long tot = (unsigned long long)g->nd * (unsigned long long)g->nT * (unsigned long long)g->nZ;
+        if (p->first_index > tot || ions->n > tot - p->first_index) { TG_SET_ERR(ctx, "seed_beam_grid: first_index + n exceeds nd*nT*nZ"); return TAIGA_E_ARG; }
+        if (ions->n && !ions->w0) { TG_SET_ERR(ctx, "seed_beam_grid: ions->w0 is null"); return TAIGA_E_ARG; }
+    }
     if (ions->n == 0) return TAIGA_OK;
     TG_CUDA(ctx, cudaSetDevice(ctx->device));
     double v0 = sqrt(2.0 * p->energy_eV * fabs(p->charge_C) / p->mass_kg);   // IEEE sqrt, host
-    return tg_seed(ctx, p, seed, ions, v0);
+    return tg_seed(ctx, p, seed, ions, v0, g);
+}
+
+extern "C" int taiga_seed_beam(taiga_ctx* ctx, const taiga_beam_params* p, uint64_t seed, taiga_ions* ions) {
+    return seed_common(ctx, p, seed, ions, nullptr);
+}
+
+extern "C" int taiga_seed_beam_grid(taiga_ctx* ctx, const taiga_beam_params* p, const taiga_seed_grid* g, taiga_ions* ions) {
+    if (!ctx) return TAIGA_E_ARG;
+    if (!g) { TG_SET_ERR(ctx, "seed_beam_grid: null grid"); return TAIGA_E_ARG; }
+    return seed_common(ctx, p, 0, ions, g);
 }
 
 static int check_det(taiga_ctx* ctx, const taiga_detector* d, bool need_edges) {
@@ -175,7 +191,7 @@ extern "C" int taiga_detector_histogram_weighted(taiga_ctx* ctx, const taiga_ion
     if (rc) return rc;
     if (n_hist < 1 || n_hist > 65536 || !wcounts || !wsummary) { TG_SET_ERR(ctx, "histogram_weighted: bad n_hist / null output"); return TAIGA_E_ARG; }
     if (ions->n == 0) return TAIGA_OK;
-    if (!ions->weight) { TG_SET_ERR(ctx, "histogram_weighted: ions->weight is null"); return TAIGA_E_ARG; }
+    if (!ions->weight && !ions->w0) { TG_SET_ERR(ctx, "histogram_weighted: ions->weight and ions->w0 are null"); return TAIGA_E_ARG; }
     TG_CUDA(ctx, cudaSetDevice(ctx->device));
     return tg_histogram_weighted(ctx, ions, det, n_hist, wcounts, wsummary);
 }

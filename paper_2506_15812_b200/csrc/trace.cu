@@ -27,6 +27,7 @@ struct TraceParams {
     LossDev loss;                     // secondary-ionisation loss model (LOSS kernels)
     double hdt;                       // dt/2
     double* weight;
+    const double* w0;                 // initial statistical weight (null = 1)
     double nrD;                       // normal . origin
     double a1, a2, b1;                // dt/(2 qm), dt^2/8, qm dt/2   (stage 2/3)
     double c6, d6, dtq;               // dt^2/6, qm dt/6, dt/qm
@@ -237,7 +238,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 if (!(s0 < 0.0)) {             // O4: must start in front of the plane
                     P.hit_u[idx] = 0.0; P.hit_w[idx] = 0.0; P.cell[idx] = TAIGA_CELL_BADSTART; P.steps[idx] = 0;
                     P.flags[idx] = (fabs(s0) < TG_GRAZE) ? TAIGA_FLAG_PLANE : 0;
-                    if constexpr (LOSS) P.weight[idx] = 1.0;
+                    if constexpr (LOSS) P.weight[idx] = P.w0 ? P.w0[idx] : 1.0;
                     alive = false;
                 }
             }
@@ -260,7 +261,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
             }
             if (outside || nst == P.max_steps) {
                 uint8_t fl = 0;
-                if constexpr (LOSS) P.weight[idx] = (outside && nst == 0) ? 1.0 : exp(-Lam);
+                if constexpr (LOSS) P.weight[idx] = (P.w0 ? P.w0[idx] : 1.0) * ((outside && nst == 0) ? 1.0 : exp(-Lam));
                 if (outside && (fabs(R - P.f.Rmin) < TG_GRAZE || fabs(R - P.f.Rmax) < TG_GRAZE ||
                                 fabs(Z - P.f.Zmin) < TG_GRAZE || fabs(Z - P.f.Zmax) < TG_GRAZE)) fl = TAIGA_FLAG_GRID;
                 P.hit_u[idx] = 0.0; P.hit_w[idx] = 0.0;
@@ -383,7 +384,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                     if constexpr (LOSS) {               // crossing step: up to the plane, nu interpolated linearly (reading L2)
                         double nun = tg_loss_rate(P, sqrt(fma(Xn, Xn, Yn * Yn)), Zn);
                         double nuh = fma(lam, nun - nu1, nu1);
-                        P.weight[idx] = exp(-fma(lam * P.hdt, nu1 + nuh, Lam));
+                        P.weight[idx] = (P.w0 ? P.w0[idx] : 1.0) * exp(-fma(lam * P.hdt, nu1 + nuh, Lam));
                     }
                     P.steps[idx] = nst;
                     P.flags[idx] = (fabs(s0) < TG_GRAZE || fabs(s1) < TG_GRAZE) ? TAIGA_FLAG_PLANE : 0;
@@ -546,7 +547,7 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     cudaStream_t st = ctx->stream;
     TraceParams P;
     P.f = ctx->field; P.det = det;
-    P.loss = ctx->loss; P.hdt = 0.5 * dt; P.weight = ions->weight;
+    P.loss = ctx->loss; P.hdt = 0.5 * dt; P.weight = ions->weight; P.w0 = ions->w0;
     const bool loss = ctx->loss.psi != nullptr && ions->weight != nullptr;
     if (ctx->opt_precision == 32) {            // fp32 field evaluation (BASELINE config 5 "fp32 variant")
         if (ctx->field.kind != 2 || variant > 1) {

@@ -27,7 +27,7 @@ CELL_MISS, CELL_MAXSTEPS, CELL_OUT, CELL_BADSTART = -1, -2, -3, -4
 FLAG_EDGE, FLAG_PLANE, FLAG_GRID = 1, 2, 4
 
 EXPORTS = ["taiga_create", "taiga_destroy", "taiga_last_error", "taiga_load_field", "taiga_load_loss",
-           "taiga_detector_histogram_weighted",
+           "taiga_detector_histogram_weighted", "taiga_seed_beam_grid",
            "taiga_field_eval", "taiga_field_table", "taiga_seed_beam", "taiga_trace",
            "taiga_detector_histogram", "taiga_set_efield", "taiga_set_option", "taiga_get_stats",
            "taiga_measure_fp64_peak"]
@@ -55,7 +55,11 @@ class BeamS(C.Structure):
 
 class IonsS(C.Structure):
     _fields_ = [(k, C.c_void_p) for k in ("x", "y", "z", "vx", "vy", "vz", "hit_u", "hit_w",
-                                          "cell", "steps", "flags", "group", "t0", "weight")] + [("n", C.c_uint64)]
+                                          "cell", "steps", "flags", "group", "t0", "weight", "w0")] + [("n", C.c_uint64)]
+
+
+class SeedGridS(C.Structure):
+    _fields_ = [("nd", C.c_int), ("nT", C.c_int), ("nZ", C.c_int), ("z_lim", C.c_double)]
 
 
 class LossProfileS(C.Structure):
@@ -81,6 +85,7 @@ _lib.taiga_trace.argtypes = [C.c_void_p, C.POINTER(IonsS), C.c_double, C.c_doubl
                              C.POINTER(DetS), C.c_int]
 _lib.taiga_detector_histogram.argtypes = [C.c_void_p, C.POINTER(IonsS), C.POINTER(DetS), C.c_int,
                                           C.c_void_p, C.c_void_p]
+_lib.taiga_seed_beam_grid.argtypes = [C.c_void_p, C.POINTER(BeamS), C.POINTER(SeedGridS), C.POINTER(IonsS)]
 _lib.taiga_load_loss.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(LossProfileS)]
 _lib.taiga_detector_histogram_weighted.argtypes = [C.c_void_p, C.POINTER(IonsS), C.POINTER(DetS), C.c_int,
                                                    C.c_void_p, C.c_void_p]
@@ -102,26 +107,33 @@ class Ions:
               ("vx", torch.float64), ("vy", torch.float64), ("vz", torch.float64),
               ("hit_u", torch.float64), ("hit_w", torch.float64), ("cell", torch.int32),
               ("steps", torch.int32), ("flags", torch.uint8), ("group", torch.int16),
-              ("t0", torch.float64), ("weight", torch.float64))
+              ("t0", torch.float64), ("weight", torch.float64), ("w0", torch.float64))
 
-    def __init__(self, n, device="cuda:0", _arrays=None):
+    def __init__(self, n, device="cuda:0", _arrays=None, _meta=None):
         self.n = int(n)
         if _arrays is None:
             _arrays = {k: torch.zeros(self.n, dtype=dt, device=device) for k, dt in self._specs}
         self.a = _arrays
+        # use_w0: the w0 array holds initial weights (set by seed_beam_grid, cleared by seed_beam);
+        # otherwise a null w0 pointer (= weight 1) is passed to the library
+        self.meta = _meta if _meta is not None else {"use_w0": False}
 
     def view(self, lo, hi):
-        return Ions(hi - lo, _arrays={k: v[lo:hi] for k, v in self.a.items()})
+        return Ions(hi - lo, _arrays={k: v[lo:hi] for k, v in self.a.items()}, _meta=self.meta)
 
-    def struct(self):
+    def struct(self, weight=True):
         s = IonsS()
         for k, _ in self._specs:
             setattr(s, k, self.a[k].data_ptr() if self.n else None)
+        if not self.meta["use_w0"]:
+            s.w0 = None
+        if not weight:
+            s.weight = None
         s.n = self.n
         return s
 
     def __getattr__(self, k):
-        if k in ("a", "n"):
+        if k in ("a", "n", "meta"):
             raise AttributeError(k)
         return self.a[k]
 
@@ -197,8 +209,24 @@ class Taiga:
         p.cdf_normal, p.n_normal, p.z_max = cn.ctypes.data, len(cn) - 1, beam.z_max
         p.sigma_pos_m, p.sigma_ang_rad = beam.sigma_pos_m, beam.sigma_ang_rad
         p.first_index, p.group, p.t0 = int(first_index), int(group), float(t0)
+        ions.meta["use_w0"] = False
         s = ions.struct()
         self._chk(_lib.taiga_seed_beam(self.h, C.byref(p), C.c_uint64(seed), C.byref(s)))
+
+    def seed_beam_grid(self, beam, cdf_depth, cdf_normal, nd, nT, nZ, z_lim, ions, first_index=0, group=0, t0=0.0):
+        """Deterministic weighted-grid initialisation; writes ions.w0."""
+        cd, cn = _host(cdf_depth), _host(cdf_normal)
+        p = BeamS()
+        p.mass_kg, p.charge_C, p.energy_eV = beam.mass_kg, beam.charge_C, beam.energy_eV
+        p.origin, p.axis, p.eT, p.eZ = D3(*beam.origin), D3(*beam.axis), D3(*beam.eT), D3(*beam.eZ)
+        p.cdf_depth, p.n_depth, p.depth_max = cd.ctypes.data, len(cd) - 1, beam.depth_max
+        p.cdf_normal, p.n_normal, p.z_max = cn.ctypes.data, len(cn) - 1, beam.z_max
+        p.sigma_pos_m, p.sigma_ang_rad = beam.sigma_pos_m, 0.0
+        p.first_index, p.group, p.t0 = int(first_index), int(group), float(t0)
+        g = SeedGridS(int(nd), int(nT), int(nZ), float(z_lim))
+        ions.meta["use_w0"] = True
+        s = ions.struct()
+        self._chk(_lib.taiga_seed_beam_grid(self.h, C.byref(p), C.byref(g), C.byref(s)))
 
     @staticmethod
     def _det(det):
@@ -228,9 +256,10 @@ class Taiga:
             a = _host(psi_nodal)
             self._chk(_lib.taiga_load_loss(self.h, a.ctypes.data, 0, C.byref(prof)))
 
-    def detector_histogram_weighted(self, ions, det, n_hist, wcounts, wsummary):
+    def detector_histogram_weighted(self, ions, det, n_hist, wcounts, wsummary, use_loss_weight=True):
+        """use_loss_weight=False: weight by ions.w0 only (no loss model traced)."""
         d, keep = self._det(det)
-        s = ions.struct()
+        s = ions.struct(weight=use_loss_weight)
         assert wcounts.dtype == torch.int64 and wsummary.dtype == torch.int64
         assert wcounts.numel() == n_hist * d.nu * d.nw and wsummary.numel() == n_hist * 4
         self._chk(_lib.taiga_detector_histogram_weighted(self.h, C.byref(s), C.byref(d), int(n_hist),

@@ -546,3 +546,73 @@ def test_bezier_plane_interpolation_parity(tg, icfg, n):
     cr = (g["status"] == 0) & (g0["status"] == 0)
     d = np.hypot(g["u"][cr] - g0["u"][cr], g["w"][cr] - g0["w"][cr]).max()
     assert 1e-8 < d < 1e-3                    # micrometres (more at grazing incidence): the switch is live
+
+
+def test_deterministic_grid_seeding_parity(tg):
+    """weighted-grid initialisation, bit-exact against the
+    oracle (positions, velocities, weights), incl. sub-ranges (sharding) and a tilted beam frame;
+    then the whole path: trace + loss + weighted counters with the initial weights."""
+    from paper_2506_15812_b200 import taiga
+    cd, cn = wl.depth_cdf(), wl.normal_cdf()
+    tilted = wl.Beam(wl.MASS_NA23, wl.E_CHARGE, 40e3, sigma_pos_m=7e-3, sigma_ang_rad=0.0,
+                     origin=(0.8, 0.01, -0.02), axis=(-0.6, 0.0, 0.8), eT=(0.0, 1.0, 0.0), eZ=(0.8, 0.0, 0.6))
+    tilted.depth_max, tilted.z_max = wl.DEPTH_MAX, wl.NORMAL_ZMAX
+    for beam, (nd, nT, nZ, zl), first, n in ((wl.config(1).groups[0].beam, (64, 9, 11, 6.0), 0, 64 * 9 * 11),
+                                               (tilted, (1000, 31, 17, 3.5), 123457, 10007),
+                                               (tilted, (3, 1, 1, 0.5), 2, 1)):
+        ions = taiga.Ions(n)
+        tg.seed_beam_grid(beam, cd, cn, nd, nT, nZ, zl, ions, first_index=first, group=2, t0=1e-6)
+        torch.cuda.synchronize()
+        st, w0 = orc.seed_grid(beam, cd, cn, nd, nT, nZ, zl, first, n)
+        for k, a in zip(("x", "y", "z", "vx", "vy", "vz"), st):
+            assert np.array_equal(_np(ions.a[k]), a), k
+        assert np.array_equal(_np(ions.w0), w0)
+        assert np.all(_np(ions.group) == 2) and np.all(_np(ions.t0) == 1e-6)
+    with pytest.raises(taiga.TaigaError):
+        tg.seed_beam_grid(tilted, cd, cn, 3, 1, 1, 0.5, taiga.Ions(2), first_index=2)       # beyond the grid
+    # whole path on config 1's field: grid seeding -> trace with the loss model -> weighted counters
+    cfg = wl.config(1)
+    grid, nodal = cfg.field_builder()
+    g = cfg.groups[0]
+    nd, nT, nZ, zl = 128, 7, 7, 4.0
+    n = nd * nT * nZ
+    psi0, dpsi, ne, te = wl.loss_profile_inputs()
+    psi_nodal = wl.nodal_psi(grid)
+    tg.load_field(grid, nodal)
+    ions = taiga.Ions(n)
+    counts = torch.zeros((1, 8, 8), dtype=torch.int64, device="cuda")
+    summary = torch.zeros((1, 6), dtype=torch.int64, device="cuda")
+    wcounts = torch.zeros((1, 8, 8), dtype=torch.int64, device="cuda")
+    wsummary = torch.zeros((1, 4), dtype=torch.int64, device="cuda")
+    w0counts, w0summary = torch.zeros_like(wcounts), torch.zeros_like(wsummary)
+    qm = g.beam.charge_C / g.beam.mass_kg
+    try:
+        tg.load_loss(psi_nodal, psi0, dpsi, ne, te, wl.E12_LI)
+        tg.seed_beam_grid(g.beam, cd, cn, nd, nT, nZ, zl, ions)
+        tg.trace(ions, qm, cfg.dt, cfg.max_steps, cfg.detector)
+        tg.detector_histogram(ions, cfg.detector, 1, counts, summary)
+        tg.detector_histogram_weighted(ions, cfg.detector, 1, wcounts, wsummary)
+        tg.detector_histogram_weighted(ions, cfg.detector, 1, w0counts, w0summary, use_loss_weight=False)
+        torch.cuda.synchronize()
+    finally:
+        tg.load_loss(None)
+    f = orc.OracleField(grid, nodal)
+    L = orc.OracleLoss(grid, psi_nodal, psi0, dpsi, orc.mcwhirter_rate(ne, te, wl.E12_LI))
+    st, w0 = orc.seed_grid(g.beam, cd, cn, nd, nT, nZ, zl, 0, n)
+    res = orc.trace_loss(f, L, qm, st, None, cfg.dt, cfg.max_steps, cfg.detector, w0=w0)
+    orc.histogram(res, None, cfg.detector, 1)
+    ok = ((_np(ions.flags) | res["flags"]) == 0)
+    assert ok.mean() > 0.99
+    assert np.array_equal(_np(ions.cell)[ok], res["cell"][ok]) and np.array_equal(_np(ions.steps)[ok].astype(np.uint32), res["steps"][ok])
+    nz = ok & (res["weight"] > 0)
+    assert np.abs(_np(ions.weight)[nz] / res["weight"][nz] - 1).max() < 1e-12
+    assert np.array_equal(_np(ions.weight)[ok & ~nz], res["weight"][ok & ~nz])
+    wc_ref, ws_ref = orc.histogram_weighted(dict(cell=np.where(ok, res["cell"], _np(ions.cell)).astype(np.int32),
+                                                 weight=np.where(ok, res["weight"], _np(ions.weight))), None, cfg.detector, 1)
+    assert np.abs(_np(wcounts) - wc_ref.astype(np.int64)).sum() <= 8 and np.abs(_np(wsummary)[:, :2] - ws_ref[:, :2].astype(np.int64)).sum() <= 8
+    # w0-only counters: exact integers (identical doubles on both sides)
+    w0_ref, w0s_ref = orc.histogram_weighted(dict(cell=_np(ions.cell), weight=w0), None, cfg.detector, 1)
+    assert np.array_equal(_np(w0counts), w0_ref.astype(np.int64)) and np.array_equal(_np(w0summary), w0s_ref.astype(np.int64))
+    # the loss reduces the weighted signal by about a percent for these profiles
+    ratio = _np(wsummary)[0, :2].sum() / _np(w0summary)[0, :2].sum()
+    assert 0.95 < ratio < 0.999
