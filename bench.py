@@ -25,8 +25,8 @@ sys.path.insert(0, ROOT)
 # (3 field evaluations x 61 + 4 cross products x 6 + stage/Eq.5/plane 45).
 ALG_FP64_INSTR_PER_ION_STEP = {0: 252.0, 1: 402.0, 2: 840.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_trace launch on config 2, from the
-# `ncu --set full` capture summarised in profiles/r1c_trace_ncu.md (per launch; None elsewhere)
-NCU_DRAM_BYTES_PER_LAUNCH = {2: 233.7e6}
+# `ncu --set full` capture summarised in profiles/r1d_trace_ncu.md (per launch; None elsewhere)
+NCU_DRAM_BYTES_PER_LAUNCH = {2: 244.5e6}
 
 
 def parse():
