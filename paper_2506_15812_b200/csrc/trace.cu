@@ -608,18 +608,18 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         }
         grid = (unsigned)(ctx->sm_count * 2); if (grid > need) grid = need;
         const int kind = ctx->field.kind;
-        if (kind == 0 && variant == 0) TG_LAUNCH(0, true, 128, 255, 0, 0, false, false, true);
+        if (kind == 0 && variant == 0) TG_LAUNCH(0, true, 128, 255, 2, 0, false, false, true);
         else if (kind == 0) TG_LAUNCH(0, false, 128, 255, 0, 0, false, false, true);
         else if (kind == 1) TG_LAUNCH(1, false, 128, 255, 0, 0, false, false, true);
         else TG_LAUNCH(2, false, 128, 255, 0, 0, false, false, true);
-    } else if (loss) {                     // RKN + Eq. 2 loss integral: on-demand cache (kind 0) / uncached gathers
+    } else if (loss) {                     // RKN + Eq. 2 loss integral: rolling-refill cache (kind 0) / uncached gathers
         if (variant > 1 || hasE || ctx->opt_precision == 32) {
             TG_SET_ERR(ctx, "the loss model is offered with the RKN solvers, E = 0, fp64");
             return TAIGA_E_ARG;
         }
         grid = (unsigned)(ctx->sm_count * 2); if (grid > need) grid = need;
         const int kind = ctx->field.kind;
-        if (kind == 0 && variant == 0) TG_LAUNCH(0, true, 128, 255, 0, 0, false, true);
+        if (kind == 0 && variant == 0) TG_LAUNCH(0, true, 128, 255, 2, 0, false, true);
         else if (kind == 0) TG_LAUNCH(0, false, 128, 255, 0, 0, false, true);
         else if (kind == 1) TG_LAUNCH(1, false, 128, 255, 0, 0, false, true);
         else TG_LAUNCH(2, false, 128, 255, 0, 0, false, true);
@@ -632,12 +632,12 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     case 1: if (kv == 2) TG_LAUNCH(1, false, 128, 128); else TG_LAUNCH(1, false, 128, 255); break;
     default: if (kv == 2) TG_LAUNCH(2, false, 128, 128); else TG_LAUNCH(2, false, 128, 255); break;
     }
-    } else {                               // other solvers (Eq. 4, Eq. 7-8) and / or a uniform E: on-demand cache, 8 warps/SM
+    } else {                               // other solvers (Eq. 4, Eq. 7-8: on-demand cache) and / or a uniform E (RKN: rolling refill), 8 warps/SM
         grid = (unsigned)(ctx->sm_count * 2); if (grid > need) grid = need;
         const int S = variant <= 1 ? 0 : (variant == 2 ? 2 : 3);
         const int kind = ctx->field.kind;
         if (kind == 0 && variant == 1) TG_LAUNCH(0, false, 128, 255, 0, 0, true);
-        else if (kind == 0 && S == 0) TG_LAUNCH(0, true, 128, 255, 0, 0, true);
+        else if (kind == 0 && S == 0) TG_LAUNCH(0, true, 128, 255, 2, 0, true);
         else if (kind == 0 && S == 2) TG_LAUNCH(0, true, 128, 255, 0, 2, true);
         else if (kind == 0) TG_LAUNCH(0, true, 128, 255, 0, 3, true);
         else if (kind == 1 && S == 0) TG_LAUNCH(1, false, 128, 255, 0, 0, true);
