@@ -176,6 +176,19 @@ static std::vector<double> circulant_inverse_col(int n) {
     return x;
 }
 
+// kind 1: D[cell][k] = T[cell][k+1] - T[cell][k], so that B(t) = H(T_k) + tau H(D_k) and the tracer can keep
+// T_k in registers and gather only D_k (half the bytes of gathering both slices)
+__global__ void k_slice_diff(const double* __restrict__ T, double* __restrict__ D, long long ncell, int nS) {
+    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    long long tot = ncell * (nS - 1) * 48;
+    if (t >= tot) return;
+    int e = (int)(t % 48);
+    long long ck = t / 48, cell = ck / (nS - 1);
+    int k = (int)(ck % (nS - 1));
+    const double* a = T + ((cell * nS + k) * 48 + e);
+    D[t] = a[48] - a[0];
+}
+
 int tg_precompute(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c) {
     const int nR = g->nR, nZ = g->nZ, nS = g->nS, cR = nR - 1, cZ = nZ - 1;
     const long long ncell = (long long)cR * cZ, nnode = (long long)nS * nR * nZ;
@@ -254,7 +267,15 @@ int tg_precompute(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c) {
     f.inv_hR = 1.0 / hR; f.inv_hZ = 1.0 / hZ;
     f.offR = g->Rmin / hR; f.offZ = g->Zmin / hZ;
     f.s0 = g->s0; f.inv_ds = (g->kind == 0) ? 0.0 : 1.0 / g->ds;
-    f.table = ctx->table; f.table32 = nullptr;
+    f.table = ctx->table; f.table32 = nullptr; f.dtable = nullptr;
+    if (g->kind == 1) {
+        size_t nd = (size_t)ncell * (nS - 1) * 48;
+        int rc2 = tg_reserve(ctx, &ctx->dtable, &ctx->cap_dtable, nd);
+        if (rc2) return rc2;
+        k_slice_diff<<<(unsigned)((nd + 255) / 256), 256, 0, st>>>(ctx->table, ctx->dtable, ncell, nS);
+        TG_CUDA(ctx, cudaGetLastError());
+        f.dtable = ctx->dtable;
+    }
     return TAIGA_OK;
 }
 

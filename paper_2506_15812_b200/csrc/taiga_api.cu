@@ -50,7 +50,7 @@ extern "C" int taiga_destroy(taiga_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     void* bufs[] = {ctx->table, ctx->scratch, ctx->band[0], ctx->band[1], ctx->cdf_depth, ctx->cdf_normal, ctx->edges, ctx->order,
                     ctx->bins, ctx->surv[0], ctx->surv[1], ctx->surv_idx[0], ctx->surv_idx[1],
-                    ctx->surv_steps[0], ctx->surv_steps[1], ctx->counters, ctx->table32, ctx->psi_table, ctx->loss_rate};
+                    ctx->surv_steps[0], ctx->surv_steps[1], ctx->counters, ctx->table32, ctx->psi_table, ctx->loss_rate, ctx->dtable};
     for (void* b : bufs) if (b) cudaFree(b);
     if (ctx->counters_host) cudaFreeHost(ctx->counters_host);
     delete ctx;

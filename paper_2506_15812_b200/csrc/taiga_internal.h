@@ -19,6 +19,7 @@ struct FieldDev {
     // kind 1: [iR][iZ][slice][comp][16]     (the two slices of a cell are adjacent)
     // kind 2: [iphi][iR][iZ][comp][64]
     const double* table;
+    const double* dtable;            // kind 1: slice differences [iR][iZ][k < nS-1][comp][16] = table[k+1] - table[k]
     const float* table32;            // kind 2, "precision" = 32: the same table rounded to fp32 (else null)
 };
 
@@ -45,6 +46,7 @@ struct taiga_ctx {
     FieldDev field;
     double* table;            size_t table_bytes;
     double* scratch;          size_t scratch_bytes;     // precompute work arrays
+    double* dtable;           size_t cap_dtable;
     float* table32;           size_t cap_table32;  bool table32_valid;   // fp32 copy of a kind-2 table
     double* band[2];          size_t band_cap[2]; int band_n[2];   // y -> y'' band operators (Z, R)
 

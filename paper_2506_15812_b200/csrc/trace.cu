@@ -66,7 +66,11 @@ struct CellCache<0> {
     double oR, oZ;                             // offR + i, offZ + j of the cached cell
 };
 template <>
-struct CellCache<1> {};
+struct CellCache<1> {                          // slice k of the current cell; the slice difference is gathered
+    double c[48];
+    double oR, oZ;
+    int k, cell;                               // cached slice, linear cell index i * cZ + j
+};
 template <>
 struct CellCache<2> {};
 
@@ -105,6 +109,19 @@ __device__ __forceinline__ void tg_ldpred16(const double* src, int need, double*
                      : "l"(src + 4 * k), "r"(need));
 }
 
+// kind 1: re-read slice k of the cell containing the global cell coordinates (pR, pZ)
+__device__ __forceinline__ void tg_refill1(const TraceParams& P, CellCache<1>& cc, unsigned& reloads, double pR, double pZ, int k) {
+    int i = tg_clampi(__double2int_rd(pR), 0, P.f.cR - 1), j = tg_clampi(__double2int_rd(pZ), 0, P.f.cZ - 1);
+    cc.oR = P.f.offR + (double)i; cc.oZ = P.f.offZ + (double)j; cc.k = k; cc.cell = i * P.f.cZ + j;
+    const double* src = P.f.table + ((size_t)cc.cell * P.f.nS + k) * 48;
+#pragma unroll
+    for (int q = 0; q < 12; ++q)
+        asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];"
+                     : "+d"(cc.c[4 * q]), "+d"(cc.c[4 * q + 1]), "+d"(cc.c[4 * q + 2]), "+d"(cc.c[4 * q + 3])
+                     : "l"(src + 4 * q));
+    ++reloads;
+}
+
 template <int KIND, bool CACHED, bool FIRST = false, bool ROLL = false>
 __device__ __forceinline__ void tg_fieldCyl(const TraceParams& P, CellCache<KIND>& cc, unsigned& reloads, bool& outside,
                                             double X, double Y, double Z, double t, double R,
@@ -135,6 +152,36 @@ __device__ __forceinline__ void tg_fieldCyl(const TraceParams& P, CellCache<KIND
         BR = tg_horner16(cc.c, tR, tZ);      tg_ldpred16(src, need, cc.c);
         BZ = tg_horner16(cc.c + 16, tR, tZ); tg_ldpred16(src + 16, need, cc.c + 16);
         Bp = tg_horner16(cc.c + 32, tR, tZ); tg_ldpred16(src + 32, need, cc.c + 32);
+    } else if constexpr (KIND == 1 && CACHED) {
+        // Time slices: B(t) = H(T_k) + tau H(T_k+1 - T_k).  Slice k of the current cell is cached in
+        // registers with the same rolling predictive refill as kind 0; only the slice DIFFERENCE is
+        // gathered (384 instead of 768 bytes per lane and evaluation).
+        double xs = (t - P.f.s0) * P.f.inv_ds;
+        int k = tg_clampi(__double2int_rd(xs), 0, P.f.nS - 2);
+        double tau = fmin(fmax(xs - (double)k, 0.0), 1.0);
+        tR = fma(R, P.f.inv_hR, -cc.oR); tZ = fma(Z, P.f.inv_hZ, -cc.oZ);
+        if (!(tg_in01(tR) && tg_in01(tZ)) || k != cc.k) {
+            if constexpr (FIRST) outside = (R < P.f.Rmin) | (R > P.f.Rmax) | (Z < P.f.Zmin) | (Z > P.f.Zmax);
+            tg_refill1(P, cc, reloads, fma(R, P.f.inv_hR, -P.f.offR), fma(Z, P.f.inv_hZ, -P.f.offZ), k);
+            tR = fma(R, P.f.inv_hR, -cc.oR); tZ = fma(Z, P.f.inv_hZ, -cc.oZ);
+        }
+        const double* dsrc = P.f.dtable + ((size_t)cc.cell * (P.f.nS - 1) + k) * 48;   // of the CURRENT cell
+        double tRp = tR + dR, tZp = tZ + dZ;
+        int need = ROLL && !(tg_in01(tRp) && tg_in01(tZp));
+        const double* src = P.f.table;
+        if (need) {
+            int i = tg_clampi(__double2int_rd(tRp + (cc.oR - P.f.offR)), 0, P.f.cR - 1);
+            int j = tg_clampi(__double2int_rd(tZp + (cc.oZ - P.f.offZ)), 0, P.f.cZ - 1);
+            cc.oR = P.f.offR + (double)i; cc.oZ = P.f.offZ + (double)j; cc.cell = i * P.f.cZ + j;
+            src += ((size_t)cc.cell * P.f.nS + k) * 48;
+            ++reloads;
+        }
+        double a0 = tg_horner16(cc.c, tR, tZ);      tg_ldpred16(src, need, cc.c);
+        double a1 = tg_horner16(cc.c + 16, tR, tZ); tg_ldpred16(src + 16, need, cc.c + 16);
+        double a2 = tg_horner16(cc.c + 32, tR, tZ); tg_ldpred16(src + 32, need, cc.c + 32);
+        BR = fma(tau, tg_bicubic(dsrc, tR, tZ), a0);
+        BZ = fma(tau, tg_bicubic(dsrc + 16, tR, tZ), a1);
+        Bp = fma(tau, tg_bicubic(dsrc + 32, tR, tZ), a2);
     } else if constexpr (KIND == 0 && CACHED) {
         tR = fma(R, P.f.inv_hR, -cc.oR); tZ = fma(Z, P.f.inv_hZ, -cc.oZ);
         if (!(tg_in01(tR) && tg_in01(tZ))) {
@@ -207,7 +254,8 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     CellCache<KIND> cc;
-    if constexpr (KIND == 0 && CACHED) { cc.oR = 1e300; cc.oZ = 1e300;
+    if constexpr (KIND == 1 && CACHED) { cc.k = -1; cc.cell = 0; }
+    if constexpr (KIND <= 1 && CACHED) { cc.oR = 1e300; cc.oZ = 1e300;
 #pragma unroll
         for (int k = 0; k < 48; ++k) cc.c[k] = 0.0; }
     double X = 0, Y = 0, Z = 0, Ux = 0, Uy = 0, Uz = 0, t = 0, s0 = -1.0;
@@ -594,7 +642,8 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     //   3: cache on demand, 3 x 128 (168 regs)
     //   1: no cache, 2 x 128   2: no cache, 4 x 128 (128 regs)   (the only ones for kinds 1, 2)
     int kv = ctx->opt_variant;
-    if (ctx->field.kind != 0 || variant != 0) kv = (kv == 2 || kv == 3) ? 2 : 1;   // (the cached kernels assume k2 and k3 share their position)
+    if (ctx->field.kind == 2 || variant != 0) kv = (kv == 2 || kv == 3) ? 2 : 1;   // (the cached kernels assume k2 and k3 share their position)
+    else if (ctx->field.kind == 1 && kv != 0) kv = (kv == 2 || kv == 3) ? 2 : 1;    // kind 1: 0 = slice cache + rolling refill, else uncached
     const int threads = 128;
     int per_sm = ctx->opt_ctas_per_sm > 0 ? ctx->opt_ctas_per_sm : (kv == 2 ? 4 : (kv == 3 ? 3 : 2));
     unsigned grid = (unsigned)(ctx->sm_count * per_sm);
@@ -629,7 +678,7 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         if (kv == 0) TG_LAUNCH(0, true, 128, 255, 2); else if (kv == 4) TG_LAUNCH(0, true, 128, 255, 1); else if (kv == 5) TG_LAUNCH(0, true, 128, 255); else if (kv == 3) TG_LAUNCH(0, true, 128, 168);
         else if (kv == 2) TG_LAUNCH(0, false, 128, 128); else TG_LAUNCH(0, false, 128, 255);
         break;
-    case 1: if (kv == 2) TG_LAUNCH(1, false, 128, 128); else TG_LAUNCH(1, false, 128, 255); break;
+    case 1: if (kv == 2) TG_LAUNCH(1, false, 128, 128); else if (kv == 1) TG_LAUNCH(1, false, 128, 255); else TG_LAUNCH(1, true, 128, 255, 2); break;
     default: if (kv == 2) TG_LAUNCH(2, false, 128, 128); else TG_LAUNCH(2, false, 128, 255); break;
     }
     } else {                               // other solvers (Eq. 4, Eq. 7-8: on-demand cache) and / or a uniform E (RKN: rolling refill), 8 warps/SM
