@@ -37,7 +37,7 @@ extern "C" int taiga_create(taiga_ctx** out, int device, void* cuda_stream) {
         delete ctx; return TAIGA_E_NOMEM;
     }
     ctx->opt_sort = 1; ctx->opt_sort_sub = 16;
-    ctx->opt_chunk0 = 0; ctx->opt_chunk = 2048; ctx->opt_min_active = 32;
+    ctx->opt_min_active = 32;
     ctx->opt_ctas_per_sm = 0; ctx->opt_variant = 0; ctx->opt_stats = 1; ctx->opt_precision = 64; ctx->opt_plane_interp = 0;
     strcpy(ctx->err, "ok");
     *out = ctx;
@@ -49,8 +49,7 @@ extern "C" int taiga_destroy(taiga_ctx* ctx) {
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     void* bufs[] = {ctx->table, ctx->scratch, ctx->band[0], ctx->band[1], ctx->cdf_depth, ctx->cdf_normal, ctx->edges, ctx->order,
-                    ctx->bins, ctx->surv[0], ctx->surv[1], ctx->surv_idx[0], ctx->surv_idx[1],
-                    ctx->surv_steps[0], ctx->surv_steps[1], ctx->counters, ctx->table32, ctx->psi_table, ctx->loss_rate, ctx->dtable};
+                    ctx->bins, ctx->counters, ctx->table32, ctx->psi_table, ctx->loss_rate, ctx->dtable};
     for (void* b : bufs) if (b) cudaFree(b);
     if (ctx->counters_host) cudaFreeHost(ctx->counters_host);
     delete ctx;
@@ -219,8 +218,8 @@ extern "C" int taiga_detector_histogram(taiga_ctx* ctx, const taiga_ions* ions, 
 extern "C" int taiga_set_option(taiga_ctx* ctx, const char* key, long long v) {
     if (!ctx || !key) return TAIGA_E_ARG;
     struct { const char* k; int* p; } tab[] = {
-        {"sort", &ctx->opt_sort}, {"sort_sub", &ctx->opt_sort_sub}, {"chunk0", &ctx->opt_chunk0},
-        {"chunk", &ctx->opt_chunk}, {"precision", &ctx->opt_precision}, {"plane_interp", &ctx->opt_plane_interp}, {"min_active", &ctx->opt_min_active},
+        {"sort", &ctx->opt_sort}, {"sort_sub", &ctx->opt_sort_sub},
+        {"precision", &ctx->opt_precision}, {"plane_interp", &ctx->opt_plane_interp}, {"min_active", &ctx->opt_min_active},
         {"ctas_per_sm", &ctx->opt_ctas_per_sm}, {"variant", &ctx->opt_variant}, {"stats", &ctx->opt_stats}};
     for (auto& t : tab) if (!strcmp(key, t.k)) { *t.p = (int)v; return TAIGA_OK; }
     TG_SET_ERR(ctx, "set_option: unknown key '%s'", key);

@@ -66,15 +66,12 @@ struct taiga_ctx {
     // trace scratch
     uint32_t* order;          size_t cap_order;          // permutation (sorted by birth cell)
     uint32_t* bins;           size_t cap_bins;           // counting-sort bins
-    double* surv[2];          size_t cap_surv;           // survivor state, ping-pong: 7 doubles/ion
-    uint32_t* surv_idx[2];
-    uint32_t* surv_steps[2];
     unsigned long long* counters;                        // device counters (16)
     unsigned long long* counters_host;                   // pinned mirror
     unsigned long long stats[8];
 
     // options
-    int opt_sort, opt_chunk0, opt_chunk, opt_min_active, opt_ctas_per_sm, opt_variant, opt_stats;
+    int opt_sort, opt_min_active, opt_ctas_per_sm, opt_variant, opt_stats;
     int opt_sort_sub, opt_precision, opt_plane_interp;
 };
 

@@ -616,3 +616,63 @@ def test_deterministic_grid_seeding_parity(tg):
     # the loss reduces the weighted signal by about a percent for these profiles
     ratio = _np(wsummary)[0, :2].sum() / _np(w0summary)[0, :2].sum()
     assert 0.95 < ratio < 0.999
+
+
+def test_error_paths_of_the_widened_entry_points(tg):
+    """Combinations that are not offered are refused (TAIGA_E_ARG / TAIGA_E_STATE), never computed
+    differently; null / malformed inputs are rejected."""
+    from paper_2506_15812_b200 import taiga
+    cfg = wl.config(1, n_override=64)
+    grid, nodal = cfg.field_builder()
+    psi0, dpsi, ne, te = wl.loss_profile_inputs()
+    g = cfg.groups[0]
+    qm = g.beam.charge_C / g.beam.mass_kg
+    t2 = taiga.Taiga(0)
+    with pytest.raises(taiga.TaigaError) as e:
+        t2.load_loss(wl.nodal_psi(grid), psi0, dpsi, ne, te, wl.E12_LI)            # before load_field
+    assert e.value.code == taiga.E_STATE
+    t2.load_field(grid, nodal)
+    for bad in (dict(dpsi=0.0), dict(E12=-1.0), dict(ne=-ne), dict(ne=ne[:1], te=te[:1])):
+        kw = dict(psi0=psi0, dpsi=dpsi, ne=ne, Te=te, E12=wl.E12_LI)
+        kw.update({("Te" if k == "te" else k): v for k, v in bad.items()})
+        with pytest.raises(taiga.TaigaError) as e:
+            t2.load_loss(wl.nodal_psi(grid), **kw)
+        assert e.value.code == taiga.E_ARG
+    ions = taiga.Ions(64)
+    t2.seed_beam(g.beam, wl.depth_cdf(), wl.normal_cdf(), 0, ions)
+    with pytest.raises(taiga.TaigaError):
+        t2.trace(ions, qm, cfg.dt, 100, cfg.detector, 5)                            # unknown solver
+    with pytest.raises(taiga.TaigaError):
+        t2.set_efield((float("nan"), 0.0, 0.0))
+    t2.load_loss(wl.nodal_psi(grid), psi0, dpsi, ne, te, wl.E12_LI)
+    for setup in (lambda: t2.set_option("plane_interp", 1), lambda: t2.set_efield((1e3, 0, 0))):
+        setup()
+        with pytest.raises(taiga.TaigaError) as e:
+            t2.trace(ions, qm, cfg.dt, 100, cfg.detector)                           # loss + Bezier / loss + E
+        assert e.value.code == taiga.E_ARG
+        t2.set_option("plane_interp", 0); t2.set_efield((0, 0, 0))
+    with pytest.raises(taiga.TaigaError):
+        t2.trace(ions, qm, cfg.dt, 100, cfg.detector, 3)                            # loss + Boris
+    t2.load_loss(None)
+    t2.set_option("plane_interp", 1)
+    with pytest.raises(taiga.TaigaError):
+        t2.trace(ions, qm, cfg.dt, 100, cfg.detector, 2)                            # Bezier + RK4
+    t2.set_option("plane_interp", 0)
+    t2.set_option("precision", 16)
+    with pytest.raises(taiga.TaigaError):
+        t2.trace(ions, qm, cfg.dt, 100, cfg.detector)
+    t2.set_option("precision", 64)
+    # a new field invalidates the loss model (psi lives on the old grid)
+    t2.load_loss(wl.nodal_psi(grid), psi0, dpsi, ne, te, wl.E12_LI)
+    t2.load_field(grid, nodal)
+    ions.a["weight"].fill_(5.0)
+    t2.trace(ions, qm, cfg.dt, 100, cfg.detector)
+    torch.cuda.synchronize()
+    assert float(ions.weight.min()) == 5.0
+    # weighted histogram needs weights
+    wc = torch.zeros((1, 8, 8), dtype=torch.int64, device="cuda"); ws = torch.zeros((1, 4), dtype=torch.int64, device="cuda")
+    s = ions.struct(weight=False)
+    assert s.w0 is None
+    with pytest.raises(taiga.TaigaError):
+        t2.detector_histogram_weighted(ions, cfg.detector, 1, wc, ws, use_loss_weight=False)
+    t2.close()
