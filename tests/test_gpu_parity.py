@@ -676,3 +676,40 @@ def test_error_paths_of_the_widened_entry_points(tg):
     with pytest.raises(taiga.TaigaError):
         t2.detector_histogram_weighted(ions, cfg.detector, 1, wc, ws, use_loss_weight=False)
     t2.close()
+
+
+def test_printed_k3_variant_with_loss_and_with_bezier(tg):
+    """The printed-Eq. 6 RKN reading (solver 1) through the loss and the Bezier kernels (uncached
+    instantiations, since k2 and k3 no longer share their position)."""
+    from paper_2506_15812_b200 import taiga
+    cfg = wl.config(1, n_override=1024 + 9)
+    grid, nodal = cfg.field_builder()
+    g = cfg.groups[0]
+    qm = g.beam.charge_C / g.beam.mass_kg
+    psi0, dpsi, ne, te = wl.loss_profile_inputs()
+    psi_nodal = wl.nodal_psi(grid)
+    f = orc.OracleField(grid, nodal)
+    st = orc.seed(g.beam, wl.depth_cdf(), wl.normal_cdf(), cfg.seed, 0, cfg.n_ions)
+    tg.load_field(grid, nodal)
+    try:
+        tg.load_loss(psi_nodal, psi0, dpsi, ne, te, wl.E12_LI)
+        ions, counts, summary = taiga.run_config(tg, cfg, field_loaded=True, rkn_variant=1)
+        torch.cuda.synchronize()
+    finally:
+        tg.load_loss(None)
+    L = orc.OracleLoss(grid, psi_nodal, psi0, dpsi, orc.mcwhirter_rate(ne, te, wl.E12_LI))
+    res = orc.trace_loss(f, L, qm, st, None, cfg.dt, cfg.max_steps, cfg.detector, variant=1)
+    orc.histogram(res, None, cfg.detector, 1)
+    ok = (_np(ions.flags) | res["flags"]) == 0
+    assert np.array_equal(_np(ions.cell)[ok], res["cell"][ok]) and np.array_equal(_np(ions.steps)[ok].astype(np.uint32), res["steps"][ok])
+    assert np.abs(_np(ions.weight)[ok] / res["weight"][ok] - 1).max() < 1e-12
+    cr = ok & (res["status"] == 0)
+    assert np.abs(_np(ions.hit_w)[cr] - res["w"][cr]).max() < TOL_UW
+    try:
+        tg.set_option("plane_interp", 1)
+        ions, counts, summary = taiga.run_config(tg, cfg, field_loaded=True, rkn_variant=1)
+        torch.cuda.synchronize()
+    finally:
+        tg.set_option("plane_interp", 0)
+    ref = orc.run_config(cfg, field=f, variant=1, interp=1)
+    compare_groups(ions, ref, "cfg1 printed k3 + bezier")
