@@ -290,6 +290,18 @@ class Taiga:
         return r.value
 
 
+def loss_statistics(wsummary):
+    """Mean and standard deviation of the secondary-ionisation loss 1 - weight over the plane-crossing
+    ions of each histogram (the form of PAPER.md Table 1), from the 32.32 fixed-point sums
+    wsummary[n_hist][4] = {sum q in segments, sum q outside, sum q^2 >> 32, crossers}.  Host arithmetic
+    on a few integers (the division by N the paper does on the CPU, L350)."""
+    ws = np.asarray(wsummary.detach().cpu().numpy() if isinstance(wsummary, torch.Tensor) else wsummary, dtype=np.float64)
+    n = np.maximum(ws[:, 3], 1.0)
+    mean_w = (ws[:, 0] + ws[:, 1]) / 4294967296.0 / n
+    var_w = np.maximum(ws[:, 2] / 4294967296.0 / n - mean_w ** 2, 0.0)
+    return 1.0 - mean_w, np.sqrt(var_w)
+
+
 def run_config(tg: Taiga, cfg, field_loaded=False, host_field=True, ions=None, rkn_variant=0):
     """Whole hot path (a1-a5) of one workloads.Config through the C ABI.  Returns
     (ions, counts, summary) with counts/summary as device int64 tensors."""

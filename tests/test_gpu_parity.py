@@ -488,6 +488,7 @@ def test_secondary_ionisation_loss_parity(tg, icfg, n, species):
     wc_ref = np.zeros((cfg.n_hist, det0.nw, det0.nu), dtype=np.uint64)
     ws_ref = np.zeros((cfg.n_hist, 4), dtype=np.uint64)
     off, n_cross, worst, n_round = 0, 0, 0.0, 0
+    ref_weights = []
     for g in cfg.groups:
         det = g.detector or cfg.detector
         st = orc.seed(g.beam, cd, cn, cfg.seed, g.first_index, g.n_ions)
@@ -509,6 +510,7 @@ def test_secondary_ionisation_loss_parity(tg, icfg, n, species):
         qg = np.floor(wg * 4294967296.0 + 0.5); qr = np.floor(res_w["weight"] * 4294967296.0 + 0.5)
         n_round += int((qg != qr).sum())
         n_cross += int((res["status"] == 0).sum())
+        ref_weights.append(res["weight"][res["status"] == 0])
         off += g.n_ions
     assert worst < 1e-12, worst
     wc, ws = _np(wcounts).astype(np.int64), _np(wsummary).astype(np.int64)
@@ -520,6 +522,11 @@ def test_secondary_ionisation_loss_parity(tg, icfg, n, species):
     # the loss is live: percent level for these profiles
     loss = 1.0 - ws[:, :2].sum() / 4294967296.0 / max(ws[:, 3].sum(), 1)
     assert 1e-3 < loss < 0.5, loss
+    # Table-1 style statistics from the fixed-point sums against the oracle's per-ion weights
+    if cfg.n_hist == 1:
+        mean_loss, std_loss = taiga.loss_statistics(wsummary)
+        wr_all = np.concatenate([r for r in ref_weights])
+        assert abs(mean_loss[0] - (1.0 - wr_all.mean())) < 1e-9 and abs(std_loss[0] - wr_all.std()) < 1e-6
     # without a loss model the same call leaves the weights alone
     ions.a["weight"].fill_(7.0)
     taiga.run_config(tg, wl.config(icfg, n_override=64), field_loaded=True, ions=ions.view(0, 64 * len(cfg.groups)))
