@@ -720,3 +720,68 @@ def test_printed_k3_variant_with_loss_and_with_bezier(tg):
         tg.set_option("plane_interp", 0)
     ref = orc.run_config(cfg, field=f, variant=1, interp=1)
     compare_groups(ions, ref, "cfg1 printed k3 + bezier")
+
+
+def _random_scenario(rng):
+    """A small random but physically sensible setup: grid size, field kind, species, energy, beam
+    direction tilt, divergence, tilted detector plane with a gapped non-uniform matrix, dt, solver,
+    E field, plane interpolation."""
+    kind = int(rng.integers(0, 3))
+    nR, nZ = int(rng.integers(9, 41)), int(rng.integers(12, 61))
+    if kind == 0:
+        fb = lambda: wl.nodal_field_2d(nR, nZ)
+    elif kind == 1:
+        nS = int(rng.integers(2, 7))
+        fb = lambda: wl.nodal_field_time_slices(nR, nZ, nS, dt_slice=2.0e-7)
+    else:
+        nS = int(rng.integers(3, 9))
+        fb = lambda: wl.nodal_field_ripple(nR, nZ, nS)
+    species = wl.MASS_LI7 if rng.random() < 0.6 else wl.MASS_NA23
+    energy = float(rng.uniform(20e3, 90e3))
+    tilt = rng.normal(0, 0.05, 2)
+    axis = np.array([-1.0, tilt[0], tilt[1]]); axis /= np.linalg.norm(axis)
+    eT = np.cross([0.0, 0.0, 1.0], axis); eT /= np.linalg.norm(eT)
+    eZ = np.cross(axis, eT)
+    beam = wl.Beam(species, wl.E_CHARGE, energy, sigma_pos_m=float(rng.uniform(1e-3, 8e-3)),
+                   sigma_ang_rad=float(rng.choice([0.0, 1e-3, 4e-3])), origin=(0.78, 0.0, float(rng.uniform(-0.03, 0.03))),
+                   axis=tuple(axis), eT=tuple(eT), eZ=tuple(eZ))
+    beam.depth_max, beam.z_max = wl.DEPTH_MAX, wl.NORMAL_ZMAX
+    # detector plane: normal tilted a few degrees from +X, anywhere the ions pass (most will miss the matrix)
+    a, b = rng.normal(0, 0.06, 2)
+    nrm = np.array([1.0, a, b]); nrm /= np.linalg.norm(nrm)
+    eu = np.cross([0.0, 0.0, 1.0], nrm); eu /= np.linalg.norm(eu)
+    ew = np.cross(nrm, eu)
+    nu, nw = int(rng.integers(1, 9)), int(rng.integers(1, 9))
+    cu, cw = rng.uniform(-0.01, 0.05), rng.uniform(0.02, 0.3)
+    edges_u = cu + np.sort(rng.uniform(-0.03, 0.03, 2 * nu)); edges_w = cw + np.sort(rng.uniform(-0.05, 0.05, 2 * nw))
+    det = wl.Detector((float(rng.uniform(0.80, 0.84)), 0.0, 0.0), tuple(nrm), tuple(eu), tuple(ew),
+                      edges_u[0::2].copy(), edges_u[1::2].copy(), edges_w[0::2].copy(), edges_w[1::2].copy())
+    n = int(rng.integers(1, 400))
+    groups = [wl.Group(beam, n, int(rng.integers(0, 2 ** 40)), 0, float(rng.uniform(0, 3e-7)) if kind == 1 else 0.0)]
+    cfg = wl.Config("rand", fb, groups, float(rng.choice([2e-10, 5e-10, 1e-9, 2e-9])), int(rng.integers(1, 3000)),
+                    int(rng.integers(0, 2 ** 62)), 1, det)
+    solver = int(rng.choice([0, 0, 0, 1, 2, 3, 4]))
+    E = tuple(rng.normal(0, 3e4, 3)) if rng.random() < 0.3 else (0.0, 0.0, 0.0)
+    interp = int(rng.random() < 0.3) if (solver <= 1 and not any(E)) else 0
+    return cfg, solver, E, interp
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_random_scenarios_parity(tg, seed):
+    """Randomised end-to-end parity: grids, kinds, species, tilted beams and detector planes,
+    gapped matrices, step sizes, step limits, solvers, E fields, plane interpolation."""
+    from paper_2506_15812_b200 import taiga
+    rng = np.random.default_rng(1000 + seed)
+    cfg, solver, E, interp = _random_scenario(rng)
+    grid, nodal = cfg.field_builder()
+    try:
+        tg.set_efield(E); tg.set_option("plane_interp", interp)
+        ions, counts, summary = taiga.run_config(tg, cfg, rkn_variant=solver)
+        torch.cuda.synchronize()
+    finally:
+        tg.set_efield((0.0, 0.0, 0.0)); tg.set_option("plane_interp", 0)
+    f = orc.OracleField(grid, nodal, E=E)
+    ref = orc.run_config(cfg, field=f, variant=solver, interp=interp)
+    st = compare_groups(ions, ref, "random %d (kind %d solver %d interp %d)" % (seed, grid.kind, solver, interp))
+    check_histogram(cfg, ions, counts, summary, ref)
+    assert st["flagged"] <= max(3, st["n"] // 50)
