@@ -38,6 +38,7 @@ def parse():
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--ions", type=int, default=0, help="override ions per group (debug)")
     ap.add_argument("--oracle-sample", type=int, default=131072)
+    ap.add_argument("--solver", type=int, default=0, help="0 RKN (default, the metric), 1 printed-k3 RKN, 2 RK4, 3/4 Boris")
     ap.add_argument("--opt", action="append", default=[], help="key=value for taiga_set_option")
     return ap.parse_args()
 
@@ -78,14 +79,14 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_run(cfg_index, sample, nthreads=0):
+def oracle_run(cfg_index, sample, nthreads=0, solver=0):
     """The oracle as it stands on a prefix sample; returns (ion_steps, ions, seconds, threads)."""
     sys.path.insert(0, os.path.join(ROOT, "oracle"))
     import oracle as orc
     from paper_2506_15812_b200 import workloads as wl
     cfg = wl.config(cfg_index, n_override=max(sample // len(wl.config(cfg_index).groups), 1))
     t0 = time.perf_counter()
-    res = orc.run_config(cfg, nthreads=nthreads)
+    res = orc.run_config(cfg, nthreads=nthreads, variant=solver)
     dt = time.perf_counter() - t0
     steps = sum(int(g["steps"].astype("int64").sum()) for g in res["groups"])
     return steps, cfg.n_ions, dt, orc.max_threads(), cfg
@@ -96,10 +97,10 @@ def main_reference(args):
     if rank != 0:
         return
     for _ in range(min(args.warmup, 1)):
-        oracle_run(args.config, max(args.oracle_sample // 8, 1024))
+        oracle_run(args.config, max(args.oracle_sample // 8, 1024), solver=args.solver)
     tot_steps, tot_t, n_ions, cores = 0, 0.0, 0, 1
     for _ in range(args.steps):
-        s, n, dt, cores, cfg = oracle_run(args.config, args.oracle_sample)
+        s, n, dt, cores, cfg = oracle_run(args.config, args.oracle_sample, solver=args.solver)
         tot_steps += s; tot_t += dt; n_ions = n
     v = tot_steps / tot_t
     sample = "first %d ions of config %d (prefix sample; identical ions, Philox counter = ion index), whole path a1-a5 per step" % (n_ions, args.config)
@@ -170,10 +171,10 @@ def main_ours(args):
         e0.record()
         if cfg.detector is not None:
             b = cfg.groups[0].beam
-            tg.trace(ions, b.charge_C / b.mass_kg, cfg.dt, cfg.max_steps, cfg.detector)   # a3 + a4
+            tg.trace(ions, b.charge_C / b.mass_kg, cfg.dt, cfg.max_steps, cfg.detector, args.solver)   # a3 + a4
         else:
             for v, g in spans:
-                tg.trace(v, g.beam.charge_C / g.beam.mass_kg, cfg.dt, cfg.max_steps, g.detector)
+                tg.trace(v, g.beam.charge_C / g.beam.mass_kg, cfg.dt, cfg.max_steps, g.detector, args.solver)
         e1.record()
         if cfg.detector is not None:
             tg.detector_histogram(ions, cfg.detector, cfg.n_hist, counts, summary)       # a5
@@ -224,6 +225,9 @@ def main_ours(args):
     t_trace = sum(a.elapsed_time(b) for a, b in trace_ms) / len(trace_ms)
     kind = grid.kind
     alg = ALG_FP64_INSTR_PER_ION_STEP[kind]
+    if args.solver:                             # other solvers: field evaluations per step 4 (solver 1, 2) / 1 (Boris)
+        per_eval = (alg - 69.0) / 3.0
+        alg = {1: 4 * per_eval + 69.0, 2: 4 * per_eval + 75.0, 3: per_eval + 45.0, 4: per_eval + 45.0}[args.solver]
     achieved = ion_steps_rank * alg / (t_trace * 1e-3)
     h2d = sum(p.numel() * 8 for p in nodal_pin) + (len(cd) + len(cn)) * 8 * len(cfg.groups) + 4 * (det0.nu + det0.nw) * 8
     d2h = counts.numel() * 8 + summary.numel() * 8
@@ -233,7 +237,8 @@ def main_ours(args):
         "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "BASELINE config %d (%s): %d ions/GPU, grid %dx%dx%d kind %d, dt=%g, max_steps=%d, whole path a1-a5 per step"
-                               % (args.config, cfg.name, cfg.n_ions, grid.nR, grid.nZ, grid.nS, kind, cfg.dt, cfg.max_steps),
+                               % (args.config, cfg.name, cfg.n_ions, grid.nR, grid.nZ, grid.nS, kind, cfg.dt, cfg.max_steps)
+                               + ("" if not args.solver else ", solver %d" % args.solver),
                    "l2": "256 MiB buffer written between timed iterations (L2 flush)",
                    "ion_steps_per_step": ion_steps, "ions_per_step": n_ions, "invariant_counts_sum_to_n": s_ok},
         "ions_per_s": n_ions * args.steps / (total_ms * 1e-3),
@@ -253,7 +258,7 @@ def main_ours(args):
     }
     if rank == 0:
         if world == 1:
-            s, n, dt, cores, _ = oracle_run(args.config, args.oracle_sample)
+            s, n, dt, cores, _ = oracle_run(args.config, args.oracle_sample, solver=args.solver)
             out["cpu_baseline"] = {"value": s / dt, "unit": "ion-steps/s", "cores": cores, "kind": "oracle",
                                    "ions_per_s": n / dt, "seconds": dt,
                                    "sample": "first %d ions of config %d (prefix sample, identical ions), whole path a1-a5, OpenMP over ions" % (n, args.config)}

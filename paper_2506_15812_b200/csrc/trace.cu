@@ -339,7 +339,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 if (P.variant) {               // printed Eq. 6: k3 position increment from k2
                     Xm = fma(k2x, P.a2, fma(Ux, P.a1, X)); Ym = fma(k2y, P.a2, fma(Uy, P.a1, Y)); Zm = fma(k2z, P.a2, fma(Uz, P.a1, Z));
                     R2 = fma(Xm, Xm, Ym * Ym); rinv = tg_rsqrt(R2); R = R2 * rinv;
-                    tg_fieldCyl<KIND, false>(P, cc, reloads, dummy, Xm, Ym, Zm, tm, R, BR, Bz, Bp, tR, tZ);
+                    tg_fieldCyl<KIND, CACHED>(P, cc, reloads, dummy, Xm, Ym, Zm, tm, R, BR, Bz, Bp, tR, tZ);   // on-demand verify / refill
                     tg_rotate(Xm, Ym, rinv, BR, Bp, Bx, By);
                 }
                 double k3x = fma(uy, Bz, -(uz * By)), k3y = fma(uz, Bx, -(ux * Bz)), k3z = fma(ux, By, -(uy * Bx));
@@ -642,7 +642,9 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     //   3: cache on demand, 3 x 128 (168 regs)
     //   1: no cache, 2 x 128   2: no cache, 4 x 128 (128 regs)   (the only ones for kinds 1, 2)
     int kv = ctx->opt_variant;
-    if (ctx->field.kind == 2 || variant != 0) kv = (kv == 2 || kv == 3) ? 2 : 1;   // (the cached kernels assume k2 and k3 share their position)
+    if (ctx->field.kind == 2) kv = (kv == 2 || kv == 3) ? 2 : 1;
+    else if (variant != 0) kv = (ctx->field.kind == 0 && kv != 1 && kv != 2) ? 5 : ((kv == 2 || kv == 3) ? 2 : 1);   // printed k3: a 4th evaluation between the
+                                              // predicted stages: cache refilled on demand only (kind 0), uncached (kind 1)
     else if (ctx->field.kind == 1 && kv != 0) kv = (kv == 2 || kv == 3) ? 2 : 1;    // kind 1: 0 = slice cache + rolling refill, else uncached
     const int threads = 128;
     int per_sm = ctx->opt_ctas_per_sm > 0 ? ctx->opt_ctas_per_sm : (kv == 2 ? 4 : (kv == 3 ? 3 : 2));
@@ -658,7 +660,7 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         grid = (unsigned)(ctx->sm_count * 2); if (grid > need) grid = need;
         const int kind = ctx->field.kind;
         if (kind == 0 && variant == 0) TG_LAUNCH(0, true, 128, 255, 2, 0, false, false, true);
-        else if (kind == 0) TG_LAUNCH(0, false, 128, 255, 0, 0, false, false, true);
+        else if (kind == 0) TG_LAUNCH(0, true, 128, 255, 0, 0, false, false, true);
         else if (kind == 1) TG_LAUNCH(1, false, 128, 255, 0, 0, false, false, true);
         else TG_LAUNCH(2, false, 128, 255, 0, 0, false, false, true);
     } else if (loss) {                     // RKN + Eq. 2 loss integral: rolling-refill cache (kind 0) / uncached gathers
@@ -669,7 +671,7 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         grid = (unsigned)(ctx->sm_count * 2); if (grid > need) grid = need;
         const int kind = ctx->field.kind;
         if (kind == 0 && variant == 0) TG_LAUNCH(0, true, 128, 255, 2, 0, false, true);
-        else if (kind == 0) TG_LAUNCH(0, false, 128, 255, 0, 0, false, true);
+        else if (kind == 0) TG_LAUNCH(0, true, 128, 255, 0, 0, false, true);
         else if (kind == 1) TG_LAUNCH(1, false, 128, 255, 0, 0, false, true);
         else TG_LAUNCH(2, false, 128, 255, 0, 0, false, true);
     } else if (variant <= 1 && !hasE) {           // the production path: RKN, E = 0
@@ -685,7 +687,7 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         grid = (unsigned)(ctx->sm_count * 2); if (grid > need) grid = need;
         const int S = variant <= 1 ? 0 : (variant == 2 ? 2 : 3);
         const int kind = ctx->field.kind;
-        if (kind == 0 && variant == 1) TG_LAUNCH(0, false, 128, 255, 0, 0, true);
+        if (kind == 0 && variant == 1) TG_LAUNCH(0, true, 128, 255, 0, 0, true);
         else if (kind == 0 && S == 0) TG_LAUNCH(0, true, 128, 255, 2, 0, true);
         else if (kind == 0 && S == 2) TG_LAUNCH(0, true, 128, 255, 0, 2, true);
         else if (kind == 0) TG_LAUNCH(0, true, 128, 255, 0, 3, true);
