@@ -182,8 +182,9 @@ int taiga_detector_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga
  * (ii) the rate profile nu_k = n_e,k sqrt(t) exp(-1/t) / (E12^1.5 (6+t)) 1e-11 [1/s], t = T_e,k/E12
  * (Eq. 2) at psi0 + k dpsi, k < n; nu(psi) is linear in between and held constant outside.
  * While a loss model is loaded and ions->weight is not null, taiga_trace (RKN solvers, E = 0)
- * also writes weight = w0 exp(-integral of nu dt) (w0 = 1 when ions->w0 is null), the integral taken by the trapezoidal rule over
- * the step end points, the crossing step counted up to the plane with nu interpolated linearly
+ * also writes weight = w0 exp(-integral of nu dt) (w0 = 1 when ions->w0 is null), the integral taken
+ * by the trapezoidal rule over the step end points, the crossing step counted up to the plane with nu
+ * interpolated linearly
  * (reading L2); ions that do not cross keep the weight of their completed steps (1 for bad starts).
  * psi_nodal = NULL unloads the model.  ne / Te: host pointers; psi_nodal host or dev. */
 typedef struct {
@@ -197,8 +198,9 @@ int taiga_load_loss(taiga_ctx* ctx, const double* psi_nodal, int psi_on_device,
 
 /* Weighted counters (L350): every plane-crossing ion adds q = floor(weight 2^32 + 1/2) (32.32 fixed
  * point: integer sums, independent of the order of the atomics) to wcounts_dev[n_hist][nw][nu] at
- * its segment (weight = ions->weight if not null, else ions->w0); wsummary_dev[n_hist][4] = {sum q in segments, sum q of crossers outside the
- * segments, sum floor(q^2 / 2^32) over crossers, number of crossers}.  Both are ACCUMULATED into.
+ * its segment (weight = ions->weight if not null, else ions->w0); wsummary_dev[n_hist][4] = {sum q in
+ * segments, sum q of crossers outside the segments, sum floor(q^2 / 2^32) over crossers, number of
+ * crossers}.  Both are ACCUMULATED into.
  * Call after taiga_detector_histogram (uses ions->cell); needs ions->weight or ions->w0. */
 int taiga_detector_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det,
                                       int n_hist, unsigned long long* wcounts_dev,
