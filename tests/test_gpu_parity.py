@@ -785,3 +785,40 @@ def test_random_scenarios_parity(tg, seed):
     st = compare_groups(ions, ref, "random %d (kind %d solver %d interp %d)" % (seed, grid.kind, solver, interp))
     check_histogram(cfg, ions, counts, summary, ref)
     assert st["flagged"] <= max(3, st["n"] // 50)
+
+
+def test_philox_against_curand_device_generator():
+    """Pin P1 on the GPU box: the oracle's Philox4x32-10 against cuRAND's
+    Philox4_32_10 device generator -- a library routine independent of the oracle and of libtaiga --
+    and through it the product's seeding (bit-exact against the oracle in the tests above)."""
+    import ctypes
+    import os
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    lib_path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "cuda", "libphilox_curand.so")
+    assert os.path.exists(lib_path), "run __graft_entry__.build() (tests/cuda/build.py)"
+    lib = ctypes.CDLL(lib_path)
+    rng = np.random.default_rng(99)
+    n = 257
+    sub = rng.integers(0, 2 ** 63, n, dtype=np.uint64); sub[:3] = (0, 1, 2)
+    off = rng.integers(0, 2 ** 60, n, dtype=np.uint64); off[:4] = (0, 1, 2 ** 32 - 1, 2 ** 32)
+    for seed in (0, 1, 0xDEADBEEFCAFEF00D):
+        out = np.zeros((n, 4), dtype=np.uint32)
+        rc = lib.philox_curand_words(ctypes.c_ulonglong(seed), sub.ctypes.data_as(ctypes.c_void_p), off.ctypes.data_as(ctypes.c_void_p),
+                                     ctypes.c_int(n), out.ctypes.data_as(ctypes.c_void_p))
+        assert rc == 0
+        for i in range(n):
+            ctr = (int(off[i]) & 0xFFFFFFFF, int(off[i]) >> 32, int(sub[i]) & 0xFFFFFFFF, int(sub[i]) >> 32)
+            key = (seed & 0xFFFFFFFF, seed >> 32)
+            assert tuple(int(x) for x in out[i]) == tuple(int(x) for x in orc.philox4x32_10(ctr, key)), (seed, i)
+    # the counter layout of the seeding (O2.1): counter = (i lo, i hi, block j, 0) = cuRAND (offset i, subsequence j)
+    i_ion, seed = (1 << 40) + 12345, 7
+    U = orc.uniforms(seed, i_ion)
+    sub3 = np.array([0, 1, 2], dtype=np.uint64); off3 = np.full(3, i_ion, dtype=np.uint64)
+    out = np.zeros((3, 4), dtype=np.uint32)
+    assert lib.philox_curand_words(ctypes.c_ulonglong(seed), sub3.ctypes.data_as(ctypes.c_void_p), off3.ctypes.data_as(ctypes.c_void_p),
+                                   ctypes.c_int(3), out.ctypes.data_as(ctypes.c_void_p)) == 0
+    w = out.reshape(-1)
+    for k in range(5):
+        nk = (int(w[2 * k]) >> 6) * 2 ** 26 + (int(w[2 * k + 1]) >> 6)
+        assert U[k] == (nk + 0.5) * 2.0 ** -52
