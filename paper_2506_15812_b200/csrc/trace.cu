@@ -661,6 +661,7 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         const int kind = ctx->field.kind;
         if (kind == 0 && variant == 0) TG_LAUNCH(0, true, 128, 255, 2, 0, false, false, true);
         else if (kind == 0) TG_LAUNCH(0, true, 128, 255, 0, 0, false, false, true);
+        else if (kind == 1 && variant == 0) TG_LAUNCH(1, true, 128, 255, 2, 0, false, false, true);
         else if (kind == 1) TG_LAUNCH(1, false, 128, 255, 0, 0, false, false, true);
         else TG_LAUNCH(2, false, 128, 255, 0, 0, false, false, true);
     } else if (loss) {                     // RKN + Eq. 2 loss integral: rolling-refill cache (kind 0) / uncached gathers
@@ -672,6 +673,7 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         const int kind = ctx->field.kind;
         if (kind == 0 && variant == 0) TG_LAUNCH(0, true, 128, 255, 2, 0, false, true);
         else if (kind == 0) TG_LAUNCH(0, true, 128, 255, 0, 0, false, true);
+        else if (kind == 1 && variant == 0) TG_LAUNCH(1, true, 128, 255, 2, 0, false, true);
         else if (kind == 1) TG_LAUNCH(1, false, 128, 255, 0, 0, false, true);
         else TG_LAUNCH(2, false, 128, 255, 0, 0, false, true);
     } else if (variant <= 1 && !hasE) {           // the production path: RKN, E = 0
@@ -691,6 +693,7 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         else if (kind == 0 && S == 0) TG_LAUNCH(0, true, 128, 255, 2, 0, true);
         else if (kind == 0 && S == 2) TG_LAUNCH(0, true, 128, 255, 0, 2, true);
         else if (kind == 0) TG_LAUNCH(0, true, 128, 255, 0, 3, true);
+        else if (kind == 1 && variant == 0) TG_LAUNCH(1, true, 128, 255, 2, 0, true);
         else if (kind == 1 && S == 0) TG_LAUNCH(1, false, 128, 255, 0, 0, true);
         else if (kind == 1 && S == 2) TG_LAUNCH(1, false, 128, 255, 0, 2, true);
         else if (kind == 1) TG_LAUNCH(1, false, 128, 255, 0, 3, true);
