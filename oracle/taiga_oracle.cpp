@@ -634,7 +634,10 @@ extern "C" void orc_histogram_weighted(uint64_t n, const int32_t* cell, const do
     for (uint64_t i = 0; i < n; ++i) {
         int g = group ? (int)group[i] : 0;
         if (g >= n_hist || cell[i] < -1) continue;
-        uint64_t q = (uint64_t)std::floor(weight[i] * 4294967296.0 + 0.5);
+        double wv = weight[i];
+        if (!(wv >= 0.0)) wv = 0.0;                           /* negative / NaN weights count as 0 */
+        if (wv > 1048576.0) wv = 1048576.0;
+        uint64_t q = (uint64_t)std::floor(wv * 4294967296.0 + 0.5);
         if (cell[i] >= 0) { wcounts[(size_t)g * ncell + (size_t)cell[i]] += q; wsummary[g * 4 + 0] += q; }
         else wsummary[g * 4 + 1] += q;
         wsummary[g * 4 + 2] += (uint64_t)(((unsigned __int128)q * q) >> 32);

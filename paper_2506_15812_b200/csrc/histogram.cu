@@ -141,7 +141,10 @@ __global__ void k_histogram_weighted(const int32_t* __restrict__ cell, const dou
     if (i >= n) return;
     int g = group ? (int)group[i] : 0, c = cell[i];
     if (g >= n_hist || c < TAIGA_CELL_MISS) return;
-    unsigned long long q = (unsigned long long)floor(fma(weight[i], 4294967296.0, 0.5));
+    double wv = weight[i];
+    if (!(wv >= 0.0)) wv = 0.0;                // negative / NaN weights count as 0
+    if (wv > 1048576.0) wv = 1048576.0;        // keeps q < 2^52 (weights are <= 1 for this method)
+    unsigned long long q = (unsigned long long)floor(fma(wv, 4294967296.0, 0.5));
     if (c >= 0) { atomicAdd(&wcounts[(size_t)g * ncell + c], q); atomicAdd(&wsummary[g * 4 + 0], q); }
     else atomicAdd(&wsummary[g * 4 + 1], q);
     atomicAdd(&wsummary[g * 4 + 2], __umul64hi(q, q) << 32 | (q * q) >> 32);
