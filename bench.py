@@ -27,6 +27,9 @@ ALG_FP64_INSTR_PER_ION_STEP = {0: 252.0, 1: 402.0, 2: 840.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_trace launch on config 2, from the
 # `ncu --set full` capture summarised in profiles/r1d_trace_ncu.md (per launch; None elsewhere)
 NCU_DRAM_BYTES_PER_LAUNCH = {2: 244.5e6}
+# kinds 1 and 2 are bound by the L1 -> register delivery of the gathered coefficients:
+# bytes per ion-step = 3 evaluations x (384: slice difference, kind 1 | 1536: tricubic cell, kind 2; fp32 halves it)
+ALG_L1_BYTES_PER_ION_STEP = {1: 1152.0, 2: 4608.0}
 
 
 def parse():
@@ -256,6 +259,16 @@ def main_ours(args):
                                     "nominal 148 SM x 64 lanes x 1.965 GHz = 18.6e12 instr/s"},
         "clocks": sampler.summary(),
     }
+    if kind != 0 and not args.solver:
+        f32 = any(kv.strip() == "precision=32" for kv in args.opt)
+        l1_peak = tg.l1_gather_peak(50.0, 1)
+        l1_bytes = ALG_L1_BYTES_PER_ION_STEP[kind] * (0.5 if f32 else 1.0)
+        out["roofline"] = {"bound": "l1", "achieved": 1e-9 * ion_steps_rank * l1_bytes / (t_trace * 1e-3), "peak": 1e-9 * l1_peak,
+                           "unit": "GB/s (gathered field coefficients delivered to registers)",
+                           "frac": ion_steps_rank * l1_bytes / (t_trace * 1e-3) / l1_peak, "traffic": None, "kernel": "k_trace",
+                           "alg_l1_bytes_per_ion_step": l1_bytes, "fp64_frac": achieved / peak_dfma,
+                           "peak_source": "measured live: L1-resident 256-bit gather microkernel, all lanes of a warp in one cell "
+                                          "(taiga_measure_l1_gather_peak, spread 1: 128 B/clk/SM; 64 with two cells per warp, 32 with four or more)"}
     if rank == 0:
         if world == 1:
             s, n, dt, cores, _ = oracle_run(args.config, args.oracle_sample, solver=args.solver)

@@ -12,7 +12,7 @@
  *    taiga_load_field synchronises once the first time it sees a new grid line length (it
  *    uploads a host-built band operator); taiga_trace synchronises at its end only while the
  *    "stats" option is on (default; it reads the counters back), taiga_field_table and
- *    taiga_measure_fp64_peak always do.
+ *    taiga_measure_fp64_peak / taiga_measure_l1_gather_peak always do.
  *  - Coordinates: right-handed Cartesian (X,Y,Z), Z vertical, torus axis = Z,
  *    R = sqrt(X^2+Y^2); (R,phi,Z) right-handed; SI units.
  *  - There is no CPU fallback: every entry point needs an sm_100 device.
@@ -219,7 +219,9 @@ int taiga_detector_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, co
  * bit-exact; taiga_trace returns TAIGA_E_ARG for other kinds / solvers), "plane_interp" (0 default:
  * linear interpolation to the detector plane; 1: quadratic Bezier through r_n, r_n+1 with the
  * control point at the mean of r_n + v_n dt/2 and r_n+1 - v_n+1 dt/2, reading Z1;
- * RKN solvers, E = 0, no loss model). */
+ * RKN solvers, E = 0, no loss model), "regroup" (kind-2 fields, plain RKN: the CTA re-sorts its 128
+ * ions over its lanes by field cell every this many steps, so that the lanes of a warp gather from
+ * few distinct cells; default 8, 0 = off: per-warp tiles as for the other kinds). */
 int taiga_set_option(taiga_ctx* ctx, const char* key, long long value);
 /* counters of the last taiga_trace (valid with "stats" on): [0] ion-steps, [1] warp-steps*32
  * (lane slots issued), [2] 1, [3] kernel launches, [4] cell refills, [5..7] 0. */
@@ -227,6 +229,10 @@ int taiga_get_stats(taiga_ctx* ctx, unsigned long long stats_host[8]);
 /* register-resident DFMA microkernel: measured FP64 FMA instructions per second (thread-level,
  * i.e. lanes x instr) over ~`ms` milliseconds; the roofline denominator. */
 int taiga_measure_fp64_peak(taiga_ctx* ctx, double ms, double* dfma_per_s);
+/* L1-resident gather microkernel shaped like the uncached field evaluation (8 warps/SM, 48 x 256-bit
+ * loads of a 1536-B cell per lane): bytes per second delivered to registers; `spread` = distinct cells
+ * read by the lanes of a warp (1 ... 32).  The roofline denominator of the kind-1 / kind-2 kernels. */
+int taiga_measure_l1_gather_peak(taiga_ctx* ctx, double ms, int spread, double* bytes_per_s);
 
 #ifdef __cplusplus
 }

@@ -48,3 +48,59 @@ int tg_fp64_peak(taiga_ctx* ctx, double ms, double* rate) {
     *rate = best;
     return TAIGA_OK;
 }
+
+// ------------------------------------------------------------------------------------------
+// Roofline denominator of the uncached field gathers (kinds 1 and 2): bytes per second that L1-resident
+// 256-bit loads deliver to the registers of a kernel shaped like k_trace's gather (8 warps per SM, every
+// lane reading a whole 1536-B "cell" with 48 x LDG.E.256).  spread = number of distinct cells the lanes
+// of a warp read (1: all lanes the same addresses ... 32: every lane its own cell).
+__global__ void __launch_bounds__(128) k_l1_gather_peak(const double* __restrict__ tab, int ncell, int spread, int iters, double* out) {
+    int lane = threadIdx.x & 31, warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    double acc = 0.0;
+    for (int it = 0; it < iters; ++it) {
+        int cell = (warp * 7 + it * 3 + (lane % spread)) % ncell;
+        const double* c = tab + (size_t)cell * 192;
+#pragma unroll
+        for (int k = 0; k < 48; ++k) {
+            double a, b, d, e;
+            asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(d), "=d"(e) : "l"(c + 4 * k));
+            acc += (a + b) + (d + e);              // three adds per 32 bytes: the loads, not the ALU, are the work
+        }
+    }
+    if (acc == 123.456) out[0] = acc;
+}
+
+int tg_l1_gather_peak(taiga_ctx* ctx, double ms, int spread, double* bytes_per_s) {
+    cudaStream_t st = ctx->stream;
+    const int ncell = 32;                              // 48 KB: L1-resident
+    double* tab = nullptr;
+    TG_CUDA(ctx, cudaMalloc((void**)&tab, (size_t)ncell * 192 * sizeof(double)));
+    cudaMemsetAsync(tab, 0, (size_t)ncell * 192 * sizeof(double), st);
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    double* dummy = (double*)ctx->counters + 12;
+    unsigned grid = (unsigned)ctx->sm_count * 2;       // 2 x 128 threads = 8 warps per SM, as k_trace
+    if (spread < 1) spread = 1;
+    if (spread > 32) spread = 32;
+    int iters = 64;
+    float t = 0.f;
+    double best = 0.0;
+    cudaError_t err = cudaSuccess;
+    for (int rep = 0; rep < 6 && err == cudaSuccess; ++rep) {
+        cudaEventRecord(e0, st);
+        k_l1_gather_peak<<<grid, 128, 0, st>>>(tab, ncell, spread, iters, dummy);
+        cudaEventRecord(e1, st);
+        err = cudaEventSynchronize(e1);
+        if (err != cudaSuccess) break;
+        cudaEventElapsedTime(&t, e0, e1);
+        double n = (double)grid * 128.0 * (double)iters * 1536.0;
+        if (rep >= 2) { double r = n / (t * 1e-3); if (r > best) best = r; }
+        if (rep == 1 && t > 0.f) { double scale = ms / t; iters = (int)(iters * scale) + 1; if (iters > (1 << 22)) iters = 1 << 22; }
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(tab);
+    TG_CUDA(ctx, err);
+    TG_CUDA(ctx, cudaGetLastError());
+    *bytes_per_s = best;
+    return TAIGA_OK;
+}

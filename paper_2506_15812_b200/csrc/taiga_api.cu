@@ -38,7 +38,7 @@ extern "C" int taiga_create(taiga_ctx** out, int device, void* cuda_stream) {
     }
     ctx->opt_sort = 1; ctx->opt_sort_sub = 16;
     ctx->opt_min_active = 32;
-    ctx->opt_ctas_per_sm = 0; ctx->opt_variant = 0; ctx->opt_stats = 1; ctx->opt_precision = 64; ctx->opt_plane_interp = 0;
+    ctx->opt_ctas_per_sm = 0; ctx->opt_variant = 0; ctx->opt_stats = 1; ctx->opt_precision = 64; ctx->opt_plane_interp = 0; ctx->opt_regroup = 8;
     strcpy(ctx->err, "ok");
     *out = ctx;
     return TAIGA_OK;
@@ -219,7 +219,7 @@ extern "C" int taiga_set_option(taiga_ctx* ctx, const char* key, long long v) {
     if (!ctx || !key) return TAIGA_E_ARG;
     struct { const char* k; int* p; } tab[] = {
         {"sort", &ctx->opt_sort}, {"sort_sub", &ctx->opt_sort_sub},
-        {"precision", &ctx->opt_precision}, {"plane_interp", &ctx->opt_plane_interp}, {"min_active", &ctx->opt_min_active},
+        {"precision", &ctx->opt_precision}, {"plane_interp", &ctx->opt_plane_interp}, {"regroup", &ctx->opt_regroup}, {"min_active", &ctx->opt_min_active},
         {"ctas_per_sm", &ctx->opt_ctas_per_sm}, {"variant", &ctx->opt_variant}, {"stats", &ctx->opt_stats}};
     for (auto& t : tab) if (!strcmp(key, t.k)) { *t.p = (int)v; return TAIGA_OK; }
     TG_SET_ERR(ctx, "set_option: unknown key '%s'", key);
@@ -230,6 +230,12 @@ extern "C" int taiga_get_stats(taiga_ctx* ctx, unsigned long long out[8]) {
     if (!ctx || !out) return TAIGA_E_ARG;
     for (int i = 0; i < 8; ++i) out[i] = ctx->stats[i];
     return TAIGA_OK;
+}
+
+extern "C" int taiga_measure_l1_gather_peak(taiga_ctx* ctx, double ms, int spread, double* bytes_per_s) {
+    if (!ctx || !bytes_per_s || !(ms > 0)) return TAIGA_E_ARG;
+    TG_CUDA(ctx, cudaSetDevice(ctx->device));
+    return tg_l1_gather_peak(ctx, ms, spread, bytes_per_s);
 }
 
 extern "C" int taiga_measure_fp64_peak(taiga_ctx* ctx, double ms, double* rate) {

@@ -72,7 +72,7 @@ struct taiga_ctx {
 
     // options
     int opt_sort, opt_min_active, opt_ctas_per_sm, opt_variant, opt_stats;
-    int opt_sort_sub, opt_precision, opt_plane_interp;
+    int opt_sort_sub, opt_precision, opt_plane_interp, opt_regroup;
 };
 
 #define TG_SET_ERR(ctx, ...) snprintf((ctx)->err, sizeof((ctx)->err), __VA_ARGS__)
@@ -113,3 +113,4 @@ int tg_load_loss(taiga_ctx* ctx, const double* psi_nodal, int on_device, const t
 int tg_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
                           unsigned long long* wcounts, unsigned long long* wsummary);
 int tg_fp64_peak(taiga_ctx* ctx, double ms, double* rate);
+int tg_l1_gather_peak(taiga_ctx* ctx, double ms, int spread, double* bytes_per_s);

@@ -36,6 +36,7 @@ struct TraceParams {
     double pa1R, pa1Z;                // a1/hR, a1/hZ: half-step displacement in cells per unit u (predictive refill)
     uint32_t max_steps, n;
     int variant, refill_min;
+    int regroup_every;
     const double *x, *y, *z, *vx, *vy, *vz, *t0;
     const uint32_t* order;
     double *hit_u, *hit_w;
@@ -248,8 +249,12 @@ __device__ __forceinline__ void tg_fieldXYZ(const TraceParams& P, CellCache<KIND
 // Verlet form with leap-frog start, 4 = Eq. 8 as printed).  HAS_E: uniform E of Eq. 3 added to every k.
 // LOSS: integrate Eq. 2 along the trajectory (trapezoid over step end points) and write exp(-integral).
 // BEZ: quadratic Bezier instead of linear interpolation to the plane (reading Z1).
+// REGROUP (uncached kinds): the CTA draws tiles of THREADS ions and, every P.regroup_every steps, re-sorts
+// its ions over the lanes by field cell through shared memory, so that the lanes of a warp gather from as
+// few distinct cells as possible: L1 delivers 128 B/clk/SM when a warp reads one cell, 64 with two, 32 with
+// four or more (taiga_measure_l1_gather_peak).
 template <int KIND, bool CACHED, int THREADS, int MAXREG, int PRED = 0, int SOLVER = 0, bool HAS_E = false, bool LOSS = false,
-          bool BEZ = false>
+          bool BEZ = false, bool REGROUP = false>
 __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const TraceParams P) {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
@@ -265,8 +270,69 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
     unsigned reloads = 0, ion_steps = 0;       // per lane; < 2^32 for any run the queue allows
     unsigned long long warp_steps = 0;
 
+    [[maybe_unused]] int since = 0;            // REGROUP: iterations since the last CTA sync point
     while (true) {
-        unsigned am = __ballot_sync(FULL, alive), freem = ~am;
+      unsigned am;
+      if constexpr (REGROUP) {
+        __shared__ double sh_d[8][THREADS];
+        __shared__ uint32_t sh_u[2][THREADS];
+        __shared__ int sh_key[2][THREADS];
+        __shared__ unsigned long long s_base;
+        const int tid = threadIdx.x;
+        if (since == 0) {                      // every warp of the CTA arrives here at the same iteration count
+            int nalive = __syncthreads_count(alive);
+            if (nalive == 0) {                 // CTA-wide tile of THREADS consecutive queue entries
+                if (exhausted) break;
+                if (tid == 0) s_base = atomicAdd(&P.counters[0], (unsigned long long)THREADS);
+                __syncthreads();
+                unsigned long long q = s_base + tid;
+                if (s_base + THREADS >= P.n) exhausted = true;
+                if (q < P.n) {
+                    idx = P.order ? P.order[q] : (uint32_t)q;
+                    X = P.x[idx]; Y = P.y[idx]; Z = P.z[idx];
+                    Ux = P.qm * P.vx[idx]; Uy = P.qm * P.vy[idx]; Uz = P.qm * P.vz[idx];
+                    t = P.t0 ? P.t0[idx] : 0.0;
+                    nst = 0;
+                    s0 = fma(P.det.normal[0], X, fma(P.det.normal[1], Y, fma(P.det.normal[2], Z, -P.nrD)));
+                    alive = true;
+                    if (!(s0 < 0.0)) {
+                        P.hit_u[idx] = 0.0; P.hit_w[idx] = 0.0; P.cell[idx] = TAIGA_CELL_BADSTART; P.steps[idx] = 0;
+                        P.flags[idx] = (fabs(s0) < TG_GRAZE) ? TAIGA_FLAG_PLANE : 0;
+                        alive = false;
+                    }
+                }
+            } else {                           // re-sort the CTA's ions over its lanes by field cell
+                int key = 0x7fffffff;
+                if (alive) {
+                    double p_, w_;
+                    int i = tg_locate(sqrt(fma(X, X, Y * Y)), P.f.inv_hR, P.f.offR, P.f.cR, p_);
+                    int j = tg_locate(Z, P.f.inv_hZ, P.f.offZ, P.f.cZ, w_);
+                    int k = 0;
+                    if constexpr (KIND == 2) {
+                        double xs = (atan2(Y, X) - P.f.s0) * P.f.inv_ds;
+                        xs -= (double)P.f.nS * floor(xs / (double)P.f.nS);
+                        k = tg_clampi(__double2int_rd(xs), 0, P.f.nS - 1);
+                    }
+                    key = (k * P.f.cR + i) * P.f.cZ + j;
+                }
+                sh_key[0][tid] = key;
+                __syncthreads();
+                int rank = 0;
+#pragma unroll 8
+                for (int o = 0; o < THREADS; ++o) { int ko = sh_key[0][o]; rank += (ko < key) | ((ko == key) & (o < tid)); }
+                sh_d[0][rank] = X; sh_d[1][rank] = Y; sh_d[2][rank] = Z; sh_d[3][rank] = Ux; sh_d[4][rank] = Uy; sh_d[5][rank] = Uz;
+                sh_d[6][rank] = t; sh_d[7][rank] = s0; sh_u[0][rank] = idx; sh_u[1][rank] = nst; sh_key[1][rank] = key;
+                __syncthreads();
+                X = sh_d[0][tid]; Y = sh_d[1][tid]; Z = sh_d[2][tid]; Ux = sh_d[3][tid]; Uy = sh_d[4][tid]; Uz = sh_d[5][tid];
+                t = sh_d[6][tid]; s0 = sh_d[7][tid]; idx = sh_u[0][tid]; nst = sh_u[1][tid]; alive = sh_key[1][tid] != 0x7fffffff;
+            }
+        }
+        since = (since + 1 >= P.regroup_every) ? 0 : since + 1;
+        am = __ballot_sync(FULL, alive);
+        if (am == 0) continue;                 // this warp idles until the next sync point
+      } else {
+        am = __ballot_sync(FULL, alive);
+        unsigned freem = ~am;
         int nfree = __popc(freem);
         if (nfree >= P.refill_min && !exhausted) {
             unsigned long long base = 0;
@@ -293,6 +359,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
             am = __ballot_sync(FULL, alive);
         }
         if (am == 0) { if (exhausted) break; else continue; }
+      }
         ++warp_steps;
         if (alive) {
             // ---- stage 1 at (r, u); its grid test is the out-of-grid test of the previous step (O4)
@@ -623,6 +690,7 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     for (int c = 0; c < 3; ++c) { P.qE[c] = qm * ctx->E[c]; P.eh[c] = qm * qm * ctx->E[c] * dt * 0.5; hasE |= ctx->E[c] != 0.0; }
     P.pa1R = P.a1 * ctx->field.inv_hR; P.pa1Z = P.a1 * ctx->field.inv_hZ;
     P.max_steps = max_steps; P.n = (uint32_t)ions->n; P.variant = variant;
+    P.regroup_every = ctx->opt_regroup > 0 ? ctx->opt_regroup : 0;
     P.refill_min = ctx->opt_min_active > 0 ? (ctx->opt_min_active > 32 ? 32 : ctx->opt_min_active) : 1;
     P.x = ions->x; P.y = ions->y; P.z = ions->z; P.vx = ions->vx; P.vy = ions->vy; P.vz = ions->vz; P.t0 = ions->t0;
     P.hit_u = ions->hit_u; P.hit_w = ions->hit_w; P.cell = ions->cell; P.steps = ions->steps; P.flags = ions->flags;
@@ -683,7 +751,9 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         else if (kv == 2) TG_LAUNCH(0, false, 128, 128); else TG_LAUNCH(0, false, 128, 255);
         break;
     case 1: if (kv == 2) TG_LAUNCH(1, false, 128, 128); else if (kv == 1) TG_LAUNCH(1, false, 128, 255); else TG_LAUNCH(1, true, 128, 255, 2); break;
-    default: if (kv == 2) TG_LAUNCH(2, false, 128, 128); else TG_LAUNCH(2, false, 128, 255); break;
+    default: if (kv == 2) TG_LAUNCH(2, false, 128, 128);
+             else if (P.regroup_every > 0 && ions->n >= 128) TG_LAUNCH(2, false, 128, 255, 0, 0, false, false, false, true);
+             else TG_LAUNCH(2, false, 128, 255); break;
     }
     } else {                               // other solvers (Eq. 4, Eq. 7-8: on-demand cache) and / or a uniform E (RKN: rolling refill), 8 warps/SM
         grid = (unsigned)(ctx->sm_count * 2); if (grid > need) grid = need;

@@ -30,7 +30,7 @@ EXPORTS = ["taiga_create", "taiga_destroy", "taiga_last_error", "taiga_load_fiel
            "taiga_detector_histogram_weighted", "taiga_seed_beam_grid",
            "taiga_field_eval", "taiga_field_table", "taiga_seed_beam", "taiga_trace",
            "taiga_detector_histogram", "taiga_set_efield", "taiga_set_option", "taiga_get_stats",
-           "taiga_measure_fp64_peak"]
+           "taiga_measure_fp64_peak", "taiga_measure_l1_gather_peak"]
 
 
 class GridS(C.Structure):
@@ -93,6 +93,7 @@ _lib.taiga_set_efield.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
 _lib.taiga_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_longlong]
 _lib.taiga_get_stats.argtypes = [C.c_void_p, C.POINTER(C.c_ulonglong * 8)]
 _lib.taiga_measure_fp64_peak.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
+_lib.taiga_measure_l1_gather_peak.argtypes = [C.c_void_p, C.c_double, C.c_int, C.POINTER(C.c_double)]
 
 
 class TaigaError(RuntimeError):
@@ -283,6 +284,11 @@ class Taiga:
         out = (C.c_ulonglong * 8)()
         self._chk(_lib.taiga_get_stats(self.h, C.byref(out)))
         return dict(ion_steps=out[0], lane_slots=out[1], passes=out[2], launches=out[3], reloads=out[4])
+
+    def l1_gather_peak(self, ms=50.0, spread=1):
+        r = C.c_double()
+        self._chk(_lib.taiga_measure_l1_gather_peak(self.h, ms, int(spread), C.byref(r)))
+        return r.value
 
     def fp64_peak(self, ms=50.0):
         r = C.c_double()
