@@ -102,6 +102,7 @@ static inline int tg_reserve(taiga_ctx* ctx, T** p, size_t* cap, size_t need) {
 int tg_precompute(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c);
 int tg_seed(taiga_ctx* ctx, const taiga_beam_params* p, uint64_t seed, taiga_ions* ions, double v0,
             const taiga_seed_grid* grid /* null: stochastic */);
+int tg_build_order(taiga_ctx* ctx, const taiga_ions* ions);      // queue_sort.cu: fills ctx->order
 int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t max_steps,
              const DetDev& det, int variant);
 int tg_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
