@@ -822,3 +822,47 @@ def test_philox_against_curand_device_generator():
     for k in range(5):
         nk = (int(w[2 * k]) >> 6) * 2 ** 26 + (int(w[2 * k + 1]) >> 6)
         assert U[k] == (nk + 0.5) * 2.0 ** -52
+
+
+def test_loss_table_shape_energy_and_species(tg):
+    """The form of PAPER.md Table 1 (L147-158) through the product path, on the synthetic profiles:
+    percent-level mean loss with a spread over the ionisation depth that is a fraction of the mean, and
+    Na+ losing several times more than Li+ (E12 = 47.3 eV against 75.6 eV; the paper: ~20 % against
+    ~4.7 %).  The paper's own percentages and their fall with beam energy need the COMPASS profiles and the
+    per-energy RENATE-OD ionisation profiles (parity unpinned); with ONE depth profile for all energies the
+    faster ions reach hotter, denser plasma and lose more."""
+    from paper_2506_15812_b200 import taiga
+    cfg = wl.config(1)
+    grid, nodal = cfg.field_builder()
+    psi0, dpsi, ne, te = wl.loss_profile_inputs()
+    psi_nodal = wl.nodal_psi(grid)
+    cd, cn = wl.depth_cdf(), wl.normal_cdf()
+    tg.load_field(grid, nodal)
+    n = 8192
+    table = {}
+    try:
+        for species, mass, e12 in (("li", wl.MASS_LI7, wl.E12_LI), ("na", wl.MASS_NA23, wl.E12_NA)):
+            tg.load_loss(psi_nodal, psi0, dpsi, ne, te, e12)
+            for energy in (40e3, 60e3, 80e3):
+                beam = wl.Beam(mass, wl.E_CHARGE, energy)
+                beam.depth_max, beam.z_max = wl.DEPTH_MAX, wl.NORMAL_ZMAX
+                ions = taiga.Ions(n)
+                counts = torch.zeros((1, 8, 8), dtype=torch.int64, device="cuda"); summary = torch.zeros((1, 6), dtype=torch.int64, device="cuda")
+                wc = torch.zeros((1, 8, 8), dtype=torch.int64, device="cuda"); ws = torch.zeros((1, 4), dtype=torch.int64, device="cuda")
+                tg.seed_beam(beam, cd, cn, 11, ions)
+                tg.trace(ions, wl.E_CHARGE / mass, cfg.dt, 20000, cfg.detector)
+                tg.detector_histogram(ions, cfg.detector, 1, counts, summary)
+                tg.detector_histogram_weighted(ions, cfg.detector, 1, wc, ws)
+                torch.cuda.synchronize()
+                mean, std = taiga.loss_statistics(ws)
+                assert int(ws[0, 3]) > n // 3                                  # enough plane crossers
+                table[species, energy] = (float(mean[0]), float(std[0]))
+    finally:
+        tg.load_loss(None)
+    for species in ("li", "na"):
+        m = [table[species, e][0] for e in (40e3, 60e3, 80e3)]
+        assert all(1e-3 < x < 0.3 for x in m), (species, m)
+        for e in (40e3, 60e3, 80e3):
+            assert 0.02 * table[species, e][0] < table[species, e][1] < table[species, e][0]
+    for e in (40e3, 60e3, 80e3):
+        assert 2.0 < table["na", e][0] / table["li", e][0] < 12.0, table
