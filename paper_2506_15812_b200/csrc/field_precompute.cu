@@ -189,6 +189,20 @@ __global__ void k_slice_diff(const double* __restrict__ T, double* __restrict__ 
     D[t] = a[48] - a[0];
 }
 
+// kind 1, register-cached kernel only (trace.cu): the slice differences, built on first use
+int tg_build_dtable(taiga_ctx* ctx) {
+    FieldDev& f = ctx->field;
+    if (ctx->dtable_valid) { f.dtable = ctx->dtable; return TAIGA_OK; }
+    const long long ncell = (long long)f.cR * f.cZ;
+    size_t nd = (size_t)ncell * (f.nS - 1) * 48;
+    int rc = tg_reserve(ctx, &ctx->dtable, &ctx->cap_dtable, nd);
+    if (rc) return rc;
+    k_slice_diff<<<(unsigned)((nd + 255) / 256), 256, 0, ctx->stream>>>(ctx->table, ctx->dtable, ncell, f.nS);
+    TG_CUDA(ctx, cudaGetLastError());
+    f.dtable = ctx->dtable; ctx->dtable_valid = true;
+    return TAIGA_OK;
+}
+
 int tg_precompute(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c) {
     const int nR = g->nR, nZ = g->nZ, nS = g->nS, cR = nR - 1, cZ = nZ - 1;
     const long long ncell = (long long)cR * cZ, nnode = (long long)nS * nR * nZ;
@@ -268,14 +282,6 @@ int tg_precompute(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c) {
     f.offR = g->Rmin / hR; f.offZ = g->Zmin / hZ;
     f.s0 = g->s0; f.inv_ds = (g->kind == 0) ? 0.0 : 1.0 / g->ds;
     f.table = ctx->table; f.table32 = nullptr; f.dtable = nullptr;
-    if (g->kind == 1) {
-        size_t nd = (size_t)ncell * (nS - 1) * 48;
-        int rc2 = tg_reserve(ctx, &ctx->dtable, &ctx->cap_dtable, nd);
-        if (rc2) return rc2;
-        k_slice_diff<<<(unsigned)((nd + 255) / 256), 256, 0, st>>>(ctx->table, ctx->dtable, ncell, nS);
-        TG_CUDA(ctx, cudaGetLastError());
-        f.dtable = ctx->dtable;
-    }
     return TAIGA_OK;
 }
 

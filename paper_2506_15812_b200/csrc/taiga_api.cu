@@ -34,11 +34,13 @@ extern "C" int taiga_create(taiga_ctx** out, int device, void* cuda_stream) {
     ctx->sm_count = prop.multiProcessorCount;
     if (cudaMalloc((void**)&ctx->counters, 16 * sizeof(unsigned long long)) != cudaSuccess ||
         cudaMallocHost((void**)&ctx->counters_host, 16 * sizeof(unsigned long long)) != cudaSuccess) {
+        if (ctx->counters) cudaFree(ctx->counters);
         delete ctx; return TAIGA_E_NOMEM;
     }
     ctx->opt_sort = 1; ctx->opt_sort_sub = 16;
     ctx->opt_min_active = 32;
     ctx->opt_ctas_per_sm = 0; ctx->opt_variant = 0; ctx->opt_stats = 1; ctx->opt_precision = 64; ctx->opt_plane_interp = 0; ctx->opt_regroup = 8;
+    ctx->opt_mma = 1; ctx->opt_refill_cta = 0;
     strcpy(ctx->err, "ok");
     *out = ctx;
     return TAIGA_OK;
@@ -49,7 +51,7 @@ extern "C" int taiga_destroy(taiga_ctx* ctx) {
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     void* bufs[] = {ctx->table, ctx->scratch, ctx->band[0], ctx->band[1], ctx->cdf_depth, ctx->cdf_normal, ctx->edges, ctx->order,
-                    ctx->bins, ctx->counters, ctx->table32, ctx->psi_table, ctx->loss_rate, ctx->dtable};
+                    ctx->bins, ctx->counters, ctx->table32, ctx->psi_table, ctx->loss_rate, ctx->dtable, ctx->frag};
     for (void* b : bufs) if (b) cudaFree(b);
     if (ctx->counters_host) cudaFreeHost(ctx->counters_host);
     delete ctx;
@@ -68,7 +70,7 @@ extern "C" int taiga_load_field(taiga_ctx* ctx, const taiga_grid* g, const taiga
         return TAIGA_E_ARG;
     }
     TG_CUDA(ctx, cudaSetDevice(ctx->device));
-    ctx->field_loaded = false; ctx->table32_valid = false; ctx->loss.psi = nullptr;   // a new grid invalidates psi
+    ctx->field_loaded = false; ctx->table32_valid = false; ctx->frag_valid = false; ctx->dtable_valid = false; ctx->loss.psi = nullptr;   // a new grid invalidates psi
     int rc = tg_precompute(ctx, g, c);
     if (rc == TAIGA_OK) ctx->field_loaded = true;
     return rc;
@@ -217,11 +219,20 @@ extern "C" int taiga_detector_histogram(taiga_ctx* ctx, const taiga_ions* ions, 
 
 extern "C" int taiga_set_option(taiga_ctx* ctx, const char* key, long long v) {
     if (!ctx || !key) return TAIGA_E_ARG;
-    struct { const char* k; int* p; } tab[] = {
-        {"sort", &ctx->opt_sort}, {"sort_sub", &ctx->opt_sort_sub},
-        {"precision", &ctx->opt_precision}, {"plane_interp", &ctx->opt_plane_interp}, {"regroup", &ctx->opt_regroup}, {"min_active", &ctx->opt_min_active},
-        {"ctas_per_sm", &ctx->opt_ctas_per_sm}, {"variant", &ctx->opt_variant}, {"stats", &ctx->opt_stats}};
-    for (auto& t : tab) if (!strcmp(key, t.k)) { *t.p = (int)v; return TAIGA_OK; }
+    struct { const char* k; int* p; long long lo, hi; } tab[] = {
+        {"sort", &ctx->opt_sort, 0, 1}, {"sort_sub", &ctx->opt_sort_sub, 1, 64},
+        {"precision", &ctx->opt_precision, 32, 64}, {"plane_interp", &ctx->opt_plane_interp, 0, 1},
+        {"regroup", &ctx->opt_regroup, 0, 1 << 20}, {"min_active", &ctx->opt_min_active, 0, 32},
+        {"ctas_per_sm", &ctx->opt_ctas_per_sm, 0, 32}, {"variant", &ctx->opt_variant, 0, 5}, {"stats", &ctx->opt_stats, 0, 1},
+        {"mma", &ctx->opt_mma, 0, 1}, {"refill_cta", &ctx->opt_refill_cta, 0, 1024}};
+    for (auto& t : tab) if (!strcmp(key, t.k)) {
+        if (v < t.lo || v > t.hi || (t.p == &ctx->opt_precision && v != 32 && v != 64)) {
+            TG_SET_ERR(ctx, "set_option: %s = %lld out of range [%lld, %lld]", key, v, t.lo, t.hi);
+            return TAIGA_E_ARG;
+        }
+        *t.p = (int)v;
+        return TAIGA_OK;
+    }
     TG_SET_ERR(ctx, "set_option: unknown key '%s'", key);
     return TAIGA_E_ARG;
 }

@@ -46,7 +46,8 @@ struct taiga_ctx {
     FieldDev field;
     double* table;            size_t table_bytes;
     double* scratch;          size_t scratch_bytes;     // precompute work arrays
-    double* dtable;           size_t cap_dtable;
+    double* dtable;           size_t cap_dtable;   bool dtable_valid;    // kind 1: slice differences (built on first use)
+    double* frag;             size_t cap_frag;     bool frag_valid;      // kinds 1, 2: table in DMMA B-fragment order (trace_mma.cu)
     float* table32;           size_t cap_table32;  bool table32_valid;   // fp32 copy of a kind-2 table
     double* band[2];          size_t band_cap[2]; int band_n[2];   // y -> y'' band operators (Z, R)
 
@@ -73,6 +74,8 @@ struct taiga_ctx {
     // options
     int opt_sort, opt_min_active, opt_ctas_per_sm, opt_variant, opt_stats;
     int opt_sort_sub, opt_precision, opt_plane_interp, opt_regroup;
+    int opt_mma, opt_refill_cta;
+    bool weight_written;                                 // the last taiga_trace wrote ions->weight (loss model)
 };
 
 #define TG_SET_ERR(ctx, ...) snprintf((ctx)->err, sizeof((ctx)->err), __VA_ARGS__)
@@ -105,6 +108,10 @@ int tg_seed(taiga_ctx* ctx, const taiga_beam_params* p, uint64_t seed, taiga_ion
 int tg_build_order(taiga_ctx* ctx, const taiga_ions* ions);      // queue_sort.cu: fills ctx->order
 int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t max_steps,
              const DetDev& det, int variant);
+struct TraceParams;
+int tg_trace_mma(taiga_ctx* ctx, TraceParams& P, int solver, bool hasE, bool loss, bool bez, uint64_t n);   // trace_mma.cu
+bool tg_mma_supported(const taiga_ctx* ctx);
+int tg_build_dtable(taiga_ctx* ctx);                             // field_precompute.cu
 int tg_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
                  unsigned long long* counts, unsigned long long* summary);
 int tg_field_eval(taiga_ctx* ctx, uint64_t n, const double* R, const double* Z, const double* s,

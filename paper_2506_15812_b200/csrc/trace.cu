@@ -19,45 +19,7 @@
 //    registers and re-read (24 x 128-bit loads, one 128-B line per component) only when the
 //    lane leaves the cell (~0.35 times per step);
 //  * 1/R by MUFU.RSQ64H seed + one cubic (Halley) step: 6 FP64 instructions instead of ~30.
-#include "field_device.cuh"
-
-struct TraceParams {
-    FieldDev f;
-    DetDev det;
-    LossDev loss;                     // secondary-ionisation loss model (LOSS kernels)
-    double hdt;                       // dt/2
-    double* weight;
-    const double* w0;                 // initial statistical weight (null = 1)
-    double nrD;                       // normal . origin
-    double a1, a2, b1;                // dt/(2 qm), dt^2/8, qm dt/2   (stage 2/3)
-    double c6, d6, dtq;               // dt^2/6, qm dt/6, dt/qm
-    double qm, dt;
-    double qE[3], eh[3];              // (q/m) E [m/s^2];  (q/m)^2 E dt/2 (Boris half kick in u units)
-    double pa1R, pa1Z;                // a1/hR, a1/hZ: half-step displacement in cells per unit u (predictive refill)
-    uint32_t max_steps, n;
-    int variant, refill_min;
-    int regroup_every;
-    const double *x, *y, *z, *vx, *vy, *vz, *t0;
-    const uint32_t* order;
-    double *hit_u, *hit_w;
-    int32_t* cell;
-    uint32_t* steps;
-    uint8_t* flags;
-    unsigned long long* counters;     // [0] queue head, [1] warp-steps, [2] reloads, [3] ion-steps
-};
-
-#define TG_GRAZE 1e-9
-
-__device__ __forceinline__ double tg_rsqrt(double a) {
-    double y;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
-    double e = fma(-(a * y), y, 1.0);          // 1 - a y^2, |e| <~ 2^-22
-    double q = fma(0.375, e, 0.5);
-    return fma(y * e, q, y);                   // y (1 + e/2 + 3 e^2/8): cubic convergence
-}
-
-// t in [0,1)  <=>  sign 0 and exponent < 1023  <=>  (unsigned) hi word < 0x3FF00000
-__device__ __forceinline__ bool tg_in01(double t) { return (unsigned)__double2hiint(t) < 0x3FF00000u; }
+#include "trace_common.cuh"
 
 template <int KIND>
 struct CellCache;                              // register cache of the current cell (kind 0)
@@ -211,28 +173,6 @@ __device__ __forceinline__ void tg_predict(const TraceParams& P, CellCache<0>& c
     asm volatile("" ::"d"(BR), "d"(BZ), "d"(Bp));      // the stage's Horner sums are complete: the old coefficients are dead
     if (!(tg_in01(tRp) && tg_in01(tZp)))
         tg_refill(P, cc, reloads, tRp + (cc.oR - P.f.offR), tZp + (cc.oZ - P.f.offZ));
-}
-
-// O0: B_X = B_R c - B_phi s, B_Y = B_R s + B_phi c
-__device__ __forceinline__ void tg_rotate(double X, double Y, double rinv, double BR, double Bp, double& Bx, double& By) {
-    double c = X * rinv, s_ = Y * rinv;
-    Bx = fma(BR, c, -(Bp * s_));
-    By = fma(BR, s_, Bp * c);
-}
-
-// nu(psi(R,Z)): psi from its bicubic table (boundary cell extrapolates), the rate
-// profile linear in psi between its points, held constant outside.
-__device__ __forceinline__ double tg_loss_rate(const TraceParams& P, double R, double Z) {
-    double p, w;
-    int i = tg_locate(R, P.f.inv_hR, P.f.offR, P.f.cR, p);
-    int j = tg_locate(Z, P.f.inv_hZ, P.f.offZ, P.f.cZ, w);
-    double psi = tg_bicubic(P.loss.psi + ((size_t)i * P.f.cZ + j) * 48, p, w);
-    double x = (psi - P.loss.psi0) * P.loss.inv_dpsi;
-    if (!(x > 0.0)) return __ldg(P.loss.rate);
-    if (x >= (double)(P.loss.n - 1)) return __ldg(P.loss.rate + P.loss.n - 1);
-    int k = __double2int_rd(x);
-    double r0 = __ldg(P.loss.rate + k), r1 = __ldg(P.loss.rate + k + 1);
-    return fma(x - (double)k, r1 - r0, r0);
 }
 
 // Cartesian B at a stage point (on-demand cache refill / uncached gather); solvers other than RKN
@@ -528,17 +468,58 @@ __global__ void k_table_to_f32(const double* __restrict__ src, float* __restrict
     for (; i < n; i += stride) dst[i] = (float)src[i];
 }
 
+// Every instantiation of k_trace, one line each: {kind, cached, registers, PRED, SOLVER, HAS_E, LOSS, BEZ, REGROUP}.
+//   kind 0, RKN: register cell cache with rolling predictive refill (PRED 2; 2 x 128 threads/SM, 254 registers),
+//   predictive refill after each Horner (1), refill on demand (0; the 4-evaluation solvers), 168 registers, no cache;
+//   kinds 1 / 2 (option mma = 0, or precision = 32): slice cache / per-lane gathers of trace.cu; the default for these
+//   kinds is the warp-cooperative kernel of trace_mma.cu.
+struct TgVariant { int kind, cached, regs, pred, solver, hasE, loss, bez, regroup; void (*fn)(const TraceParams); };
+#define TG_V(K, C, R, P, S, E, L, B, G) {K, C, R, P, S, E, L, B, G, k_trace<K, (C) != 0, 128, R, P, S, (E) != 0, (L) != 0, (B) != 0, (G) != 0>}
+static const TgVariant tg_variants[] = {
+    // production path: RKN, E = 0
+    TG_V(0, 1, 255, 2, 0, 0, 0, 0, 0), TG_V(0, 1, 255, 1, 0, 0, 0, 0, 0), TG_V(0, 1, 255, 0, 0, 0, 0, 0, 0), TG_V(0, 1, 168, 0, 0, 0, 0, 0, 0),
+    TG_V(0, 0, 128, 0, 0, 0, 0, 0, 0), TG_V(0, 0, 255, 0, 0, 0, 0, 0, 0),
+    TG_V(1, 1, 255, 2, 0, 0, 0, 0, 0), TG_V(1, 0, 255, 0, 0, 0, 0, 0, 0), TG_V(1, 0, 128, 0, 0, 0, 0, 0, 0),
+    TG_V(2, 0, 255, 0, 0, 0, 0, 0, 1), TG_V(2, 0, 255, 0, 0, 0, 0, 0, 0), TG_V(2, 0, 128, 0, 0, 0, 0, 0, 0),
+    // quadratic Bezier plane interpolation
+    TG_V(0, 1, 255, 2, 0, 0, 0, 1, 0), TG_V(0, 1, 255, 0, 0, 0, 0, 1, 0), TG_V(1, 1, 255, 2, 0, 0, 0, 1, 0), TG_V(1, 0, 255, 0, 0, 0, 0, 1, 0),
+    TG_V(2, 0, 255, 0, 0, 0, 0, 1, 0),
+    // Eq. 2 loss integral
+    TG_V(0, 1, 255, 2, 0, 0, 1, 0, 0), TG_V(0, 1, 255, 0, 0, 0, 1, 0, 0), TG_V(1, 1, 255, 2, 0, 0, 1, 0, 0), TG_V(1, 0, 255, 0, 0, 0, 1, 0, 0),
+    TG_V(2, 0, 255, 0, 0, 0, 1, 0, 0),
+    // uniform E and / or the other solvers (Eq. 4, Eq. 7-8)
+    TG_V(0, 1, 255, 2, 0, 1, 0, 0, 0), TG_V(0, 1, 255, 0, 0, 1, 0, 0, 0), TG_V(0, 1, 255, 0, 2, 1, 0, 0, 0), TG_V(0, 1, 255, 0, 3, 1, 0, 0, 0),
+    TG_V(1, 1, 255, 2, 0, 1, 0, 0, 0), TG_V(1, 0, 255, 0, 0, 1, 0, 0, 0), TG_V(1, 0, 255, 0, 2, 1, 0, 0, 0), TG_V(1, 0, 255, 0, 3, 1, 0, 0, 0),
+    TG_V(2, 0, 255, 0, 0, 1, 0, 0, 0), TG_V(2, 0, 255, 0, 2, 1, 0, 0, 0), TG_V(2, 0, 255, 0, 3, 1, 0, 0, 0),
+};
+#undef TG_V
+
 int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t max_steps, const DetDev& det, int variant) {
     cudaStream_t st = ctx->stream;
+    const int kind = ctx->field.kind;
+    const bool loss = ctx->loss.psi != nullptr && ions->weight != nullptr;
+    const bool bez = ctx->opt_plane_interp == 1;
+    const bool f32 = ctx->opt_precision == 32;
+    bool hasE = false;
+    for (int c = 0; c < 3; ++c) hasE |= ctx->E[c] != 0.0;
+    // ---- what is offered (checked before anything is enqueued)
+    if (f32 && (kind != 2 || variant > 1)) {
+        TG_SET_ERR(ctx, "precision=32 is offered for kind-2 (R,Z,phi) fields with the RKN solver only");
+        return TAIGA_E_ARG;
+    }
+    if (bez && (variant > 1 || hasE || loss || f32)) {
+        TG_SET_ERR(ctx, "plane_interp=1 (Bezier) is offered with the RKN solvers, E = 0, no loss model, fp64");
+        return TAIGA_E_ARG;
+    }
+    if (loss && (variant > 1 || hasE || f32)) {
+        TG_SET_ERR(ctx, "the loss model is offered with the RKN solvers, E = 0, fp64");
+        return TAIGA_E_ARG;
+    }
     TraceParams P;
     P.f = ctx->field; P.det = det;
     P.loss = ctx->loss; P.hdt = 0.5 * dt; P.weight = ions->weight; P.w0 = ions->w0;
-    const bool loss = ctx->loss.psi != nullptr && ions->weight != nullptr;
-    if (ctx->opt_precision == 32) {            // fp32 field evaluation (BASELINE config 5 "fp32 variant")
-        if (ctx->field.kind != 2 || variant > 1) {
-            TG_SET_ERR(ctx, "precision=32 is offered for kind-2 (R,Z,phi) fields with the RKN solver only");
-            return TAIGA_E_ARG;
-        }
+    P.frag = nullptr; P.key_shift = 0; P.refill_cta = 0;
+    if (f32) {                                 // fp32 field evaluation (BASELINE config 5 "fp32 variant")
         if (!ctx->table32_valid) {
             size_t n = (size_t)ctx->field.nS * ctx->field.cR * ctx->field.cZ * 192;
             int rc = tg_reserve(ctx, &ctx->table32, &ctx->cap_table32, n);
@@ -548,16 +529,12 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
             ctx->table32_valid = true;
         }
         P.f.table32 = ctx->table32;
-    } else if (ctx->opt_precision != 64) {
-        TG_SET_ERR(ctx, "option precision must be 64 or 32");
-        return TAIGA_E_ARG;
     }
     P.nrD = det.normal[0] * det.origin[0] + det.normal[1] * det.origin[1] + det.normal[2] * det.origin[2];
     P.qm = qm; P.dt = dt;
     P.a1 = dt / (2.0 * qm); P.a2 = dt * dt / 8.0; P.b1 = qm * dt / 2.0;
     P.c6 = dt * dt / 6.0; P.d6 = qm * dt / 6.0; P.dtq = dt / qm;
-    bool hasE = false;
-    for (int c = 0; c < 3; ++c) { P.qE[c] = qm * ctx->E[c]; P.eh[c] = qm * qm * ctx->E[c] * dt * 0.5; hasE |= ctx->E[c] != 0.0; }
+    for (int c = 0; c < 3; ++c) { P.qE[c] = qm * ctx->E[c]; P.eh[c] = qm * qm * ctx->E[c] * dt * 0.5; }
     P.pa1R = P.a1 * ctx->field.inv_hR; P.pa1Z = P.a1 * ctx->field.inv_hZ;
     P.max_steps = max_steps; P.n = (uint32_t)ions->n; P.variant = variant;
     P.regroup_every = ctx->opt_regroup > 0 ? ctx->opt_regroup : 0;
@@ -574,76 +551,51 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         launches += 5;
     }
     TG_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, 8 * sizeof(unsigned long long), st));
-    // kernel variants (option "variant"), kind 0 with the classical RKN:
-    //   0: register cell cache + rolling predictive refill, 2 x 128 threads/SM (254 regs)
-    //   4: cache + predictive refill after each Horner   5: cache, refill on demand only (r1c kernel)
-    //   3: cache on demand, 3 x 128 (168 regs)
-    //   1: no cache, 2 x 128   2: no cache, 4 x 128 (128 regs)   (the only ones for kinds 1, 2)
-    int kv = ctx->opt_variant;
-    if (ctx->field.kind == 2) kv = (kv == 2 || kv == 3) ? 2 : 1;
-    else if (variant != 0) kv = (ctx->field.kind == 0 && kv != 1 && kv != 2) ? 5 : ((kv == 2 || kv == 3) ? 2 : 1);   // printed k3: a 4th evaluation between the
-                                              // predicted stages: cache refilled on demand only (kind 0), uncached (kind 1)
-    else if (ctx->field.kind == 1 && kv != 0) kv = (kv == 2 || kv == 3) ? 2 : 1;    // kind 1: 0 = slice cache + rolling refill, else uncached
-    const int threads = 128;
-    int per_sm = ctx->opt_ctas_per_sm > 0 ? ctx->opt_ctas_per_sm : (kv == 2 ? 4 : (kv == 3 ? 3 : 2));
-    unsigned grid = (unsigned)(ctx->sm_count * per_sm);
-    unsigned need = (unsigned)((ions->n + threads - 1) / threads);
-    if (grid > need) grid = need;
-#define TG_LAUNCH(K, C, T, B, ...) k_trace<K, C, T, B, ##__VA_ARGS__><<<grid, T, 0, st>>>(P)
-    if (ctx->opt_plane_interp == 1) {      // quadratic Bezier interpolation to the plane
-        if (variant > 1 || hasE || loss || ctx->opt_precision == 32) {
-            TG_SET_ERR(ctx, "plane_interp=1 (Bezier) is offered with the RKN solvers, E = 0, no loss model, fp64");
-            return TAIGA_E_ARG;
+    const int S = variant <= 1 ? 0 : (variant == 2 ? 2 : 3);
+    if (kind >= 1 && ctx->opt_mma && !f32 && tg_mma_supported(ctx)) {
+        // kinds 1, 2: warp-cooperative evaluation on the FP64 tensor pipe (trace_mma.cu), every solver and option
+        int rc = tg_trace_mma(ctx, P, S, hasE || S != 0, loss, bez, ions->n);
+        if (rc) return rc;
+    } else {
+        // option "variant", kind 0 with the classical RKN: 0 rolling predictive refill (default), 4 predictive refill after
+        // each Horner, 5 refill on demand, 3 on demand at 168 registers, 1 no cache, 2 no cache at 128 registers
+        const int kv = ctx->opt_variant;
+        const bool special = bez || loss || hasE || S != 0;       // these run at 2 CTAs/SM on the full-register kernels
+        TgVariant k = {kind, 0, 255, 0, S, (hasE || S != 0) ? 1 : 0, loss ? 1 : 0, bez ? 1 : 0, 0, nullptr};
+        if (kind == 0) {
+            if (special) { k.cached = 1; k.pred = (variant == 0) ? 2 : 0; }
+            else if (variant != 0) { k.cached = (kv != 1 && kv != 2); k.regs = (kv == 2) ? 128 : 255; }     // printed k3: 4th evaluation, on demand
+            else switch (kv) {
+                case 0: k.cached = 1; k.pred = 2; break;
+                case 4: k.cached = 1; k.pred = 1; break;
+                case 5: k.cached = 1; break;
+                case 3: k.cached = 1; k.regs = 168; break;
+                case 2: k.regs = 128; break;
+                default: break;
+            }
+        } else if (kind == 1) {
+            if (variant == 0 && (special || kv == 0)) { k.cached = 1; k.pred = 2; }   // slice cache + rolling refill
+            else if (!special && (kv == 2 || kv == 3)) k.regs = 128;
+        } else {
+            if (!special && (kv == 2 || kv == 3)) k.regs = 128;
+            else if (!special && P.regroup_every > 0 && ions->n >= 128) k.regroup = 1;
         }
-        grid = (unsigned)(ctx->sm_count * 2); if (grid > need) grid = need;
-        const int kind = ctx->field.kind;
-        if (kind == 0 && variant == 0) TG_LAUNCH(0, true, 128, 255, 2, 0, false, false, true);
-        else if (kind == 0) TG_LAUNCH(0, true, 128, 255, 0, 0, false, false, true);
-        else if (kind == 1 && variant == 0) TG_LAUNCH(1, true, 128, 255, 2, 0, false, false, true);
-        else if (kind == 1) TG_LAUNCH(1, false, 128, 255, 0, 0, false, false, true);
-        else TG_LAUNCH(2, false, 128, 255, 0, 0, false, false, true);
-    } else if (loss) {                     // RKN + Eq. 2 loss integral: rolling-refill cache (kind 0) / uncached gathers
-        if (variant > 1 || hasE || ctx->opt_precision == 32) {
-            TG_SET_ERR(ctx, "the loss model is offered with the RKN solvers, E = 0, fp64");
-            return TAIGA_E_ARG;
-        }
-        grid = (unsigned)(ctx->sm_count * 2); if (grid > need) grid = need;
-        const int kind = ctx->field.kind;
-        if (kind == 0 && variant == 0) TG_LAUNCH(0, true, 128, 255, 2, 0, false, true);
-        else if (kind == 0) TG_LAUNCH(0, true, 128, 255, 0, 0, false, true);
-        else if (kind == 1 && variant == 0) TG_LAUNCH(1, true, 128, 255, 2, 0, false, true);
-        else if (kind == 1) TG_LAUNCH(1, false, 128, 255, 0, 0, false, true);
-        else TG_LAUNCH(2, false, 128, 255, 0, 0, false, true);
-    } else if (variant <= 1 && !hasE) {           // the production path: RKN, E = 0
-    switch (ctx->field.kind) {
-    case 0:
-        if (kv == 0) TG_LAUNCH(0, true, 128, 255, 2); else if (kv == 4) TG_LAUNCH(0, true, 128, 255, 1); else if (kv == 5) TG_LAUNCH(0, true, 128, 255); else if (kv == 3) TG_LAUNCH(0, true, 128, 168);
-        else if (kv == 2) TG_LAUNCH(0, false, 128, 128); else TG_LAUNCH(0, false, 128, 255);
-        break;
-    case 1: if (kv == 2) TG_LAUNCH(1, false, 128, 128); else if (kv == 1) TG_LAUNCH(1, false, 128, 255); else TG_LAUNCH(1, true, 128, 255, 2); break;
-    default: if (kv == 2) TG_LAUNCH(2, false, 128, 128);
-             else if (P.regroup_every > 0 && ions->n >= 128) TG_LAUNCH(2, false, 128, 255, 0, 0, false, false, false, true);
-             else TG_LAUNCH(2, false, 128, 255); break;
+        if (kind == 1 && k.cached) { int rc = tg_build_dtable(ctx); if (rc) return rc; P.f.dtable = ctx->dtable; }
+        const TgVariant* sel = nullptr;
+        for (const TgVariant& v : tg_variants)
+            if (v.kind == k.kind && v.cached == k.cached && v.regs == k.regs && v.pred == k.pred && v.solver == k.solver &&
+                v.hasE == k.hasE && v.loss == k.loss && v.bez == k.bez && v.regroup == k.regroup) { sel = &v; break; }
+        if (!sel) { TG_SET_ERR(ctx, "trace: no kernel for kind %d solver %d with these options", kind, variant); return TAIGA_E_ARG; }
+        const int threads = 128;
+        int per_sm = ctx->opt_ctas_per_sm > 0 ? ctx->opt_ctas_per_sm : (k.regs == 128 ? 4 : (k.regs == 168 ? 3 : 2));
+        unsigned grid = (unsigned)(ctx->sm_count * per_sm);
+        unsigned need = (unsigned)((ions->n + threads - 1) / threads);
+        if (grid > need) grid = need;
+        sel->fn<<<grid, threads, 0, st>>>(P);
     }
-    } else {                               // other solvers (Eq. 4, Eq. 7-8: on-demand cache) and / or a uniform E (RKN: rolling refill), 8 warps/SM
-        grid = (unsigned)(ctx->sm_count * 2); if (grid > need) grid = need;
-        const int S = variant <= 1 ? 0 : (variant == 2 ? 2 : 3);
-        const int kind = ctx->field.kind;
-        if (kind == 0 && variant == 1) TG_LAUNCH(0, true, 128, 255, 0, 0, true);
-        else if (kind == 0 && S == 0) TG_LAUNCH(0, true, 128, 255, 2, 0, true);
-        else if (kind == 0 && S == 2) TG_LAUNCH(0, true, 128, 255, 0, 2, true);
-        else if (kind == 0) TG_LAUNCH(0, true, 128, 255, 0, 3, true);
-        else if (kind == 1 && variant == 0) TG_LAUNCH(1, true, 128, 255, 2, 0, true);
-        else if (kind == 1 && S == 0) TG_LAUNCH(1, false, 128, 255, 0, 0, true);
-        else if (kind == 1 && S == 2) TG_LAUNCH(1, false, 128, 255, 0, 2, true);
-        else if (kind == 1) TG_LAUNCH(1, false, 128, 255, 0, 3, true);
-        else if (S == 0) TG_LAUNCH(2, false, 128, 255, 0, 0, true);
-        else if (S == 2) TG_LAUNCH(2, false, 128, 255, 0, 2, true);
-        else TG_LAUNCH(2, false, 128, 255, 0, 3, true);
-    }
-#undef TG_LAUNCH
     ++launches;
     TG_CUDA(ctx, cudaGetLastError());
+    ctx->weight_written = loss;
     if (ctx->opt_stats) {
         TG_CUDA(ctx, cudaMemcpyAsync(ctx->counters_host, ctx->counters, 8 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
         TG_CUDA(ctx, cudaStreamSynchronize(st));

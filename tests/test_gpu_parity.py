@@ -17,8 +17,10 @@ from paper_2506_15812_b200 import workloads as wl  # noqa: E402
 TOL_UW = 1e-9
 
 
-@pytest.fixture(scope="module")
+@pytest.fixture
 def tg():
+    """A fresh context per test: every test starts from the library defaults (the launch configuration
+    bench.py times); options a test sets never leak into the next one."""
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     from paper_2506_15812_b200 import taiga
@@ -85,12 +87,12 @@ def check_histogram(cfg, ions, counts, summary, ref):
         assert s[h, :5].sum() == n_h                       # O5 invariant
 
 
-@pytest.mark.parametrize("opts", [dict(), dict(sort=0), dict(variant=1), dict(min_active=1), dict(min_active=32)])
+@pytest.mark.parametrize("opts", [dict(), dict(sort=0), dict(variant=1), dict(min_active=1), dict(min_active=12), dict(variant=4), dict(variant=5)])
 def test_cfg1_full_parity(tg, opts):
+    """dict() = the library defaults (sort=1, variant=0, min_active=32: whole-tile refill), the others are the
+    alternative launch options of taiga_set_option."""
     from paper_2506_15812_b200 import taiga
     cfg = wl.config(1)
-    for k, v in dict(sort=1, variant=0, min_active=12).items():
-        tg.set_option(k, v)
     for k, v in opts.items():
         tg.set_option(k, v)
     ions, counts, summary = taiga.run_config(tg, cfg)
@@ -99,8 +101,6 @@ def test_cfg1_full_parity(tg, opts):
     st = compare_groups(ions, ref, "cfg1 %s" % opts)
     check_histogram(cfg, ions, counts, summary, ref)
     assert st["flagged"] < 20
-    for k, v in dict(sort=1, variant=0, min_active=12).items():
-        tg.set_option(k, v)
 
 
 def test_cfg1_printed_k3_variant(tg):
@@ -132,6 +132,25 @@ def test_prefix_parity(tg, icfg, n):
     ngpu = int(_np(ions.steps).astype(np.int64).sum())
     assert tg.stats()["launches"] >= 1
     assert ngpu > 0
+
+
+@pytest.mark.parametrize("icfg,n", [(2, None), (3, 65536 + 21), (4, 2048 + 3), (5, 65536 + 77)])
+def test_full_histogram_parity(tg, icfg, n):
+    """The method's output is the counters.  COMPLETE detector histograms + summary, bit for bit
+    (ions flagged as grazing by either side removed from both), and cell / steps / (u, w) of EVERY ion, in the launch
+    configuration bench.py times (library defaults): config 2 in full (1,048,576 ions), configs 3 / 4 / 5 on prefixes
+    of 65,557 ions per energy, 2,051 per time slice (131,264 ions over all 64 slices) and 65,613 ions: multi-tile
+    queues, ragged tails, the CTA refill / re-sort of the cooperative kernel all active."""
+    from paper_2506_15812_b200 import taiga
+    cfg = wl.config(icfg, n_override=n)
+    ions, counts, summary = taiga.run_config(tg, cfg)
+    torch.cuda.synchronize()
+    assert tg.stats()["ion_steps"] == int(ions.steps.to(torch.int64).sum().item())
+    ref = orc.run_config(cfg)
+    st = compare_groups(ions, ref, cfg.name + " full histogram")
+    check_histogram(cfg, ions, counts, summary, ref)
+    assert st["flagged"] <= max(8, st["n"] // 2000), st
+    assert np.array_equal(_np(summary)[:, :5].sum(axis=1), [sum(g.n_ions for g in cfg.groups if g.group == h) for h in range(cfg.n_hist)])
 
 
 def test_seeding_bit_exact_large_indices_and_divergence(tg):
@@ -665,10 +684,11 @@ def test_error_paths_of_the_widened_entry_points(tg):
     with pytest.raises(taiga.TaigaError):
         t2.trace(ions, qm, cfg.dt, 100, cfg.detector, 2)                            # Bezier + RK4
     t2.set_option("plane_interp", 0)
-    t2.set_option("precision", 16)
-    with pytest.raises(taiga.TaigaError):
-        t2.trace(ions, qm, cfg.dt, 100, cfg.detector)
-    t2.set_option("precision", 64)
+    for key, bad in (("precision", 16), ("ctas_per_sm", 1 << 20), ("variant", 99), ("regroup", -1), ("no_such_option", 1)):
+        with pytest.raises(taiga.TaigaError) as e:                                 # options are validated when set
+            t2.set_option(key, bad)
+        assert e.value.code == taiga.E_ARG
+    t2.trace(ions, qm, cfg.dt, 100, cfg.detector)                                   # and a rejected value changes nothing
     # a new field invalidates the loss model (psi lives on the old grid)
     t2.load_loss(wl.nodal_psi(grid), psi0, dpsi, ne, te, wl.E12_LI)
     t2.load_field(grid, nodal)
