@@ -2,7 +2,10 @@
 """bench.py -- whole hot path (a1 field precompute -> a2 seeding -> a3/a4 RKN trace -> a5
 histogram) of BASELINE.json config 2 (1,048,576 7Li+ ions, 257x513 grid) on N GPUs of one node.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2] [--scaling weak|strong]
+
+With --gpus N > 1 and no torchrun environment (WORLD_SIZE unset) it re-executes itself under
+`python -m torch.distributed.run --standalone --nproc-per-node N`, one rank per GPU (rank r on cuda:r).
 
 Prints ONE JSON line (rank 0).  `value` = ion-steps/s with inputs resident in HBM; `e2e` = the
 same through the C ABI with HOST buffers (pinned nodal field H2D + counter D2H inside the timed
@@ -24,9 +27,10 @@ sys.path.insert(0, ROOT)
 # FP64-pipe instructions per ion-step of the classical RKN step on a 2-D bicubic field
 # (3 field evaluations x 61 + 4 cross products x 6 + stage/Eq.5/plane 45).
 ALG_FP64_INSTR_PER_ION_STEP = {0: 252.0, 1: 402.0, 2: 840.0}
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_trace launch on config 2, from the
-# `ncu --set full` capture summarised in profiles/r1d_trace_ncu.md (per launch; None elsewhere)
-NCU_DRAM_BYTES_PER_LAUNCH = {2: 244.5e6}
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel at the FULL size of the config, from
+# the latest `ncu --set full` capture of that kernel (not measured by this run): {config: (bytes, capture)}
+NCU_DRAM_BYTES_PER_LAUNCH = {2: (244.5e6, "profiles/r1d_trace_ncu.md")}
+NOMINAL_FP64_INSTR_PER_S = 148 * 64 * 1.965e9      # B200: 148 SMs x 64 FP64 lanes x 1965 MHz
 # kinds 1 and 2 are bound by the L1 -> register delivery of the gathered coefficients:
 # bytes per ion-step = 3 evaluations x (384: slice difference, kind 1 | 1536: tricubic cell, kind 2; fp32 halves it)
 ALG_L1_BYTES_PER_ION_STEP = {1: 1152.0, 2: 4608.0}
@@ -43,7 +47,24 @@ def parse():
     ap.add_argument("--oracle-sample", type=int, default=131072)
     ap.add_argument("--solver", type=int, default=0, help="0 RKN (default, the metric), 1 printed-k3 RKN, 2 RK4, 3/4 Boris")
     ap.add_argument("--opt", action="append", default=[], help="key=value for taiga_set_option")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = every rank traces the config's ions (default), strong = the config's ions are split")
+    ap.add_argument("--oracle-full", action="store_true", help="time the oracle ONCE on the full config (16 threads and 1 thread on a prefix) and exit")
+    ap.add_argument("--dry-run-ranks", action="store_true", help="stop after the rank / shard set-up (CPU test of the launch path)")
     return ap.parse_args()
+
+
+def spawn_command(argv, n):
+    """The command that runs this script as n ranks of one node (what the driver runs for N > 1)."""
+    return [sys.executable, "-m", "torch.distributed.run", "--standalone", "--nnodes=1", "--nproc-per-node", str(n),
+            "--local-addr", "127.0.0.1", os.path.abspath(__file__)] + list(argv)
+
+
+def maybe_spawn(args):
+    """--gpus N > 1 without a torchrun environment: become the launcher of N ranks."""
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        env = dict(os.environ, MASTER_ADDR="127.0.0.1")
+        sys.exit(subprocess.run(spawn_command(sys.argv[1:], args.gpus), env=env).returncode)
 
 
 class ClockSampler(threading.Thread):
@@ -83,16 +104,26 @@ class ClockSampler(threading.Thread):
 
 
 def oracle_run(cfg_index, sample, nthreads=0, solver=0):
-    """The oracle as it stands on a prefix sample; returns (ion_steps, ions, seconds, threads)."""
+    """The oracle as it stands on a prefix sample (sample = 0: the full config); returns (ion_steps, ions, seconds, threads, cfg)."""
     sys.path.insert(0, os.path.join(ROOT, "oracle"))
     import oracle as orc
     from paper_2506_15812_b200 import workloads as wl
-    cfg = wl.config(cfg_index, n_override=max(sample // len(wl.config(cfg_index).groups), 1))
+    cfg = wl.config(cfg_index, n_override=max(sample // len(wl.config(cfg_index).groups), 1) if sample else None)
     t0 = time.perf_counter()
     res = orc.run_config(cfg, nthreads=nthreads, variant=solver)
     dt = time.perf_counter() - t0
     steps = sum(int(g["steps"].astype("int64").sum()) for g in res["groups"])
-    return steps, cfg.n_ions, dt, orc.max_threads(), cfg
+    return steps, cfg.n_ions, dt, (nthreads or orc.max_threads()), cfg
+
+
+def main_oracle_full(args):
+    """the oracle timed once on the FULL config on all host threads, and on one thread on a
+    prefix (numbers kept in profiles/; not part of the per-run bench line)."""
+    s, n, dt, cores, cfg = oracle_run(args.config, 0, solver=args.solver)
+    s1, n1, dt1, _, _ = oracle_run(args.config, min(args.oracle_sample, 16384), nthreads=1, solver=args.solver)
+    print(json.dumps({"oracle_full": {"config": args.config, "ions": n, "ion_steps": s, "seconds": dt, "cores": cores,
+                                      "ion_steps_per_s": s / dt, "ions_per_s": n / dt,
+                                      "one_thread": {"ions": n1, "seconds": dt1, "ion_steps_per_s": s1 / dt1}}}))
 
 
 def main_reference(args):
@@ -129,15 +160,34 @@ def main_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
+    from paper_2506_15812_b200 import sharding, workloads as wl
+    # weak scaling (default): every rank traces its own cfg.n_ions ions (disjoint Philox counters);
+    # strong: the config's ions are split into `world` contiguous index ranges
+    cfg = sharding.shard_config(wl.config(args.config, n_override=args.ions or None), rank, world, args.scaling)
     dist = None
+    if args.dry_run_ranks:                      # launch / shard logic only: gloo, no CUDA, no library
+        import torch.distributed as dist
+        if world > 1:
+            dist.init_process_group("gloo")
+        mine = torch.tensor([rank, local, cfg.groups[0].first_index, cfg.n_ions], dtype=torch.int64)
+        allr = [torch.zeros_like(mine) for _ in range(world)]
+        if world > 1:
+            dist.all_gather(allr, mine)
+        else:
+            allr = [mine]
+        if rank == 0:
+            print(json.dumps({"n_gpus": world, "scaling": args.scaling, "dry_run": True,
+                              "ranks": [dict(rank=int(a[0]), device="cuda:%d" % int(a[1]), first_index=int(a[2]), n_ions=int(a[3])) for a in allr]}))
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    torch.cuda.set_device(local)
     if world > 1:
         import torch.distributed as dist
+        os.environ.setdefault("NCCL_DEBUG", "WARN")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    from paper_2506_15812_b200 import sharding, taiga, workloads as wl
+    from paper_2506_15812_b200 import taiga
     dev = "cuda:%d" % local
-    # weak scaling: every rank traces its own cfg.n_ions ions (disjoint Philox counters)
-    cfg = sharding.shard_config(wl.config(args.config, n_override=args.ions or None), rank, world, "weak")
     grid, nodal = cfg.field_builder()
     nodal_dev = [torch.from_numpy(np.ascontiguousarray(c)).to(dev) for c in nodal]
     nodal_pin = [torch.from_numpy(np.ascontiguousarray(c)).pin_memory() for c in nodal]
@@ -146,6 +196,8 @@ def main_ours(args):
         k, v = kv.split("=")
         tg.set_option(k, int(v))
     peak_dfma = tg.fp64_peak(100.0)             # FP64-pipe instructions / s, measured live
+    mma_on = grid.kind == 2 and not any(kv.strip() in ("mma=0", "precision=32") for kv in args.opt) or any(kv.strip() == "mma=1" for kv in args.opt)
+    mma_on = mma_on and grid.kind != 0
     tg.set_option("stats", 0)                   # no host sync inside taiga_trace while timing
     ions = taiga.Ions(cfg.n_ions, dev)
     det0 = cfg.detector or cfg.groups[0].detector
@@ -232,13 +284,15 @@ def main_ours(args):
         per_eval = (alg - 69.0) / 3.0
         alg = {1: 4 * per_eval + 69.0, 2: 4 * per_eval + 75.0, 3: per_eval + 45.0, 4: per_eval + 45.0}[args.solver]
     achieved = ion_steps_rank * alg / (t_trace * 1e-3)
+    tr = NCU_DRAM_BYTES_PER_LAUNCH.get(args.config) if not (args.ions or args.solver or args.opt or world > 1 and args.scaling == "strong") else None
+    traffic = (tr[0], "per launch, from the ncu --set full capture in %s (not measured by this run)" % tr[1]) if tr else (None, None)
     h2d = sum(p.numel() * 8 for p in nodal_pin) + (len(cd) + len(cn)) * 8 * len(cfg.groups) + 4 * (det0.nu + det0.nw) * 8
     d2h = counts.numel() * 8 + summary.numel() * 8
     s_ok = int(summary[:, :5].sum().item()) == n_ions
     out = {
         "metric": "ion-steps/s", "value": ion_steps * args.steps / (total_ms * 1e-3), "unit": "ion-steps/s",
         "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "BASELINE config %d (%s): %d ions/GPU, grid %dx%dx%d kind %d, dt=%g, max_steps=%d, whole path a1-a5 per step"
                                % (args.config, cfg.name, cfg.n_ions, grid.nR, grid.nZ, grid.nS, kind, cfg.dt, cfg.max_steps)
                                + ("" if not args.solver else ", solver %d" % args.solver),
@@ -253,13 +307,19 @@ def main_ours(args):
         "roofline": {"bound": "alu", "achieved": 2e-12 * achieved, "peak": 2e-12 * peak_dfma,
                      "unit": "TFLOP/s (FP64 pipe; every FP64 instruction counted as one FMA = 2 flop)",
                      "frac": achieved / peak_dfma,
-                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.config) if not args.ions else None,
-                     "kernel": "k_trace", "alg_fp64_instr_per_ion_step": alg,
-                     "peak_source": "measured live: register-resident DFMA microkernel (taiga_measure_fp64_peak); "
-                                    "nominal 148 SM x 64 lanes x 1.965 GHz = 18.6e12 instr/s"},
+                     "peak_nominal": 2e-12 * NOMINAL_FP64_INSTR_PER_S, "frac_nominal": achieved / NOMINAL_FP64_INSTR_PER_S,
+                     "traffic": traffic[0], "traffic_source": traffic[1],
+                     "kernel": "k_trace_mma" if mma_on else "k_trace", "alg_fp64_instr_per_ion_step": alg,
+                     "alg": "analytic count of the method's FP64 instructions per ion-step (DESIGN.md section 6), not an executed count",
+                     "peak_source": "measured live: register-resident DFMA microkernel, 4 chains with their own operand registers "
+                                    "(taiga_measure_fp64_peak); nominal 148 SM x 64 lanes x 1.965 GHz = 18.6e12 instr/s"},
         "clocks": sampler.summary(),
     }
-    if kind != 0 and not args.solver:
+    if mma_on:
+        out["roofline"]["dmma_peak"] = 2e-12 * tg.dmma_peak(50.0)
+        out["roofline"]["note"] = ("field evaluation on the FP64 tensor pipe (DMMA.8x8x4, same FMA rate as DFMA on B200: dmma_peak); "
+                                   "frac counts the method's %d FP64 instructions per ion-step, not the padded tensor work" % int(alg))
+    if kind != 0 and not args.solver and not mma_on:
         f32 = any(kv.strip() == "precision=32" for kv in args.opt)
         l1_peak = tg.l1_gather_peak(50.0, 1)
         l1_bytes = ALG_L1_BYTES_PER_ION_STEP[kind] * (0.5 if f32 else 1.0)
@@ -272,9 +332,13 @@ def main_ours(args):
     if rank == 0:
         if world == 1:
             s, n, dt, cores, _ = oracle_run(args.config, args.oracle_sample, solver=args.solver)
+            s1, n1, dt1, _, _ = oracle_run(args.config, max(args.oracle_sample // 16, 256), nthreads=1, solver=args.solver)
             out["cpu_baseline"] = {"value": s / dt, "unit": "ion-steps/s", "cores": cores, "kind": "oracle",
-                                   "ions_per_s": n / dt, "seconds": dt,
-                                   "sample": "first %d ions of config %d (prefix sample, identical ions), whole path a1-a5, OpenMP over ions" % (n, args.config)}
+                                   "ions_per_s": n / dt, "seconds": dt, "value_1thread": s1 / dt1, "seconds_1thread": dt1,
+                                   "note": "the oracle is the correctness reference as it stands (-O2, no contraction, 4 field evaluations per step), "
+                                           "not a tuned CPU code: the GPU/CPU ratio is not a speed-up claim",
+                                   "sample": "first %d ions of config %d (prefix sample, identical ions), whole path a1-a5, OpenMP over ions; "
+                                             "value_1thread on the first %d ions" % (n, args.config, n1)}
         print(json.dumps(out))
     tg.close()
     if world > 1:
@@ -283,7 +347,10 @@ def main_ours(args):
 
 if __name__ == "__main__":
     a = parse()
-    if a.impl == "reference":
+    if a.oracle_full:
+        main_oracle_full(a)
+    elif a.impl == "reference":
         main_reference(a)
     else:
+        maybe_spawn(a)
         main_ours(a)

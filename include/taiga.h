@@ -12,7 +12,7 @@
  *    taiga_load_field synchronises once the first time it sees a new grid line length (it
  *    uploads a host-built band operator); taiga_trace synchronises at its end only while the
  *    "stats" option is on (default; it reads the counters back), taiga_field_table and
- *    taiga_measure_fp64_peak / taiga_measure_l1_gather_peak always do.
+ *    taiga_measure_fp64_peak / taiga_measure_dmma_peak / taiga_measure_l1_gather_peak always do.
  *  - Coordinates: right-handed Cartesian (X,Y,Z), Z vertical, torus axis = Z,
  *    R = sqrt(X^2+Y^2); (R,phi,Z) right-handed; SI units.
  *  - There is no CPU fallback: every entry point needs an sm_100 device.
@@ -108,7 +108,15 @@ typedef struct {
  *   depth d along `axis` from cdf_depth; cross-section offsets sigma_pos*(z1 eT + z2 eZ) and
  *   divergence angles sigma_ang*(z3, z4) from cdf_normal (table on [-z_max, z_max]);
  *   speed v0 = sqrt(2 energy_eV e / m) with e = charge_C.
- * CDF tables: host pointers, K+1 entries, F[0]=0, F[K]=1, non-decreasing. */
+ * profile = TAIGA_PROFILE_DISC ("a ... beam with a 5 mm diameter"): the cross-section
+ *   offset is radius_m (a eT + c eZ) with (a, c) uniform over the unit disc, by rejection from the square:
+ *   try 0 = (2 U_1 - 1, 2 U_2 - 1), try k >= 1 = two fresh uniforms from counter (i lo, i hi, 2 + k, 0),
+ *   accepted when a^2 + c^2 <= 1 (64 tries at most, then the axis); depth and divergence as above.
+ * CDF tables: host pointers, K+1 entries, F[0]=0, F[K]=1, non-decreasing; read during the call, the copy to the
+ * device is enqueued on the context's stream from a context-owned staging buffer, so the caller may free or
+ * change them as soon as the call returns. */
+#define TAIGA_PROFILE_GAUSSIAN 0
+#define TAIGA_PROFILE_DISC 1
 typedef struct {
     double mass_kg, charge_C, energy_eV;
     double origin[3], axis[3], eT[3], eZ[3];       /* orthonormal (axis, eT, eZ)              */
@@ -117,6 +125,8 @@ typedef struct {
     double sigma_pos_m, sigma_ang_rad;
     uint64_t first_index;
     uint16_t group; double t0;                     /* written to ions->group / ions->t0       */
+    int profile;                                   /* TAIGA_PROFILE_*                         */
+    double radius_m;                               /* disc radius (TAIGA_PROFILE_DISC), > 0   */
 } taiga_beam_params;
 
 int taiga_seed_beam(taiga_ctx* ctx, const taiga_beam_params* params, uint64_t seed,
@@ -200,11 +210,22 @@ int taiga_load_loss(taiga_ctx* ctx, const double* psi_nodal, int psi_on_device,
  * point: integer sums, independent of the order of the atomics) to wcounts_dev[n_hist][nw][nu] at
  * its segment (weight = ions->weight if not null, else ions->w0); wsummary_dev[n_hist][4] = {sum q in
  * segments, sum q of crossers outside the segments, sum floor(q^2 / 2^32) over crossers, number of
- * crossers}.  Both are ACCUMULATED into.
- * Call after taiga_detector_histogram (uses ions->cell); needs ions->weight or ions->w0. */
+ * crossers}.  Both are ACCUMULATED into.  Weights outside [0, 2^20] (reading L3': weights are probability masses
+ * or counts) are clamped: negative and NaN count as 0, larger ones as 2^20; ions whose group is >= n_hist are
+ * skipped (as in taiga_detector_histogram).
+ * Call after taiga_detector_histogram (uses ions->cell); needs ions->weight or ions->w0.  A non-null
+ * ions->weight must have been written by the last taiga_trace of this context (a loss model loaded), else
+ * TAIGA_E_STATE: pass weight = NULL to count w0 only. */
 int taiga_detector_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det,
                                       int n_hist, unsigned long long* wcounts_dev,
                                       unsigned long long* wsummary_dev);
+
+/* Mean and spread of the secondary-ionisation loss 1 - weight/w0... over the plane-crossing ions of one histogram,
+ * the form of PAPER.md Table 1 (L147-158), from its four fixed-point sums wsummary_host[4] (HOST memory, read
+ * back by the caller): mean weight mu = (s0 + s1) / 2^32 / N, variance s2 / 2^32 / N - mu^2 (>= 0), N = s3
+ * (the division by N the paper does on the CPU, L350).  out_host[0] = 1 - mu, out_host[1] = sqrt(variance),
+ * out_host[2] = N.  No device work. */
+int taiga_loss_statistics(const unsigned long long wsummary_host[4], double out_host[3]);
 
 /* ---- tuning / measurement hooks (not part of the method) */
 /* integer options: "sort" (1: order the ion queue by birth cell before tracing, default 1),
@@ -219,9 +240,12 @@ int taiga_detector_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, co
  * bit-exact; taiga_trace returns TAIGA_E_ARG for other kinds / solvers), "plane_interp" (0 default:
  * linear interpolation to the detector plane; 1: quadratic Bezier through r_n, r_n+1 with the
  * control point at the mean of r_n + v_n dt/2 and r_n+1 - v_n+1 dt/2, reading Z1;
- * RKN solvers, E = 0, no loss model), "regroup" (kind-2 fields, plain RKN: the CTA re-sorts its 128
- * ions over its lanes by field cell every this many steps, so that the lanes of a warp gather from
- * few distinct cells; default 8, 0 = off: per-warp tiles as for the other kinds). */
+ * RKN solvers, E = 0, no loss model), "mma" (kinds 1 and 2, fp64: 1 = warp-cooperative evaluation on the FP64
+ * tensor pipe (trace_mma.cu; default for kind 2), 0 = one lane evaluates its own ion (trace.cu; default for kind 1),
+ * -1 = the default of the kind), "regroup" (kinds 1 / 2: the CTA re-sorts its 128 ions over its lanes by field cell
+ * every this many steps, so that the lanes of a warp / of an 8-ion group share cells; default 8; with mma = 0, 0 = off:
+ * per-warp tiles), "refill_cta" (mma: the CTA refills its finished lanes from the queue at a re-sort point once this
+ * many are free; default 16).  Values out of range are refused with TAIGA_E_ARG when set. */
 int taiga_set_option(taiga_ctx* ctx, const char* key, long long value);
 /* counters of the last taiga_trace (valid with "stats" on): [0] ion-steps, [1] warp-steps*32
  * (lane slots issued), [2] 1, [3] kernel launches, [4] cell refills, [5..7] 0. */
@@ -229,6 +253,9 @@ int taiga_get_stats(taiga_ctx* ctx, unsigned long long stats_host[8]);
 /* register-resident DFMA microkernel: measured FP64 FMA instructions per second (thread-level,
  * i.e. lanes x instr) over ~`ms` milliseconds; the roofline denominator. */
 int taiga_measure_fp64_peak(taiga_ctx* ctx, double ms, double* dfma_per_s);
+/* the same for the FP64 tensor pipe: DMMA.8x8x4 chains, FMA per second (256 per warp instruction); the
+ * denominator of the warp-cooperative tracer of kinds 1 and 2. */
+int taiga_measure_dmma_peak(taiga_ctx* ctx, double ms, double* fma_per_s);
 /* L1-resident gather microkernel shaped like the uncached field evaluation (8 warps/SM, 48 x 256-bit
  * loads of a 1536-B cell per lane): bytes per second delivered to registers; `spread` = distinct cells
  * read by the lanes of a warp (1 ... 32).  The roofline denominator of the kind-1 / kind-2 kernels. */

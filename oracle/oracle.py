@@ -40,7 +40,8 @@ class BeamS(C.Structure):
     _fields_ = [("v0", C.c_double), ("origin", D3), ("axis", D3), ("eT", D3), ("eZ", D3),
                 ("cdf_depth", _dp), ("n_depth", C.c_int), ("depth_max", C.c_double),
                 ("cdf_normal", _dp), ("n_normal", C.c_int), ("z_max", C.c_double),
-                ("sigma_pos", C.c_double), ("sigma_ang", C.c_double)]
+                ("sigma_pos", C.c_double), ("sigma_ang", C.c_double),
+                ("profile", C.c_int), ("radius", C.c_double)]
 
 
 def _p(a):
@@ -164,6 +165,7 @@ def seed(beam, cdf_depth, cdf_normal, seed_value, first_index, n):
     b.cdf_depth, b.n_depth, b.depth_max = _p(cd), len(cd) - 1, beam.depth_max
     b.cdf_normal, b.n_normal, b.z_max = _p(cn), len(cn) - 1, beam.z_max
     b.sigma_pos, b.sigma_ang = beam.sigma_pos_m, beam.sigma_ang_rad
+    b.profile, b.radius = int(getattr(beam, "profile", 0)), float(getattr(beam, "radius_m", 0.0))
     out = [np.empty(n) for _ in range(6)]
     _lib.orc_seed(C.byref(b), C.c_uint64(seed_value), C.c_uint64(first_index), C.c_uint64(n),
                   *[_p(a) for a in out])

@@ -71,8 +71,30 @@ extern "C" void orc_seed(const orc_beam* b, uint64_t seed, uint64_t first_index,
         double z3 = orc_cdf_invert(b->cdf_normal, b->n_normal, 2.0 * b->z_max, U[3]) - b->z_max;
         double z4 = orc_cdf_invert(b->cdf_normal, b->n_normal, 2.0 * b->z_max, U[4]) - b->z_max;
         double r[3], v[3];
+        double scale = b->sigma_pos;
+        if (b->profile == 1) {
+            /* Uniform disc of radius `radius` ("a 60 keV lithium atomic beam with a 5 mm
+             * diameter"; reading A7' in DESIGN.md): rejection from the enclosing square, which is exactly
+             * uniform on the disc and needs +,-,* only.  Try 0 takes (a, c) = (2 U_1 - 1, 2 U_2 - 1) from the
+             * ion's standard uniforms; try k >= 1 takes two fresh uniforms from Philox counter
+             * (i_lo, i_hi, 2 + k, 0), words (0,1) and (2,3); accepted when a^2 + c^2 <= 1.  After 64 rejected
+             * tries (probability (1 - pi/4)^64 = 1e-43) the ion sits on the axis.                      */
+            double a = 2.0 * U[1] - 1.0, c2 = 2.0 * U[2] - 1.0;
+            uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+            uint64_t index = first_index + j;
+            for (uint32_t k = 1; a * a + c2 * c2 > 1.0; ++k) {
+                if (k > 64) { a = 0.0; c2 = 0.0; break; }
+                uint32_t ctr[4] = {(uint32_t)index, (uint32_t)(index >> 32), 2u + k, 0u}, w[4];
+                orc_philox4x32_10(ctr, key, w);
+                uint64_t n0 = ((uint64_t)(w[0] >> 6) << 26) + (uint64_t)(w[1] >> 6);
+                uint64_t n1 = ((uint64_t)(w[2] >> 6) << 26) + (uint64_t)(w[3] >> 6);
+                a = 2.0 * (((double)n0 + 0.5) * 0x1p-52) - 1.0;
+                c2 = 2.0 * (((double)n1 + 0.5) * 0x1p-52) - 1.0;
+            }
+            z1 = a; z2 = c2; scale = b->radius;
+        }
         for (int c = 0; c < 3; ++c)
-            r[c] = (b->origin[c] + d * b->axis[c]) + b->sigma_pos * (z1 * b->eT[c] + z2 * b->eZ[c]);
+            r[c] = (b->origin[c] + d * b->axis[c]) + scale * (z1 * b->eT[c] + z2 * b->eZ[c]);
         if (b->sigma_ang == 0.0) {
             for (int c = 0; c < 3; ++c) v[c] = b->v0 * b->axis[c];
         } else {

@@ -17,7 +17,10 @@
  * P16 Eq. 2 values and limits; P17 loss integral: constant rate -> exp(-nu t_hit) exactly,
  * order 2 under step halving, agreement with an independent quadrature; fixed-point counters;
  * P18 Bezier plane interpolation: exact on parabolas, order 3; P19 weighted-grid seeding:
- * weights sum to 1, marginals = CDF increments, weighted detector image = stochastic image.
+ * weights sum to 1, marginals = CDF increments, weighted detector image = stochastic image;
+ * P20 stage times in a time-linear uniform field (closed-form rotation), Boris B(t_n), trace vs an ODE
+ * solution; P21 weight domain of the fixed-point counters; P22 uniform-disc cross-section: radius bound,
+ * r^2 law, uniform azimuth, second moments R^2/4, acceptance pi/4, retry counters.
  * Parity unpinned: nothing in this file; the paper's own figures that cannot be pinned
  * (Fig. 10 loss rate, Table 1, Fig. 12 curves) are listed in DESIGN.md.
  *
@@ -66,6 +69,8 @@ typedef struct {
     const double* cdf_depth;  int n_depth;  double depth_max;
     const double* cdf_normal; int n_normal; double z_max;
     double sigma_pos, sigma_ang;
+    int profile;                     /* cross-section: 0 = independent Gaussians (A7), 1 = uniform disc (A7') */
+    double radius;                   /* disc radius [m] ("5 mm diameter")              */
 } orc_beam;
 
 /* O2.1  Philox4x32-10 */

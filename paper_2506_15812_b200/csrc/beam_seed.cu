@@ -12,6 +12,7 @@ struct SeedParams {
     double sigma_pos, sigma_ang;
     unsigned long long first_index, seed, n;
     unsigned short group; double t0;
+    int profile; double radius;
 };
 
 __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
@@ -64,11 +65,24 @@ __global__ void __launch_bounds__(256) k_beam_seed(SeedParams P, double* __restr
     double d = cdf_invert(P.cdf_depth, P.n_depth, P.depth_max, U[0]);
     double z1 = __dsub_rn(cdf_invert(P.cdf_normal, P.n_normal, zw, U[1]), P.z_max);
     double z2 = __dsub_rn(cdf_invert(P.cdf_normal, P.n_normal, zw, U[2]), P.z_max);
-    double r[3], v[3];
+    double r[3], v[3], scale = P.sigma_pos;
+    if (P.profile == TAIGA_PROFILE_DISC) {
+        // uniform over the disc ("5 mm diameter"): rejection from the square; retry k reads
+        // counter (i lo, i hi, 2 + k, 0); +, -, * only, explicitly rounded
+        double a = __dsub_rn(__dmul_rn(2.0, U[1]), 1.0), c2 = __dsub_rn(__dmul_rn(2.0, U[2]), 1.0);
+        for (uint32_t k = 1; __dadd_rn(__dmul_rn(a, a), __dmul_rn(c2, c2)) > 1.0; ++k) {
+            if (k > 64) { a = 0.0; c2 = 0.0; break; }
+            uint32_t q[4];
+            philox4x32_10((uint32_t)idx, (uint32_t)(idx >> 32), 2u + k, 0u, (uint32_t)P.seed, (uint32_t)(P.seed >> 32), q);
+            a = __dsub_rn(__dmul_rn(2.0, u52(q[0], q[1])), 1.0);
+            c2 = __dsub_rn(__dmul_rn(2.0, u52(q[2], q[3])), 1.0);
+        }
+        z1 = a; z2 = c2; scale = P.radius;
+    }
 #pragma unroll
-    for (int c = 0; c < 3; ++c)   // r = (origin + d axis) + sigma_pos (z1 eT + z2 eZ)
+    for (int c = 0; c < 3; ++c)   // r = (origin + d axis) + scale (z1 eT + z2 eZ)
         r[c] = __dadd_rn(__dadd_rn(P.origin[c], __dmul_rn(d, P.axis[c])),
-                         __dmul_rn(P.sigma_pos, __dadd_rn(__dmul_rn(z1, P.eT[c]), __dmul_rn(z2, P.eZ[c]))));
+                         __dmul_rn(scale, __dadd_rn(__dmul_rn(z1, P.eT[c]), __dmul_rn(z2, P.eZ[c]))));
     if (P.sigma_ang == 0.0) {
 #pragma unroll
         for (int c = 0; c < 3; ++c) v[c] = __dmul_rn(P.v0, P.axis[c]);
@@ -143,9 +157,19 @@ int tg_seed(taiga_ctx* ctx, const taiga_beam_params* p, uint64_t seed, taiga_ion
     rc = tg_reserve(ctx, &ctx->cdf_normal, &cn, (size_t)p->n_normal + 1);
     ctx->cap_normal = (int)cn;
     if (rc) return rc;
-    // pageable-source async copies are staged before returning, so the host tables may be freed
-    TG_CUDA(ctx, cudaMemcpyAsync(ctx->cdf_depth, p->cdf_depth, ((size_t)p->n_depth + 1) * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
-    TG_CUDA(ctx, cudaMemcpyAsync(ctx->cdf_normal, p->cdf_normal, ((size_t)p->n_normal + 1) * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    // the tables are staged through a context-owned pinned buffer: the caller's arrays are read during the call only,
+    // whatever kind of host memory they live in (a copy from pinned or registered memory is truly asynchronous)
+    {
+        const size_t nd = (size_t)p->n_depth + 1, nn = (size_t)p->n_normal + 1;
+        int rs = tg_stage(ctx, (nd + nn) * sizeof(double));
+        if (rs) return rs;
+        double* h = (double*)ctx->stage;
+        memcpy(h, p->cdf_depth, nd * sizeof(double));
+        memcpy(h + nd, p->cdf_normal, nn * sizeof(double));
+        TG_CUDA(ctx, cudaMemcpyAsync(ctx->cdf_depth, h, nd * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+        TG_CUDA(ctx, cudaMemcpyAsync(ctx->cdf_normal, h + nd, nn * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+        TG_CUDA(ctx, cudaEventRecord(ctx->stage_done, ctx->stream));
+    }
     SeedParams P;
     P.v0 = v0;
     for (int c = 0; c < 3; ++c) { P.origin[c] = p->origin[c]; P.axis[c] = p->axis[c]; P.eT[c] = p->eT[c]; P.eZ[c] = p->eZ[c]; }
@@ -154,6 +178,7 @@ int tg_seed(taiga_ctx* ctx, const taiga_beam_params* p, uint64_t seed, taiga_ion
     P.sigma_pos = p->sigma_pos_m; P.sigma_ang = p->sigma_ang_rad;
     P.first_index = p->first_index; P.seed = seed; P.n = ions->n;
     P.group = p->group; P.t0 = p->t0;
+    P.profile = p->profile; P.radius = p->radius_m;
     unsigned blocks = (unsigned)((ions->n + 255) / 256);
     if (g) k_beam_seed_grid<<<blocks, 256, 0, ctx->stream>>>(P, g->nd, g->nT, g->nZ, g->z_lim, ions->x, ions->y, ions->z, ions->vx,
                                                              ions->vy, ions->vz, ions->w0, ions->group, ions->t0);

@@ -112,10 +112,15 @@ int tg_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* d
     if (rc) return rc;
     cudaStream_t st = ctx->stream;
     double* e = ctx->edges;
-    TG_CUDA(ctx, cudaMemcpyAsync(e, det->u_lo, det->nu * sizeof(double), cudaMemcpyHostToDevice, st));
-    TG_CUDA(ctx, cudaMemcpyAsync(e + det->nu, det->u_hi, det->nu * sizeof(double), cudaMemcpyHostToDevice, st));
-    TG_CUDA(ctx, cudaMemcpyAsync(e + 2 * det->nu, det->w_lo, det->nw * sizeof(double), cudaMemcpyHostToDevice, st));
-    TG_CUDA(ctx, cudaMemcpyAsync(e + 2 * det->nu + det->nw, det->w_hi, det->nw * sizeof(double), cudaMemcpyHostToDevice, st));
+    {   // edges staged through the context's pinned buffer: the caller's arrays are read during the call only
+        rc = tg_stage(ctx, ne * sizeof(double));
+        if (rc) return rc;
+        double* h = (double*)ctx->stage;
+        memcpy(h, det->u_lo, det->nu * sizeof(double)); memcpy(h + det->nu, det->u_hi, det->nu * sizeof(double));
+        memcpy(h + 2 * det->nu, det->w_lo, det->nw * sizeof(double)); memcpy(h + 2 * det->nu + det->nw, det->w_hi, det->nw * sizeof(double));
+        TG_CUDA(ctx, cudaMemcpyAsync(e, h, ne * sizeof(double), cudaMemcpyHostToDevice, st));
+        TG_CUDA(ctx, cudaEventRecord(ctx->stage_done, st));
+    }
     HistParams P;
     P.hit_u = ions->hit_u; P.hit_w = ions->hit_w; P.cell = ions->cell; P.flags = ions->flags; P.group = ions->group;
     P.n = ions->n;

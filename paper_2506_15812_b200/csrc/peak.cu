@@ -2,18 +2,21 @@
 // has no FP64 entry, so the FP64 issue rate is measured in the same run as the benchmark).
 #include "taiga_internal.h"
 
-#define PEAK_CHAINS 8
+// Four independent chains per thread, each with its own multiplicand and addend registers: eight chains sharing
+// two operand registers (the round-1 kernel) reach only 0.91 of 148 x 64 DFMA/clk because of register-bank
+// conflicts on the shared operands; this form measures 0.98-0.99 at 8-32 warps per SM (profiles/r2a_microbench.md).
+#define PEAK_CHAINS 4
 #define PEAK_INNER 64
 
-__global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters, double a, double b) {
-    double v[PEAK_CHAINS];
+__global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters, double a0, double b0) {
+    double v[PEAK_CHAINS], a[PEAK_CHAINS], b[PEAK_CHAINS];
 #pragma unroll
-    for (int c = 0; c < PEAK_CHAINS; ++c) v[c] = (double)(threadIdx.x + c) * 1e-3;
+    for (int c = 0; c < PEAK_CHAINS; ++c) { v[c] = (double)(threadIdx.x + c) * 1e-3; a[c] = a0 + c * 1e-9; b[c] = b0 + c * 1e-12; }
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
         for (int k = 0; k < PEAK_INNER; ++k) {
 #pragma unroll
-            for (int c = 0; c < PEAK_CHAINS; ++c) v[c] = fma(v[c], a, b);
+            for (int c = 0; c < PEAK_CHAINS; ++c) v[c] = fma(v[c], a[c], b[c]);
         }
     }
     double s = 0.0;
@@ -40,6 +43,54 @@ int tg_fp64_peak(taiga_ctx* ctx, double ms, double* rate) {
         if (e != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); TG_CUDA(ctx, e); }
         cudaEventElapsedTime(&t, e0, e1);
         double n = (double)grid * 256.0 * (double)iters * PEAK_INNER * PEAK_CHAINS;
+        if (rep >= 2) { double r = n / (t * 1e-3); if (r > best) best = r; }
+        if (rep == 1 && t > 0.f) { double scale = ms / t; iters = (int)(iters * scale) + 1; if (iters > (1 << 22)) iters = 1 << 22; }
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    TG_CUDA(ctx, cudaGetLastError());
+    *rate = best;
+    return TAIGA_OK;
+}
+
+// FP64 tensor pipe: DMMA.8x8x4 (256 FMA per warp instruction) issue rate, in FMA per second.  On B200 it equals the
+// DFMA rate (the two share the FP64 datapath; a mix of both measures 0.89-0.92 of it), but reads each operand
+// register for 8 FMAs: the denominator of the warp-cooperative tracer (trace_mma.cu).
+__global__ void __launch_bounds__(256) k_dmma_peak(double* out, int iters, double a0, double b0) {
+    double c[4][2], a[4], b[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { c[i][0] = (double)threadIdx.x; c[i][1] = (double)i; a[i] = a0 + i * 1e-9; b[i] = b0 + i * 1e-9; }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k)
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                             : "+d"(c[i][0]), "+d"(c[i][1]) : "d"(a[i]), "d"(b[i]));
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) s += c[i][0] + c[i][1];
+    if (s == 123.456) out[0] = s;
+}
+
+int tg_dmma_peak(taiga_ctx* ctx, double ms, double* rate) {
+    cudaStream_t st = ctx->stream;
+    cudaEvent_t e0, e1;
+    TG_CUDA(ctx, cudaEventCreate(&e0));
+    TG_CUDA(ctx, cudaEventCreate(&e1));
+    double* dummy = (double*)ctx->counters + 12;
+    unsigned grid = (unsigned)ctx->sm_count * 2;      // 2 x 256 threads = 16 warps per SM
+    int iters = 256;
+    float t = 0.f;
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {
+        cudaEventRecord(e0, st);
+        k_dmma_peak<<<grid, 256, 0, st>>>(dummy, iters, 0.999999, 1e-7);
+        cudaEventRecord(e1, st);
+        cudaError_t e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); TG_CUDA(ctx, e); }
+        cudaEventElapsedTime(&t, e0, e1);
+        double n = (double)grid * 256.0 * (double)iters * 16.0 * 4.0 * 8.0;     // 8 FMA per lane and DMMA
         if (rep >= 2) { double r = n / (t * 1e-3); if (r > best) best = r; }
         if (rep == 1 && t > 0.f) { double scale = ms / t; iters = (int)(iters * scale) + 1; if (iters > (1 << 22)) iters = 1 << 22; }
     }

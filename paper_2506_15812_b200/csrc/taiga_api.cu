@@ -37,10 +37,13 @@ extern "C" int taiga_create(taiga_ctx** out, int device, void* cuda_stream) {
         if (ctx->counters) cudaFree(ctx->counters);
         delete ctx; return TAIGA_E_NOMEM;
     }
+    if (cudaEventCreateWithFlags(&ctx->stage_done, cudaEventDisableTiming) != cudaSuccess) {
+        cudaFree(ctx->counters); cudaFreeHost(ctx->counters_host); delete ctx; return TAIGA_E_CUDA;
+    }
     ctx->opt_sort = 1; ctx->opt_sort_sub = 16;
     ctx->opt_min_active = 32;
     ctx->opt_ctas_per_sm = 0; ctx->opt_variant = 0; ctx->opt_stats = 1; ctx->opt_precision = 64; ctx->opt_plane_interp = 0; ctx->opt_regroup = 8;
-    ctx->opt_mma = 1; ctx->opt_refill_cta = 0;
+    ctx->opt_mma = -1; ctx->opt_refill_cta = 0;
     strcpy(ctx->err, "ok");
     *out = ctx;
     return TAIGA_OK;
@@ -54,6 +57,8 @@ extern "C" int taiga_destroy(taiga_ctx* ctx) {
                     ctx->bins, ctx->counters, ctx->table32, ctx->psi_table, ctx->loss_rate, ctx->dtable, ctx->frag};
     for (void* b : bufs) if (b) cudaFree(b);
     if (ctx->counters_host) cudaFreeHost(ctx->counters_host);
+    if (ctx->stage) cudaFreeHost(ctx->stage);
+    if (ctx->stage_done) cudaEventDestroy(ctx->stage_done);
     delete ctx;
     return TAIGA_OK;
 }
@@ -110,7 +115,9 @@ static int seed_common(taiga_ctx* ctx, const taiga_beam_params* p, uint64_t seed
     int rc = check_ions(ctx, ions, false);
     if (rc) return rc;
     if (!(p->mass_kg > 0) || !(p->charge_C != 0) || !(p->energy_eV > 0) || !(p->depth_max > 0) || !(p->z_max > 0) ||
-        p->sigma_pos_m < 0 || p->sigma_ang_rad < 0) { TG_SET_ERR(ctx, "seed_beam: bad beam parameters"); return TAIGA_E_ARG; }
+        p->sigma_pos_m < 0 || p->sigma_ang_rad < 0 || (p->profile != TAIGA_PROFILE_GAUSSIAN && p->profile != TAIGA_PROFILE_DISC) ||
+        (p->profile == TAIGA_PROFILE_DISC && !(p->radius_m > 0))) { TG_SET_ERR(ctx, "seed_beam: bad beam parameters"); return TAIGA_E_ARG; }
+    if (g && p->profile != TAIGA_PROFILE_GAUSSIAN) { TG_SET_ERR(ctx, "seed_beam_grid: the weighted grid is defined for the Gaussian profile"); return TAIGA_E_ARG; }
     if (!orthonormal(p->axis, p->eT, p->eZ)) { TG_SET_ERR(ctx, "seed_beam: (axis,eT,eZ) not orthonormal"); return TAIGA_E_ARG; }
     if (!cdf_ok(p->cdf_depth, p->n_depth) || !cdf_ok(p->cdf_normal, p->n_normal)) {
         TG_SET_ERR(ctx, "seed_beam: CDF table must have F[0]=0, F[K]=1 and be non-decreasing"); return TAIGA_E_ARG;
@@ -193,6 +200,11 @@ extern "C" int taiga_detector_histogram_weighted(taiga_ctx* ctx, const taiga_ion
     if (n_hist < 1 || n_hist > 65536 || !wcounts || !wsummary) { TG_SET_ERR(ctx, "histogram_weighted: bad n_hist / null output"); return TAIGA_E_ARG; }
     if (ions->n == 0) return TAIGA_OK;
     if (!ions->weight && !ions->w0) { TG_SET_ERR(ctx, "histogram_weighted: ions->weight and ions->w0 are null"); return TAIGA_E_ARG; }
+    if (ions->weight && !ctx->weight_written) {
+        TG_SET_ERR(ctx, "histogram_weighted: ions->weight is set but the last taiga_trace of this context wrote no weights "
+                        "(no loss model loaded); pass weight = null to count w0 only");
+        return TAIGA_E_STATE;
+    }
     TG_CUDA(ctx, cudaSetDevice(ctx->device));
     return tg_histogram_weighted(ctx, ions, det, n_hist, wcounts, wsummary);
 }
@@ -224,7 +236,8 @@ extern "C" int taiga_set_option(taiga_ctx* ctx, const char* key, long long v) {
         {"precision", &ctx->opt_precision, 32, 64}, {"plane_interp", &ctx->opt_plane_interp, 0, 1},
         {"regroup", &ctx->opt_regroup, 0, 1 << 20}, {"min_active", &ctx->opt_min_active, 0, 32},
         {"ctas_per_sm", &ctx->opt_ctas_per_sm, 0, 32}, {"variant", &ctx->opt_variant, 0, 5}, {"stats", &ctx->opt_stats, 0, 1},
-        {"mma", &ctx->opt_mma, 0, 1}, {"refill_cta", &ctx->opt_refill_cta, 0, 1024}};
+        {"mma", &ctx->opt_mma, -1, 1}, {"refill_cta", &ctx->opt_refill_cta, 0, 1024},
+        {"mma_geom", &ctx->opt_mma_geom, 0, 5}};
     for (auto& t : tab) if (!strcmp(key, t.k)) {
         if (v < t.lo || v > t.hi || (t.p == &ctx->opt_precision && v != 32 && v != 64)) {
             TG_SET_ERR(ctx, "set_option: %s = %lld out of range [%lld, %lld]", key, v, t.lo, t.hi);
@@ -253,4 +266,20 @@ extern "C" int taiga_measure_fp64_peak(taiga_ctx* ctx, double ms, double* rate) 
     if (!ctx || !rate || !(ms > 0)) return TAIGA_E_ARG;
     TG_CUDA(ctx, cudaSetDevice(ctx->device));
     return tg_fp64_peak(ctx, ms, rate);
+}
+
+extern "C" int taiga_measure_dmma_peak(taiga_ctx* ctx, double ms, double* rate) {
+    if (!ctx || !rate || !(ms > 0)) return TAIGA_E_ARG;
+    TG_CUDA(ctx, cudaSetDevice(ctx->device));
+    return tg_dmma_peak(ctx, ms, rate);
+}
+
+extern "C" int taiga_loss_statistics(const unsigned long long ws[4], double out[3]) {
+    if (!ws || !out) return TAIGA_E_ARG;
+    const double n = ws[3] ? (double)ws[3] : 1.0;
+    const double mu = ((double)ws[0] + (double)ws[1]) / 4294967296.0 / n;
+    double var = (double)ws[2] / 4294967296.0 / n - mu * mu;
+    if (!(var > 0.0)) var = 0.0;
+    out[0] = 1.0 - mu; out[1] = sqrt(var); out[2] = (double)ws[3];
+    return TAIGA_OK;
 }

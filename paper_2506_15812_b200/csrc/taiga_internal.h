@@ -61,6 +61,9 @@ struct taiga_ctx {
     // seeding tables
     double *cdf_depth, *cdf_normal;  int cap_depth, cap_normal;
 
+    // pinned staging buffer for small host tables (CDFs, detector edges): reused once `stage_done` has passed
+    void* stage;              size_t stage_cap;    cudaEvent_t stage_done;
+
     // detector edges (histogram)
     double* edges;            int cap_edges;
 
@@ -74,7 +77,7 @@ struct taiga_ctx {
     // options
     int opt_sort, opt_min_active, opt_ctas_per_sm, opt_variant, opt_stats;
     int opt_sort_sub, opt_precision, opt_plane_interp, opt_regroup;
-    int opt_mma, opt_refill_cta;
+    int opt_mma, opt_refill_cta, opt_mma_geom;
     bool weight_written;                                 // the last taiga_trace wrote ions->weight (loss model)
 };
 
@@ -101,6 +104,19 @@ static inline int tg_reserve(taiga_ctx* ctx, T** p, size_t* cap, size_t need) {
     return TAIGA_OK;
 }
 
+// Pinned staging for small host tables: waits until the previous staged copy has left the buffer, grows it if needed.
+static inline int tg_stage(taiga_ctx* ctx, size_t bytes) {
+    if (ctx->stage_done) cudaEventSynchronize(ctx->stage_done);
+    if (ctx->stage_cap < bytes) {
+        if (ctx->stage) cudaFreeHost(ctx->stage);
+        ctx->stage = nullptr; ctx->stage_cap = 0;
+        size_t cap = bytes < 65536 ? 65536 : bytes;
+        if (cudaMallocHost(&ctx->stage, cap) != cudaSuccess) { TG_SET_ERR(ctx, "cudaMallocHost(%zu B) failed", cap); return TAIGA_E_NOMEM; }
+        ctx->stage_cap = cap;
+    }
+    return TAIGA_OK;
+}
+
 // implemented in the per-kernel translation units
 int tg_precompute(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c);
 int tg_seed(taiga_ctx* ctx, const taiga_beam_params* p, uint64_t seed, taiga_ions* ions, double v0,
@@ -121,4 +137,5 @@ int tg_load_loss(taiga_ctx* ctx, const double* psi_nodal, int on_device, const t
 int tg_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
                           unsigned long long* wcounts, unsigned long long* wsummary);
 int tg_fp64_peak(taiga_ctx* ctx, double ms, double* rate);
+int tg_dmma_peak(taiga_ctx* ctx, double ms, double* rate);
 int tg_l1_gather_peak(taiga_ctx* ctx, double ms, int spread, double* bytes_per_s);

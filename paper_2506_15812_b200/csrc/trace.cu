@@ -552,7 +552,8 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     }
     TG_CUDA(ctx, cudaMemsetAsync(ctx->counters, 0, 8 * sizeof(unsigned long long), st));
     const int S = variant <= 1 ? 0 : (variant == 2 ? 2 : 3);
-    if (kind >= 1 && ctx->opt_mma && !f32 && tg_mma_supported(ctx)) {
+    const int use_mma = ctx->opt_mma < 0 ? (kind == 2) : ctx->opt_mma;      // default: kind 2 (kind 1: 3 DMMAs per set do not pay)
+    if (kind >= 1 && use_mma && !f32 && tg_mma_supported(ctx)) {
         // kinds 1, 2: warp-cooperative evaluation on the FP64 tensor pipe (trace_mma.cu), every solver and option
         int rc = tg_trace_mma(ctx, P, S, hasE || S != 0, loss, bez, ions->n);
         if (rc) return rc;

@@ -29,12 +29,27 @@
 #include "trace_common.cuh"
 
 #define TG_IDX(L) ((L) + 2 * ((L) >> 4))          // skewed slot of lane L: quad-strided 64-bit reads hit distinct banks
+#define TG_ROW 35                                 // row stride of the per-warp buffer: 34 slots; 35 = 3 mod 16 keeps the 16 lanes
+                                                  // of a half-warp (rows r = 0..3 or 4..7, t = 0..3) on distinct 8-byte banks
+#define TG_ROWB (TG_ROW * 8)                      // ... in bytes
 
-struct __align__(16) TgWarpBuf {
-    double w[34], q[34];                          // in-cell coordinates of the warp's ions (w; q or tau)
-    double out[424];                              // f[(m * 4 + t) * 35 + slot]: 34 slots per row, stride 35 = 3 mod 16 keeps the
-                                                  // 16 lanes of a half-warp (r = 0..3 or 4..7, t = 0..3) on distinct 8-byte banks
+// Per-warp exchange buffer, rows of TG_ROW doubles indexed by the slot of an ion's own lane:
+//   rows 0..7   A operands [s * 4 + t] = w^t q^(2s)        row 8   q (kind 2) / tau (kind 1)
+//   rows 9..20  results f[m * 4 + t]
+struct __align__(16) TgWarpBuf { double v[21 * TG_ROW + 1]; };
+
+// Shared-memory addresses of one lane, computed once per kernel: ptxas otherwise rematerialises them from
+// %tid / the CTA's window base inside the item loop (60 integer instructions per 6 DMMAs in the r2a profile).
+struct TgLane {
+    unsigned own;                                 // &v[slot of my lane]                  (my ion's column)
+    unsigned quad;                                // &v[t * TG_ROW + slot of lane 4r]     (+ 8 g: column of ion (g, r), row t)
+    unsigned qrow;                                // &v[8 * TG_ROW + slot of lane 4r]
+    unsigned bit0;                                // 1 << 4r: bit of ion (0, r) in a lane mask
+    const double* frag;                           // fragment table + lane
 };
+
+__device__ __forceinline__ double tg_lds(unsigned a) { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a)); return v; }
+__device__ __forceinline__ void tg_sts(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
 
 __device__ __forceinline__ void tg_dmma(double& d0, double& d1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
@@ -62,72 +77,79 @@ __device__ __forceinline__ int tg_locate_cell(const FieldDev& f, double X, doubl
 }
 
 // Warp-collective evaluation: every lane calls it; cell < 0 = this lane has no ion to evaluate.
+// Work items = (cell, group) pairs: the ions of one group (lanes 4r + g) that sit in one cell.  The operands of
+// item i+1 are fetched right after the DMMAs of item i have issued (DMMA reads its registers at issue), so their
+// latency overlaps the tensor pipe.
 template <int KIND>
-__device__ __forceinline__ void tg_eval_mma(const double* __restrict__ frag, TgWarpBuf& wb, int lane, int cell,
-                                            double p, double w, double q, double& BR, double& BZ, double& Bp, unsigned& sets) {
+__device__ __forceinline__ void tg_eval_mma(const TgLane& L, int cell, double p, double w, double q,
+                                            double& BR, double& BZ, double& Bp, unsigned& sets) {
     constexpr int KS = (KIND == 2) ? 2 : 1;
     const unsigned FULL = 0xffffffffu;
-    const int t = lane & 3, base = lane & ~3;
-    wb.w[TG_IDX(lane)] = w; wb.q[TG_IDX(lane)] = q;
-    __syncwarp();
-    double a[4][KS], qg[4];
-#pragma unroll
-    for (int g = 0; g < 4; ++g) {
-        const int s = TG_IDX(base + g);
-        double wg = wb.w[s];
-        qg[g] = wb.q[s];
-        double w2 = wg * wg;
-        double pw = (t == 0) ? 1.0 : ((t == 1) ? wg : ((t == 2) ? w2 : w2 * wg));
-        a[g][0] = pw;
-        if constexpr (KS == 2) a[g][1] = pw * (qg[g] * qg[g]);
+    {                                             // my ion's monomials and q into the warp buffer
+        const double w2 = w * w, w3 = w2 * w;
+        tg_sts(L.own, 1.0); tg_sts(L.own + TG_ROWB, w); tg_sts(L.own + 2 * TG_ROWB, w2); tg_sts(L.own + 3 * TG_ROWB, w3);
+        if constexpr (KS == 2) {
+            const double q2 = q * q;
+            tg_sts(L.own + 4 * TG_ROWB, q2); tg_sts(L.own + 5 * TG_ROWB, w * q2);
+            tg_sts(L.own + 6 * TG_ROWB, w2 * q2); tg_sts(L.own + 7 * TG_ROWB, w3 * q2);
+        }
+        tg_sts(L.own + 8 * TG_ROWB, q);
     }
+    __syncwarp();
     unsigned todo = __ballot_sync(FULL, cell >= 0);
-    while (todo) {
-        int leader = __ffs(todo) - 1;
-        int cs = __shfl_sync(FULL, cell, leader);
-        unsigned match = __ballot_sync(FULL, cell == cs);
-        todo &= ~match;
-        const double* src = frag + (size_t)cs * (KS * 96) + lane;
-        double b[KS][3];
+    double b[KS][3], a[KS], qg = 0.0;
+    unsigned mem = 0, gofs = 0;
+    auto fetch = [&]() {                          // next item of `todo`: group and cell of its lowest lane
+        const int lead = __ffs(todo) - 1;
+        const int cs = __shfl_sync(FULL, cell, lead);
+        const unsigned g = lead & 3;
+        mem = __ballot_sync(FULL, cell == cs) & (0x11111111u << g) & todo;
+        gofs = g * 8;
+        const double* src = L.frag + (size_t)cs * (KS * 96);
 #pragma unroll
         for (int s = 0; s < KS; ++s)
 #pragma unroll
             for (int m = 0; m < 3; ++m) b[s][m] = __ldg(src + (s * 3 + m) * 32);
 #pragma unroll
-        for (int g = 0; g < 4; ++g) {
-            unsigned gm = match & (0x11111111u << g);
-            if (gm) {                                                  // warp-uniform
-                double d[3][2];
+        for (int s = 0; s < KS; ++s) a[s] = tg_lds(L.quad + gofs + s * 4 * TG_ROWB);
+        qg = tg_lds(L.qrow + gofs);
+    };
+    if (todo) fetch();
+    while (mem) {                                 // warp-uniform
+        double d[3][2];
 #pragma unroll
-                for (int m = 0; m < 3; ++m) { d[m][0] = 0.0; d[m][1] = 0.0; }
+        for (int m = 0; m < 3; ++m) { d[m][0] = 0.0; d[m][1] = 0.0; }
 #pragma unroll
-                for (int s = 0; s < KS; ++s)
+        for (int s = 0; s < KS; ++s)
 #pragma unroll
-                    for (int m = 0; m < 3; ++m) tg_dmma(d[m][0], d[m][1], a[g][s], b[s][m]);
-                ++sets;
-                if ((gm >> (base + g)) & 1u) {                         // the ion of my row is in this cell
-                    double* o = wb.out + t * 35 + TG_IDX(base + g);
+            for (int m = 0; m < 3; ++m) tg_dmma(d[m][0], d[m][1], a[s], b[s][m]);
+        ++sets;
+        const double qc = qg;
+        const bool mine = mem & (L.bit0 << (gofs >> 3));       // the ion of my row is served by this item
+        const unsigned o = L.quad + 9 * TG_ROWB + gofs;
+        todo &= ~mem;
+        mem = 0;
+        if (todo) fetch();
+        if (mine) {
 #pragma unroll
-                    for (int m = 0; m < 3; ++m) o[m * 140] = fma(qg[g], d[m][1], d[m][0]);
-                }
-                __syncwarp();                                          // the next DMMA is warp-collective
-            }
+            for (int m = 0; m < 3; ++m) tg_sts(o + m * 4 * TG_ROWB, fma(qc, d[m][1], d[m][0]));
         }
+        __syncwarp();                             // the next DMMA is warp-collective
     }
     __syncwarp();
     if (cell >= 0) {
-        const double* o = wb.out + TG_IDX(lane);
-        BR = fma(fma(fma(o[105], p, o[70]), p, o[35]), p, o[0]);
-        BZ = fma(fma(fma(o[140 + 105], p, o[140 + 70]), p, o[140 + 35]), p, o[140]);
-        Bp = fma(fma(fma(o[280 + 105], p, o[280 + 70]), p, o[280 + 35]), p, o[280]);
+        const unsigned o = L.own + 9 * TG_ROWB;
+        BR = fma(fma(fma(tg_lds(o + 3 * TG_ROWB), p, tg_lds(o + 2 * TG_ROWB)), p, tg_lds(o + TG_ROWB)), p, tg_lds(o));
+        BZ = fma(fma(fma(tg_lds(o + 7 * TG_ROWB), p, tg_lds(o + 6 * TG_ROWB)), p, tg_lds(o + 5 * TG_ROWB)), p, tg_lds(o + 4 * TG_ROWB));
+        Bp = fma(fma(fma(tg_lds(o + 11 * TG_ROWB), p, tg_lds(o + 10 * TG_ROWB)), p, tg_lds(o + 9 * TG_ROWB)), p, tg_lds(o + 8 * TG_ROWB));
     }
 }
 
 #define TG_KEY_DEAD 0x7fffff
 
 // SOLVER / HAS_E / LOSS / BEZ as in trace.cu's k_trace.
-template <int KIND, int THREADS, int MINB, int SOLVER, bool HAS_E, bool LOSS, bool BEZ>
-__global__ void __launch_bounds__(THREADS, MINB) k_trace_mma(const TraceParams P) {
+template <int KIND, int THREADS, int MAXREG, int SOLVER, bool HAS_E, bool LOSS, bool BEZ>
+__global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const TraceParams P) {
     constexpr int NW = THREADS / 32;
     constexpr int ND = LOSS ? 10 : 8;
     const unsigned FULL = 0xffffffffu;
@@ -138,7 +160,16 @@ __global__ void __launch_bounds__(THREADS, MINB) k_trace_mma(const TraceParams P
     __shared__ unsigned long long s_base;
     __shared__ int s_wcnt[NW];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    TgWarpBuf& wb = s_wb[warp];
+    TgLane L;
+    {
+        const unsigned wb = (unsigned)__cvta_generic_to_shared(&s_wb[warp]);
+        const int t4 = lane & 3, slot0 = TG_IDX(lane & ~3);
+        L.own = wb + TG_IDX(lane) * 8;
+        L.quad = wb + t4 * TG_ROWB + slot0 * 8;
+        L.qrow = wb + 8 * TG_ROWB + slot0 * 8;
+        L.bit0 = 1u << (lane & ~3);
+        L.frag = P.frag + lane;
+    }
 
     double X = 0, Y = 0, Z = 0, Ux = 0, Uy = 0, Uz = 0, t = 0, s0 = -1.0;
     double Lam = 0.0, nu0 = 0.0;
@@ -157,7 +188,7 @@ __global__ void __launch_bounds__(THREADS, MINB) k_trace_mma(const TraceParams P
             rinv = tg_rsqrt(R2); Rs = R2 * rinv;
             cell = tg_locate_cell<KIND>(P.f, Xs, Ys, Zs, Rs, ts, p, w, q);
         }
-        tg_eval_mma<KIND>(P.frag, wb, lane, cell, p, w, q, BR, BZ, Bp, sets);
+        tg_eval_mma<KIND>(L, cell, p, w, q, BR, BZ, Bp, sets);
         if (alive) { tg_rotate(Xs, Ys, rinv, BR, Bp, bx, by); bz = BZ; }
     };
 
@@ -438,13 +469,21 @@ bool tg_mma_supported(const taiga_ctx* ctx) {
     return ncell < (1ll << 31) && f.nS >= 2;
 }
 
-template <int KIND, int SOLVER, bool HAS_E, bool LOSS, bool BEZ>
-static void tg_launch_mma_t(const TraceParams& P, unsigned sms, int per_sm, uint64_t n, cudaStream_t st) {
-    constexpr int THREADS = 128, MINB = 4;
-    unsigned grid = sms * (unsigned)(per_sm > 0 ? per_sm : MINB);
+// Launch geometry: THREADS per CTA (the pool the CTA re-sorts; 32 = every warp on its own, no CTA barrier) and the
+// register cap.  The kernel is latency-bound (throughput scales with resident warps up to the point where ptxas
+// spills: profiles/r2b_mma_kernel.md), so the grid is one persistent CTA per resident slot.
+template <int KIND, int SOLVER, bool HAS_E, bool LOSS, bool BEZ, int THREADS = 128, int MAXREG = 168>
+static int tg_launch_mma_t(taiga_ctx* ctx, const TraceParams& P, int per_sm, uint64_t n, cudaStream_t st) {
+    auto kern = k_trace_mma<KIND, THREADS, MAXREG, SOLVER, HAS_E, LOSS, BEZ>;
+    int resident = 0;
+    TG_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, THREADS, 0));
+    if (resident < 1) resident = 1;
+    if (per_sm > 0 && per_sm < resident) resident = per_sm;
+    unsigned grid = (unsigned)ctx->sm_count * (unsigned)resident;
     unsigned need = (unsigned)((n + THREADS - 1) / THREADS);
     if (grid > need) grid = need;
-    k_trace_mma<KIND, THREADS, MINB, SOLVER, HAS_E, LOSS, BEZ><<<grid, THREADS, 0, st>>>(P);
+    kern<<<grid, THREADS, 0, st>>>(P);
+    return TAIGA_OK;
 }
 
 // solver: 0 RKN (P.variant 0 / 1), 2 RK4, 3 Boris (P.variant 3 / 4).  loss / bez: with RKN and E = 0 only (as trace.cu).
@@ -458,21 +497,30 @@ int tg_trace_mma(taiga_ctx* ctx, TraceParams& P, int solver, bool hasE, bool los
     while ((ncell >> P.key_shift) >= TG_KEY_DEAD - 1) ++P.key_shift;
     if (P.regroup_every < 1) P.regroup_every = 8;
     P.refill_cta = ctx->opt_refill_cta > 0 ? ctx->opt_refill_cta : 16;
-    const unsigned sms = (unsigned)ctx->sm_count;
     const int per_sm = ctx->opt_ctas_per_sm;
     cudaStream_t st = ctx->stream;
-#define TG_MMA(K, S, E, L, B) tg_launch_mma_t<K, S, E, L, B>(P, sms, per_sm, n, st)
+#define TG_MMA(K, S, E, L, B, ...) rc = tg_launch_mma_t<K, S, E, L, B, ##__VA_ARGS__>(ctx, P, per_sm, n, st)
 #define TG_MMA_KIND(K)                                                        \
     do {                                                                      \
         if (bez) TG_MMA(K, 0, false, false, true);                            \
         else if (loss) TG_MMA(K, 0, false, true, false);                      \
-        else if (solver == 0) { if (hasE) TG_MMA(K, 0, true, false, false); else TG_MMA(K, 0, false, false, false); } \
-        else if (solver == 2) TG_MMA(K, 2, true, false, false);               \
+        else if (solver == 0 && hasE) TG_MMA(K, 0, true, false, false);       \
+        else if (solver == 0) {                                               \
+            switch (ctx->opt_mma_geom) {                                      \
+                case 1: TG_MMA(K, 0, false, false, false, 128, 128); break;   \
+                case 2: TG_MMA(K, 0, false, false, false, 64, 144); break;    \
+                case 3: TG_MMA(K, 0, false, false, false, 32, 144); break;    \
+                case 4: TG_MMA(K, 0, false, false, false, 32, 128); break;    \
+                case 5: TG_MMA(K, 0, false, false, false, 64, 128); break;    \
+                default: TG_MMA(K, 0, false, false, false); break;            \
+            }                                                                 \
+        } else if (solver == 2) TG_MMA(K, 2, true, false, false);             \
         else TG_MMA(K, 3, true, false, false);                                \
     } while (0)
     if (f.kind == 2) TG_MMA_KIND(2); else TG_MMA_KIND(1);
 #undef TG_MMA_KIND
 #undef TG_MMA
+    if (rc) return rc;
     TG_CUDA(ctx, cudaGetLastError());
     return TAIGA_OK;
 }

@@ -30,7 +30,7 @@ EXPORTS = ["taiga_create", "taiga_destroy", "taiga_last_error", "taiga_load_fiel
            "taiga_detector_histogram_weighted", "taiga_seed_beam_grid",
            "taiga_field_eval", "taiga_field_table", "taiga_seed_beam", "taiga_trace",
            "taiga_detector_histogram", "taiga_set_efield", "taiga_set_option", "taiga_get_stats",
-           "taiga_measure_fp64_peak", "taiga_measure_l1_gather_peak"]
+           "taiga_measure_fp64_peak", "taiga_measure_l1_gather_peak", "taiga_measure_dmma_peak", "taiga_loss_statistics"]
 
 
 class GridS(C.Structure):
@@ -50,7 +50,8 @@ class BeamS(C.Structure):
                 ("cdf_depth", C.c_void_p), ("n_depth", C.c_int), ("depth_max", C.c_double),
                 ("cdf_normal", C.c_void_p), ("n_normal", C.c_int), ("z_max", C.c_double),
                 ("sigma_pos_m", C.c_double), ("sigma_ang_rad", C.c_double),
-                ("first_index", C.c_uint64), ("group", C.c_uint16), ("t0", C.c_double)]
+                ("first_index", C.c_uint64), ("group", C.c_uint16), ("t0", C.c_double),
+                ("profile", C.c_int), ("radius_m", C.c_double)]
 
 
 class IonsS(C.Structure):
@@ -94,6 +95,8 @@ _lib.taiga_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_longlong]
 _lib.taiga_get_stats.argtypes = [C.c_void_p, C.POINTER(C.c_ulonglong * 8)]
 _lib.taiga_measure_fp64_peak.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
 _lib.taiga_measure_l1_gather_peak.argtypes = [C.c_void_p, C.c_double, C.c_int, C.POINTER(C.c_double)]
+_lib.taiga_measure_dmma_peak.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
+_lib.taiga_loss_statistics.argtypes = [C.POINTER(C.c_ulonglong * 4), C.POINTER(C.c_double * 3)]
 
 
 class TaigaError(RuntimeError):
@@ -210,6 +213,7 @@ class Taiga:
         p.cdf_normal, p.n_normal, p.z_max = cn.ctypes.data, len(cn) - 1, beam.z_max
         p.sigma_pos_m, p.sigma_ang_rad = beam.sigma_pos_m, beam.sigma_ang_rad
         p.first_index, p.group, p.t0 = int(first_index), int(group), float(t0)
+        p.profile, p.radius_m = int(getattr(beam, "profile", 0)), float(getattr(beam, "radius_m", 0.0))
         ions.meta["use_w0"] = False
         s = ions.struct()
         self._chk(_lib.taiga_seed_beam(self.h, C.byref(p), C.c_uint64(seed), C.byref(s)))
@@ -258,7 +262,8 @@ class Taiga:
             self._chk(_lib.taiga_load_loss(self.h, a.ctypes.data, 0, C.byref(prof)))
 
     def detector_histogram_weighted(self, ions, det, n_hist, wcounts, wsummary, use_loss_weight=True):
-        """use_loss_weight=False: weight by ions.w0 only (no loss model traced)."""
+        """use_loss_weight=False: weight by ions.w0 only (no loss model traced; with True the library refuses
+        weights that the last trace did not write)."""
         d, keep = self._det(det)
         s = ions.struct(weight=use_loss_weight)
         assert wcounts.dtype == torch.int64 and wsummary.dtype == torch.int64
@@ -295,17 +300,24 @@ class Taiga:
         self._chk(_lib.taiga_measure_fp64_peak(self.h, ms, C.byref(r)))
         return r.value
 
+    def dmma_peak(self, ms=50.0):
+        r = C.c_double()
+        self._chk(_lib.taiga_measure_dmma_peak(self.h, ms, C.byref(r)))
+        return r.value
+
 
 def loss_statistics(wsummary):
-    """Mean and standard deviation of the secondary-ionisation loss 1 - weight over the plane-crossing
-    ions of each histogram (the form of PAPER.md Table 1), from the 32.32 fixed-point sums
-    wsummary[n_hist][4] = {sum q in segments, sum q outside, sum q^2 >> 32, crossers}.  Host arithmetic
-    on a few integers (the division by N the paper does on the CPU, L350)."""
-    ws = np.asarray(wsummary.detach().cpu().numpy() if isinstance(wsummary, torch.Tensor) else wsummary, dtype=np.float64)
-    n = np.maximum(ws[:, 3], 1.0)
-    mean_w = (ws[:, 0] + ws[:, 1]) / 4294967296.0 / n
-    var_w = np.maximum(ws[:, 2] / 4294967296.0 / n - mean_w ** 2, 0.0)
-    return 1.0 - mean_w, np.sqrt(var_w)
+    """taiga_loss_statistics per histogram: (mean loss, spread of the loss) over the plane-crossing ions, the form of
+    PAPER.md Table 1; wsummary[n_hist][4] as written by detector_histogram_weighted (device tensor or host array)."""
+    ws = np.ascontiguousarray(wsummary.detach().cpu().numpy() if isinstance(wsummary, torch.Tensor) else wsummary).astype(np.uint64)
+    mean, spread = np.empty(len(ws)), np.empty(len(ws))
+    for h, row in enumerate(ws):
+        out = (C.c_double * 3)()
+        rc = _lib.taiga_loss_statistics(C.byref((C.c_ulonglong * 4)(*[int(v) for v in row])), C.byref(out))
+        if rc:
+            raise TaigaError(rc, "taiga_loss_statistics")
+        mean[h], spread[h] = out[0], out[1]
+    return mean, spread
 
 
 def run_config(tg: Taiga, cfg, field_loaded=False, host_field=True, ions=None, rkn_variant=0):

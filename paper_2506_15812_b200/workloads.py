@@ -189,6 +189,8 @@ class Beam:
     eZ: tuple = BEAM_EZ
     depth_max: float = DEPTH_MAX
     z_max: float = NORMAL_ZMAX
+    profile: int = 0               # cross-section: 0 = Gaussian sigma_pos_m, 1 = uniform disc of radius_m
+    radius_m: float = 2.5e-3
 
 
 @dataclass

@@ -1,0 +1,43 @@
+"""bench.py --gpus N launches N ranks by itself (torchrun --standalone, 127.0.0.1) and shards the config; checked on
+CPU with world size 2 (gloo): the ranks stop after the rank / shard set-up, before the CUDA library is touched."""
+import json
+import os
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _run(*extra):
+    env = dict(os.environ)
+    env.pop("WORLD_SIZE", None); env.pop("RANK", None); env.pop("LOCAL_RANK", None)
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--dry-run-ranks", *extra], capture_output=True, text=True,
+                       env=env, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, r.stdout                       # rank 0 alone prints, one line
+    return json.loads(lines[0])
+
+
+def test_spawn_command_is_the_drivers_launch_line():
+    sys.path.insert(0, ROOT)
+    import bench
+    cmd = bench.spawn_command(["--gpus", "4", "--steps", "2"], 4)
+    assert cmd[1:4] == ["-m", "torch.distributed.run", "--standalone"] and "--nproc-per-node" in cmd and cmd[cmd.index("--nproc-per-node") + 1] == "4"
+    assert "127.0.0.1" in cmd and cmd[-4:] == ["--gpus", "4", "--steps", "2"]
+
+
+def test_gpus_2_spawns_two_ranks_weak_and_strong():
+    d = _run("--gpus", "2", "--config", "2")
+    assert d["n_gpus"] == 2 and d["scaling"] == "weak"
+    r0, r1 = sorted(d["ranks"], key=lambda r: r["rank"])
+    assert (r0["device"], r1["device"]) == ("cuda:0", "cuda:1")
+    assert r0["n_ions"] == r1["n_ions"] == 1048576 and r0["first_index"] == 0 and r1["first_index"] == 1 << 40
+    d = _run("--gpus", "2", "--config", "2", "--scaling", "strong")
+    r0, r1 = sorted(d["ranks"], key=lambda r: r["rank"])
+    assert r0["n_ions"] + r1["n_ions"] == 1048576 and r1["first_index"] == r0["n_ions"] and d["scaling"] == "strong"
+
+
+def test_single_gpu_does_not_spawn():
+    d = _run()
+    assert d["n_gpus"] == 1 and len(d["ranks"]) == 1

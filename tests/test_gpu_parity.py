@@ -169,6 +169,78 @@ def test_seeding_bit_exact_large_indices_and_divergence(tg):
         assert np.all(_np(ions.group) == 3) and np.all(_np(ions.t0) == 2.5e-6)
 
 
+def test_disc_beam_profile_bit_exact(tg):
+    """Uniform-disc cross-section (PAPER.md: "5 mm diameter"; reading A7'): bit-exact against the oracle at
+    indices beyond 2^32, with divergence and a tilted frame, retries included; then the whole path on config 1."""
+    import dataclasses
+    from paper_2506_15812_b200 import taiga
+    beam = wl.Beam(wl.MASS_LI7, wl.E_CHARGE, 60e3, sigma_ang_rad=3e-3, origin=(0.8, 0.01, -0.02), axis=(-0.6, 0.0, 0.8),
+                   eT=(0.0, 1.0, 0.0), eZ=(0.8, 0.0, 0.6), profile=1, radius_m=2.5e-3)
+    cd, cn = wl.depth_cdf(), wl.normal_cdf()
+    for first, seed, n in ((0, 0, 1), ((1 << 40) + 999, 0xDEADBEEFCAFEF00D, 100003), (2 ** 32 - 7, 11, 257)):
+        ions = taiga.Ions(n)
+        tg.seed_beam(beam, cd, cn, seed, ions, first_index=first)
+        torch.cuda.synchronize()
+        ref = orc.seed(beam, cd, cn, seed, first, n)
+        for k, a in zip(("x", "y", "z", "vx", "vy", "vz"), ref):
+            assert np.array_equal(_np(ions.a[k]), a), (k, first)
+    with pytest.raises(taiga.TaigaError):
+        tg.seed_beam(dataclasses.replace(beam, radius_m=0.0), cd, cn, 0, taiga.Ions(4))
+    with pytest.raises(taiga.TaigaError):
+        tg.seed_beam(dataclasses.replace(beam, profile=7), cd, cn, 0, taiga.Ions(4))
+    cfg = wl.config(1)
+    cfg.groups[0].beam = dataclasses.replace(cfg.groups[0].beam, profile=1, radius_m=2.5e-3)
+    ions, counts, summary = taiga.run_config(tg, cfg)
+    torch.cuda.synchronize()
+    ref = orc.run_config(cfg)
+    compare_groups(ions, ref, "cfg1 disc beam")
+    check_histogram(cfg, ions, counts, summary, ref)
+    y, z = _np(ions.a["y"]), _np(ions.a["z"])
+    assert np.hypot(y, z).max() <= 2.5e-3
+
+
+def test_time_dependent_field_against_an_independent_ode_solution(tg):
+    """Reading A3 through the product path (both tracers of kind-1 fields): two slices of uniform B_Z give a field
+    exactly linear in t, whose equations of motion scipy's DOP853 integrates to 1e-13; wrong stage times or a
+    frozen t move the hit by ~1e-4 m (tests/test_oracle_pins7.py has the same pin for the oracle)."""
+    from scipy.integrate import solve_ivp
+    from paper_2506_15812_b200 import taiga
+    B0, B1, DS = 1.0, 2.0, 1e-6
+    qm = wl.E_CHARGE / wl.MASS_LI7
+    v0 = math.sqrt(2 * 60e3 * qm)
+    grid, nodal = wl.nodal_field_time_slices(9, 17, 2)
+    grid.s0, grid.ds = 0.0, DS
+    nod = [np.zeros_like(nodal[0]) for _ in range(3)]
+    nod[1][0], nod[1][1] = B0, B1
+    det = wl.Detector((0.50, 0.0, 0.0), (-1.0, 0.0, 0.0), (0.0, 1.0, 0.0), (0.0, 0.0, 1.0),
+                      np.array([-1.0]), np.array([1.0]), np.array([-1.0]), np.array([1.0]))
+    t0s = np.array([0.0, 1.0e-7, 3.0e-7] * 43)
+    n = len(t0s)
+    tg.load_field(grid, nod)
+    for mma in (1, 0):
+        tg.set_option("mma", mma)
+        ions = taiga.Ions(n)
+        for k, val in (("x", 0.55), ("y", 0.0), ("z", 0.0), ("vx", v0), ("vy", 0.0), ("vz", 3.0e4)):
+            ions.a[k].fill_(val)
+        ions.a["t0"].copy_(torch.from_numpy(t0s))
+        dt = 2.5e-10
+        tg.trace(ions, qm, dt, 20000, det)
+        torch.cuda.synchronize()
+        assert np.all(_np(ions.cell) == -1)                       # crossed the plane (segment assigned by a5)
+        for i in range(3):
+            def rhs(t, y):
+                bz = B0 + (B1 - B0) * t / DS
+                return [y[3], y[4], y[5], qm * y[4] * bz, -qm * y[3] * bz, 0.0]
+            ev = lambda t, y: 0.50 - y[0]
+            ev.terminal, ev.direction = True, 1.0
+            sol = solve_ivp(rhs, (t0s[i], t0s[i] + 2e-6), [0.55, 0.0, 0.0, v0, 0.0, 3.0e4], method="DOP853",
+                            rtol=1e-13, atol=1e-16, events=ev)
+            ye = sol.y_events[0][0]
+            sel = np.arange(i, n, 3)
+            assert np.all(_np(ions.steps)[sel] == math.ceil((sol.t_events[0][0] - t0s[i]) / dt - 1e-9))
+            assert np.abs(_np(ions.hit_u)[sel] - ye[1]).max() < 5e-7 and np.abs(_np(ions.hit_w)[sel] - ye[2]).max() < 5e-7
+
+
 @pytest.mark.parametrize("kind", [0, 1, 2])
 def test_field_precompute_vs_oracle_tables(tg, kind):
     if kind == 0:
@@ -698,6 +770,9 @@ def test_error_paths_of_the_widened_entry_points(tg):
     assert float(ions.weight.min()) == 5.0
     # weighted histogram needs weights
     wc = torch.zeros((1, 8, 8), dtype=torch.int64, device="cuda"); ws = torch.zeros((1, 4), dtype=torch.int64, device="cuda")
+    with pytest.raises(taiga.TaigaError) as e:                # weights the last trace did not write (no loss model) are refused
+        t2.detector_histogram_weighted(ions, cfg.detector, 1, wc, ws)
+    assert e.value.code == taiga.E_STATE
     s = ions.struct(weight=False)
     assert s.w0 is None
     with pytest.raises(taiga.TaigaError):
