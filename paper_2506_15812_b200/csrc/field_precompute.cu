@@ -12,8 +12,6 @@
 // running the reduction above on unit vectors) and every node is then an independent 73-point
 // stencil: one thread per node, coalesced, exact to rounding.  One thread per (cell, component)
 // finally assembles the 16 power-basis coefficients from {y, y_zz, y_rr, y_rrzz} at 4 corners.
-#include <vector>
-
 #include "field_device.cuh"
 
 #define TG_BAND_W 36
@@ -32,38 +30,65 @@ __global__ void k_second_deriv(const double* __restrict__ y, double* __restrict_
     M[t] = acc;
 }
 
-// host: band of H for line length n (Thomas reduction applied to unit vectors)
-static std::vector<double> spline_band(int n) {
-    std::vector<double> band((size_t)(2 * TG_BAND_W + 1) * n, 0.0), cp(n, 0.0), M(n), y(n);
-    for (int i = 2; i <= n - 3; ++i) cp[i] = (i == 2) ? 0.25 : 1.0 / (4.0 - cp[i - 1]);
-    for (int q = 0; q < n; ++q) {
-        // response to y = e_q is non-negligible only for |i-q| <= W (+2 for the end rows); solve on a window
-        int lo = q - TG_BAND_W - 3, hi = q + TG_BAND_W + 3;
-        if (lo < 0) lo = 0;
-        if (hi > n - 1) hi = n - 1;
-        auto Y = [&](int i) { return i == q ? 1.0 : 0.0; };
-        auto d2 = [&](int i) { return (Y(i - 1) - 2.0 * Y(i)) + Y(i + 1); };
-        // full-length solve restricted to rows where the right-hand side can be non-zero is not
-        // possible for a tridiagonal system, so solve the whole line (O(n) per column, O(n^2) total)
-        double M1 = d2(1), Mn2 = d2(n - 2), dprev = 0.0;
-        std::fill(M.begin(), M.end(), 0.0);
-        M[1] = M1; M[n - 2] = Mn2;
-        for (int i = 2; i <= n - 3; ++i) {
-            double rhs = 6.0 * d2(i);
-            if (i == 2) rhs -= M1;
-            if (i == n - 3) rhs -= Mn2;
-            double dp = (i == 2) ? rhs * cp[i] : (rhs - dprev) * cp[i];
-            M[i] = dp; dprev = dp;
-        }
-        for (int i = n - 4; i >= 2; --i) M[i] = M[i] - cp[i] * M[i + 1];
-        M[0] = 2.0 * M[1] - M[2];
-        M[n - 1] = 2.0 * M[n - 2] - M[n - 3];
-        for (int i = lo; i <= hi; ++i) {
-            int d = q - i + TG_BAND_W;
-            if (d >= 0 && d <= 2 * TG_BAND_W) band[(size_t)d * n + i] = M[i];
-        }
+// Band of H for line length n, built on the device: thread q solves the system for y = e_q.  The response decays like
+// 0.268^|i-q|, so the tridiagonal solve runs on the window |i - q| <= W + TG_BAND_MARGIN only (M = 0 beyond it: an error
+// below 0.268^(W + margin) ~ 1e-35 of the diagonal on the rows that are kept); windows that reach a grid end use the
+// exact not-a-knot rows  M_1 = d2(1), M_0 = 2 M_1 - M_2  (and their mirror images).
+#define TG_BAND_MARGIN 24
+#define TG_BAND_WIN (2 * (TG_BAND_W + TG_BAND_MARGIN) + 8)
+__global__ void k_spline_band(double* __restrict__ band, int n) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= n) return;
+    const int lo = max(0, q - TG_BAND_W - TG_BAND_MARGIN), hi = min(n - 1, q + TG_BAND_W + TG_BAND_MARGIN);
+    double M[TG_BAND_WIN], cp[TG_BAND_WIN];
+    auto Y = [&](int i) { return i == q ? 1.0 : 0.0; };
+    auto d2 = [&](int i) { return (Y(i - 1) - 2.0 * Y(i)) + Y(i + 1); };
+    for (int i = lo; i <= hi; ++i) M[i - lo] = 0.0;
+    const double M1 = d2(1), Mn2 = d2(n - 2);                       // exact end rows (zero unless q is within 2 of that end)
+    const int a = max(lo, 2), b = min(hi, n - 3);                   // unknowns of the (1,4,1) rows
+    double dprev = 0.0, cprev = 0.0;
+    for (int i = a; i <= b; ++i) {                                  // Thomas, forward
+        double rhs = 6.0 * d2(i);
+        if (i == 2) rhs -= M1;
+        if (i == n - 3) rhs -= Mn2;
+        const double c = (i == a) ? 0.25 : 1.0 / (4.0 - cprev);
+        const double dp = (i == a) ? rhs * c : (rhs - dprev) * c;
+        cp[i - lo] = c; M[i - lo] = dp; dprev = dp; cprev = c;
     }
-    return band;
+    for (int i = b - 1; i >= a; --i) M[i - lo] = M[i - lo] - cp[i - lo] * M[i + 1 - lo];
+    if (lo <= 1 && 1 <= hi) M[1 - lo] = M1;
+    if (lo <= n - 2 && n - 2 <= hi) M[n - 2 - lo] = Mn2;
+    if (lo == 0) M[0] = 2.0 * M[1 - lo] - M[2 - lo];
+    if (hi == n - 1) M[n - 1 - lo] = 2.0 * M[n - 2 - lo] - M[n - 3 - lo];
+    for (int i = max(0, q - TG_BAND_W); i <= min(n - 1, q + TG_BAND_W); ++i)
+        band[(size_t)(q - i + TG_BAND_W) * n + i] = M[i - lo];
+}
+
+// band operator of one grid direction (ax 0: Z, 1: R), cached per line length; no host work, no synchronisation
+static int tg_ensure_band(taiga_ctx* ctx, int ax, int n) {
+    if (ctx->band_n[ax] == n) return TAIGA_OK;
+    size_t cap = ctx->band_cap[ax], need = (size_t)(2 * TG_BAND_W + 1) * n;
+    int rc = tg_reserve(ctx, &ctx->band[ax], &cap, need);
+    ctx->band_cap[ax] = cap;
+    if (rc) return rc;
+    TG_CUDA(ctx, cudaMemsetAsync(ctx->band[ax], 0, need * sizeof(double), ctx->stream));
+    k_spline_band<<<(n + 63) / 64, 64, 0, ctx->stream>>>(ctx->band[ax], n);
+    TG_CUDA(ctx, cudaGetLastError());
+    ctx->band_n[ax] = n;
+    return TAIGA_OK;
+}
+
+// kind 2: first column G of the inverse of the circulant (1,4,1) matrix of the periodic spline, closed form: with
+// r = sqrt(3) - 2 (root of r^2 + 4 r + 1) the infinite chain has g_k = r^|k| / (2 sqrt 3); summing the periodic images
+// gives G_k = (r^k + r^(n-k)) / ((1 - r^n) 2 sqrt 3).
+__global__ void k_circulant_inverse_col(double* __restrict__ G, int n) {
+    if (blockIdx.x || threadIdx.x) return;
+    const double s3 = sqrt(3.0), r = s3 - 2.0;
+    double rn = 1.0;
+    for (int k = 0; k < n; ++k) rn *= r;
+    const double norm = 1.0 / ((1.0 - rn) * 2.0 * s3);
+    double up = 1.0, dn = rn;                                       // r^k, r^(n-k)
+    for (int k = 0; k < n; ++k) { G[k] = (up + dn) * norm; up *= r; dn /= r; }
 }
 
 // power-basis coefficients of one interval from end values g0,g1 and end second derivatives G0,G1
@@ -156,26 +181,6 @@ __global__ void k_field_eval(FieldDev f, unsigned long long n, const double* R, 
     BR[i] = a; BZ[i] = b; Bp[i] = c;
 }
 
-// first column of inverse of circulant(4,1,0,...,0,1), by Gaussian elimination (n <= 128)
-static std::vector<double> circulant_inverse_col(int n) {
-    std::vector<double> A((size_t)n * n, 0.0), x(n, 0.0);
-    for (int i = 0; i < n; ++i) { A[(size_t)i * n + i] += 4.0; A[(size_t)i * n + (i + 1) % n] += 1.0; A[(size_t)i * n + (i + n - 1) % n] += 1.0; }
-    x[0] = 1.0;
-    for (int c = 0; c < n; ++c)                   // diagonally dominant: no pivoting needed
-        for (int r = c + 1; r < n; ++r) {
-            double f = A[(size_t)r * n + c] / A[(size_t)c * n + c];
-            if (f == 0.0) continue;
-            for (int k = c; k < n; ++k) A[(size_t)r * n + k] -= f * A[(size_t)c * n + k];
-            x[r] -= f * x[c];
-        }
-    for (int r = n - 1; r >= 0; --r) {
-        double s = x[r];
-        for (int k = r + 1; k < n; ++k) s -= A[(size_t)r * n + k] * x[k];
-        x[r] = s / A[(size_t)r * n + r];
-    }
-    return x;
-}
-
 // kind 1: D[cell][k] = T[cell][k+1] - T[cell][k], so that B(t) = H(T_k) + tau H(D_k) and the tracer can keep
 // T_k in registers and gather only D_k (half the bytes of gathering both slices)
 __global__ void k_slice_diff(const double* __restrict__ T, double* __restrict__ D, long long ncell, int nS) {
@@ -234,25 +239,9 @@ int tg_precompute(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c) {
         if (rc) return rc;
         double *y = ctx->scratch, *Mz = y + 3 * nnode, *Myr = Mz + 3 * nnode, *Mzr = Myr + 3 * nnode;
         double *tmp = Mzr + 3 * nnode, *G = tmp + n_tmp;
-        // band operators, cached per line length
-        for (int ax = 0; ax < 2; ++ax) {
-            int n = ax ? nR : nZ;
-            if (ctx->band_n[ax] != n) {
-                std::vector<double> b = spline_band(n);
-                size_t cap = ctx->band_cap[ax];
-                rc = tg_reserve(ctx, &ctx->band[ax], &cap, b.size());
-                ctx->band_cap[ax] = cap;
-                if (rc) return rc;
-                TG_CUDA(ctx, cudaMemcpyAsync(ctx->band[ax], b.data(), b.size() * sizeof(double), cudaMemcpyHostToDevice, st));
-                TG_CUDA(ctx, cudaStreamSynchronize(st));
-                ctx->band_n[ax] = n;
-            }
-        }
-        if (g->kind == 2) {
-            std::vector<double> Gh = circulant_inverse_col(nS);
-            TG_CUDA(ctx, cudaMemcpyAsync(G, Gh.data(), nS * sizeof(double), cudaMemcpyHostToDevice, st));
-            TG_CUDA(ctx, cudaStreamSynchronize(st));
-        }
+        // band operators, cached per line length (device-built)
+        for (int ax = 0; ax < 2; ++ax) { rc = tg_ensure_band(ctx, ax, ax ? nR : nZ); if (rc) return rc; }
+        if (g->kind == 2) k_circulant_inverse_col<<<1, 32, 0, st>>>(G, nS);
         for (int m = 0; m < 3; ++m)
             TG_CUDA(ctx, cudaMemcpyAsync(y + (size_t)m * nnode, src[m], nnode * sizeof(double),
                                          c->on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
@@ -313,19 +302,7 @@ int tg_load_loss(taiga_ctx* ctx, const double* psi_nodal, int on_device, const t
     ctx->scratch_bytes = scap * sizeof(double);
     if (rc) return rc;
     double *y = ctx->scratch, *Mz = y + nnode, *Myr = Mz + nnode, *Mzr = Myr + nnode, *pne = Mzr + nnode, *pte = pne + prof->n;
-    for (int ax = 0; ax < 2; ++ax) {                 // band operators (normally cached by load_field)
-        int n = ax ? nR : nZ;
-        if (ctx->band_n[ax] != n) {
-            std::vector<double> b = spline_band(n);
-            size_t cap = ctx->band_cap[ax];
-            rc = tg_reserve(ctx, &ctx->band[ax], &cap, b.size());
-            ctx->band_cap[ax] = cap;
-            if (rc) return rc;
-            TG_CUDA(ctx, cudaMemcpyAsync(ctx->band[ax], b.data(), b.size() * sizeof(double), cudaMemcpyHostToDevice, st));
-            TG_CUDA(ctx, cudaStreamSynchronize(st));
-            ctx->band_n[ax] = n;
-        }
-    }
+    for (int ax = 0; ax < 2; ++ax) { rc = tg_ensure_band(ctx, ax, ax ? nR : nZ); if (rc) return rc; }   // normally cached by load_field
     TG_CUDA(ctx, cudaMemcpyAsync(y, psi_nodal, nnode * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
     TG_CUDA(ctx, cudaMemcpyAsync(pne, prof->ne_m3, prof->n * sizeof(double), cudaMemcpyHostToDevice, st));
     TG_CUDA(ctx, cudaMemcpyAsync(pte, prof->Te_eV, prof->n * sizeof(double), cudaMemcpyHostToDevice, st));

@@ -36,7 +36,9 @@
 // Per-warp exchange buffer, rows of TG_ROW doubles indexed by the slot of an ion's own lane:
 //   rows 0..7   A operands [s * 4 + t] = w^t q^(2s)        row 8   q (kind 2) / tau (kind 1)
 //   rows 9..20  results f[m * 4 + t]
-struct __align__(16) TgWarpBuf { double v[21 * TG_ROW + 1]; };
+// followed by the work list of the current evaluation: 32 descriptors {cell, member lanes, 8 g, -}.
+#define TG_LIST_OFF ((21 * TG_ROW + 1) * 8)
+struct __align__(16) TgWarpBuf { double v[21 * TG_ROW + 1]; int4 list[32]; };
 
 // Shared-memory addresses of one lane, computed once per kernel: ptxas otherwise rematerialises them from
 // %tid / the CTA's window base inside the item loop (60 integer instructions per 6 DMMAs in the r2a profile).
@@ -45,11 +47,20 @@ struct TgLane {
     unsigned quad;                                // &v[t * TG_ROW + slot of lane 4r]     (+ 8 g: column of ion (g, r), row t)
     unsigned qrow;                                // &v[8 * TG_ROW + slot of lane 4r]
     unsigned bit0;                                // 1 << 4r: bit of ion (0, r) in a lane mask
+    unsigned list;                                // the warp's work list
+    unsigned lane;
     const double* frag;                           // fragment table + lane
 };
 
 __device__ __forceinline__ double tg_lds(unsigned a) { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a)); return v; }
 __device__ __forceinline__ void tg_sts(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
+__device__ __forceinline__ void tg_lds4(unsigned a, int& x, unsigned& y, unsigned& z) {
+    int w;
+    asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(x), "=r"(y), "=r"(z), "=r"(w) : "r"(a));
+}
+__device__ __forceinline__ void tg_sts4(unsigned a, int x, unsigned y, unsigned z) {
+    asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%3};" ::"r"(a), "r"(x), "r"(y), "r"(z) : "memory");
+}
 
 __device__ __forceinline__ void tg_dmma(double& d0, double& d1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
@@ -77,9 +88,10 @@ __device__ __forceinline__ int tg_locate_cell(const FieldDev& f, double X, doubl
 }
 
 // Warp-collective evaluation: every lane calls it; cell < 0 = this lane has no ion to evaluate.
-// Work items = (cell, group) pairs: the ions of one group (lanes 4r + g) that sit in one cell.  The operands of
-// item i+1 are fetched right after the DMMAs of item i have issued (DMMA reads its registers at issue), so their
-// latency overlaps the tensor pipe.
+// Work items = (cell, group) pairs: the ions of one group (lanes 4r + g) that sit in one cell.  The whole list of an
+// evaluation is built up front from one match.any (lanes in the same cell) and one ballot (the lowest lane of each
+// pair writes its descriptor), so the DMMA loop carries no vote / shuffle chain; descriptors and operands are fetched
+// one item ahead, into the registers the issued DMMAs have already read.
 template <int KIND>
 __device__ __forceinline__ void tg_eval_mma(const TgLane& L, int cell, double p, double w, double q,
                                             double& BR, double& BZ, double& Bp, unsigned& sets) {
@@ -95,16 +107,17 @@ __device__ __forceinline__ void tg_eval_mma(const TgLane& L, int cell, double p,
         }
         tg_sts(L.own + 8 * TG_ROWB, q);
     }
+    const unsigned mine_g = __match_any_sync(FULL, cell) & (0x11111111u << (L.lane & 3));   // my (cell, group) pair
+    const bool lead = cell >= 0 && (mine_g & (0u - mine_g)) == (1u << L.lane);            // its lowest lane
+    const unsigned leaders = __ballot_sync(FULL, lead);
+    if (lead) tg_sts4(L.list + 16 * __popc(leaders & ((1u << L.lane) - 1u)), cell, mine_g, (L.lane & 3) * 8);
     __syncwarp();
-    unsigned todo = __ballot_sync(FULL, cell >= 0);
+    const int n_items = __popc(leaders);
+    sets += n_items;
     double b[KS][3], a[KS], qg = 0.0;
+    int cs = 0;
     unsigned mem = 0, gofs = 0;
-    auto fetch = [&]() {                          // next item of `todo`: group and cell of its lowest lane
-        const int lead = __ffs(todo) - 1;
-        const int cs = __shfl_sync(FULL, cell, lead);
-        const unsigned g = lead & 3;
-        mem = __ballot_sync(FULL, cell == cs) & (0x11111111u << g) & todo;
-        gofs = g * 8;
+    auto operands = [&]() {
         const double* src = L.frag + (size_t)cs * (KS * 96);
 #pragma unroll
         for (int s = 0; s < KS; ++s)
@@ -114,8 +127,10 @@ __device__ __forceinline__ void tg_eval_mma(const TgLane& L, int cell, double p,
         for (int s = 0; s < KS; ++s) a[s] = tg_lds(L.quad + gofs + s * 4 * TG_ROWB);
         qg = tg_lds(L.qrow + gofs);
     };
-    if (todo) fetch();
-    while (mem) {                                 // warp-uniform
+    if (n_items) { tg_lds4(L.list, cs, mem, gofs); operands(); }
+    for (int i = 0; i < n_items; ++i) {           // warp-uniform
+        int cs2 = 0; unsigned mem2 = 0, gofs2 = 0;
+        if (i + 1 < n_items) tg_lds4(L.list + 16 * (i + 1), cs2, mem2, gofs2);
         double d[3][2];
 #pragma unroll
         for (int m = 0; m < 3; ++m) { d[m][0] = 0.0; d[m][1] = 0.0; }
@@ -123,13 +138,11 @@ __device__ __forceinline__ void tg_eval_mma(const TgLane& L, int cell, double p,
         for (int s = 0; s < KS; ++s)
 #pragma unroll
             for (int m = 0; m < 3; ++m) tg_dmma(d[m][0], d[m][1], a[s], b[s][m]);
-        ++sets;
         const double qc = qg;
         const bool mine = mem & (L.bit0 << (gofs >> 3));       // the ion of my row is served by this item
         const unsigned o = L.quad + 9 * TG_ROWB + gofs;
-        todo &= ~mem;
-        mem = 0;
-        if (todo) fetch();
+        cs = cs2; mem = mem2; gofs = gofs2;
+        if (i + 1 < n_items) operands();
         if (mine) {
 #pragma unroll
             for (int m = 0; m < 3; ++m) tg_sts(o + m * 4 * TG_ROWB, fma(qc, d[m][1], d[m][0]));
@@ -168,6 +181,8 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
         L.quad = wb + t4 * TG_ROWB + slot0 * 8;
         L.qrow = wb + 8 * TG_ROWB + slot0 * 8;
         L.bit0 = 1u << (lane & ~3);
+        L.list = wb + TG_LIST_OFF;
+        L.lane = (unsigned)lane;
         L.frag = P.frag + lane;
     }
 
@@ -420,7 +435,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
     }
     if (lane == 0) {
         atomicAdd(&P.counters[1], warp_steps);
-        atomicAdd(&P.counters[2], rl >> 5);        // every lane counted the warp's sets
+        atomicAdd(&P.counters[2], rl >> 5);        // every lane counted the warp's items
         atomicAdd(&P.counters[3], is);
     }
 }
