@@ -54,7 +54,7 @@ extern "C" int taiga_destroy(taiga_ctx* ctx) {
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     void* bufs[] = {ctx->table, ctx->scratch, ctx->band[0], ctx->band[1], ctx->cdf_depth, ctx->cdf_normal, ctx->edges, ctx->order,
-                    ctx->bins, ctx->counters, ctx->table32, ctx->psi_table, ctx->loss_rate, ctx->dtable, ctx->frag};
+                    ctx->bins, ctx->counters, ctx->table32, ctx->psi_table, ctx->loss_rate, ctx->dtable, ctx->frag, ctx->phi_tab};
     for (void* b : bufs) if (b) cudaFree(b);
     if (ctx->counters_host) cudaFreeHost(ctx->counters_host);
     if (ctx->stage) cudaFreeHost(ctx->stage);

@@ -47,6 +47,7 @@ struct taiga_ctx {
     double* table;            size_t table_bytes;
     double* scratch;          size_t scratch_bytes;     // precompute work arrays
     double* dtable;           size_t cap_dtable;   bool dtable_valid;    // kind 1: slice differences (built on first use)
+    double* phi_tab;          size_t cap_phi_tab;  int phi_tab_n; double phi_tab_s0;   // kind 2: plane directions (trace_mma.cu)
     double* frag;             size_t cap_frag;     bool frag_valid;      // kinds 1, 2: table in DMMA B-fragment order (trace_mma.cu)
     float* table32;           size_t cap_table32;  bool table32_valid;   // fp32 copy of a kind-2 table
     double* band[2];          size_t band_cap[2]; int band_n[2];   // y -> y'' band operators (Z, R)

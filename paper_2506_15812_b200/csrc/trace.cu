@@ -589,7 +589,7 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     TraceParams P;
     P.f = ctx->field; P.det = det;
     P.loss = ctx->loss; P.hdt = 0.5 * dt; P.weight = ions->weight; P.w0 = ions->w0;
-    P.frag = nullptr; P.key_shift = 0; P.refill_cta = 0;
+    P.frag = nullptr; P.key_shift = 0; P.refill_cta = 0; P.phi_tab = nullptr; P.phi_n = 0;
     if (f32) {                                 // fp32 field evaluation (BASELINE config 5 "fp32 variant")
         if (!ctx->table32_valid) {
             size_t n = (size_t)ctx->field.nS * ctx->field.cR * ctx->field.cZ * 192;

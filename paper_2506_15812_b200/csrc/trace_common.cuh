@@ -29,6 +29,8 @@ struct TraceParams {
     const double* frag;               // kinds 1, 2: the table in DMMA B-fragment order (trace_mma.cu)
     int key_shift;                    // regroup sort key = cell >> key_shift (< 2^23)
     int refill_cta;                   // trace_mma: refill the CTA's free lanes once this many are free
+    const double2* phi_tab;           // kind 2, trace_mma: (cos, sin) of the lower plane of each of the phi_n toroidal cells
+    int phi_n;
 };
 
 #define TG_GRAZE 1e-9

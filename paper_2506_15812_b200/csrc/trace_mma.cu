@@ -87,6 +87,43 @@ __device__ __forceinline__ int tg_locate_cell(const FieldDev& f, double X, doubl
     }
 }
 
+// Kind 2 without atan2.  The ion carries K, the global index of the toroidal cell it is in (K ds <= phi - s0 < (K+1) ds,
+// NK = 2 pi / ds cells around the torus), and (c0, s0) = (cos, sin) of that cell's lower plane from a host-built table.
+// For a point (X, Y) the angle past the plane is small, delta = asin((Y c0 - X s0) / R) with |delta| <~ ds, so
+// q = delta / ds is a 4-term series in s = (Y c0 - X s0) / R (1/R is needed anyway): 10 FP64 instructions instead of the
+// ~65 of atan2 + modulo.  A point beyond the cell moves K (and the frame) by floor(q) and is evaluated again.
+struct TgTor { int K, k; double c0, s0; };       // k = K mod nS: plane index of the table
+
+__device__ __forceinline__ void tg_tor_set(const TraceParams& P, TgTor& T, int K) {
+    T.K = K; T.k = K % P.f.nS;
+    const double2 cs = __ldg(P.phi_tab + K);
+    T.c0 = cs.x; T.s0 = cs.y;
+}
+// K of a point from scratch (ion load): the definition, with atan2
+__device__ __forceinline__ int tg_tor_K(const TraceParams& P, double X, double Y) {
+    double xs = (atan2(Y, X) - P.f.s0) * P.f.inv_ds;
+    xs = xs - (double)P.phi_n * floor(xs / (double)P.phi_n);
+    return tg_clampi(__double2int_rd(xs), 0, P.phi_n - 1);
+}
+__device__ __forceinline__ int tg_locate_tor(const TraceParams& P, TgTor& T, double X, double Y, double Z, double R, double rinv,
+                                             double& p, double& w, double& q) {
+    const FieldDev& f = P.f;
+    int i = tg_locate(R, f.inv_hR, f.offR, f.cR, p);
+    int j = tg_locate(Z, f.inv_hZ, f.offZ, f.cZ, w);
+#pragma unroll 1
+    for (int it = 0;; ++it) {
+        const double s = fma(Y, T.c0, -(X * T.s0)) * rinv, s2 = s * s;
+        q = (s * fma(s2, fma(s2, fma(s2, 15.0 / 336.0, 3.0 / 40.0), 1.0 / 6.0), 1.0)) * f.inv_ds;   // asin(s) / ds
+        if (tg_in01(q)) break;
+        if (it == 3) { q = fmin(fmax(q, 0.0), 0x1.fffffffffffffp-1); break; }   // on a plane to rounding: either side evaluates the same (C2 spline)
+        if (!(fabs(q) < 4.0)) { tg_tor_set(P, T, tg_tor_K(P, X, Y)); continue; }  // far off (never for steps shorter than a cell): from scratch
+        int K = T.K + __double2int_rd(q);
+        K = K < 0 ? K + P.phi_n : (K >= P.phi_n ? K - P.phi_n : K);
+        tg_tor_set(P, T, K);
+    }
+    return (T.k * f.cR + i) * f.cZ + j;
+}
+
 // Warp-collective evaluation: every lane calls it; cell < 0 = this lane has no ion to evaluate.
 // Work items = (cell, group) pairs: the ions of one group (lanes 4r + g) that sit in one cell.  The whole list of an
 // evaluation is built up front from one match.any (lanes in the same cell) and one ballot (the lowest lane of each
@@ -168,7 +205,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
     const unsigned FULL = 0xffffffffu;
     __shared__ TgWarpBuf s_wb[NW];
     __shared__ double sh_d[ND][THREADS];
-    __shared__ uint32_t sh_u[3][THREADS];
+    __shared__ uint32_t sh_u[KIND == 2 ? 4 : 3][THREADS];
     __shared__ __align__(16) int sh_key[THREADS];
     __shared__ unsigned long long s_base;
     __shared__ int s_wcnt[NW];
@@ -190,6 +227,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
     double Lam = 0.0, nu0 = 0.0;
     uint32_t idx = 0, nst = 0;
     bool alive = false, exhausted = false;
+    [[maybe_unused]] TgTor T = {0, 0, 1.0, 0.0};
     unsigned sets = 0, ion_steps = 0;
     unsigned long long warp_steps = 0;
     int since = 0;
@@ -201,7 +239,8 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
         if (alive) {
             double R2 = fma(Xs, Xs, Ys * Ys);
             rinv = tg_rsqrt(R2); Rs = R2 * rinv;
-            cell = tg_locate_cell<KIND>(P.f, Xs, Ys, Zs, Rs, ts, p, w, q);
+            if constexpr (KIND == 2) cell = tg_locate_tor(P, T, Xs, Ys, Zs, Rs, rinv, p, w, q);
+            else cell = tg_locate_cell<KIND>(P.f, Xs, Ys, Zs, Rs, ts, p, w, q);
         }
         tg_eval_mma<KIND>(L, cell, p, w, q, BR, BZ, Bp, sets);
         if (alive) { tg_rotate(Xs, Ys, rinv, BR, Bp, bx, by); bz = BZ; }
@@ -230,6 +269,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
                     if constexpr (LOSS) Lam = 0.0;
                     s0 = fma(P.det.normal[0], X, fma(P.det.normal[1], Y, fma(P.det.normal[2], Z, -P.nrD)));
                     alive = true;
+                    if constexpr (KIND == 2) tg_tor_set(P, T, tg_tor_K(P, X, Y));
                     if (!(s0 < 0.0)) {             // O4: must start in front of the plane
                         P.hit_u[idx] = 0.0; P.hit_w[idx] = 0.0; P.cell[idx] = TAIGA_CELL_BADSTART; P.steps[idx] = 0;
                         P.flags[idx] = (fabs(s0) < TG_GRAZE) ? TAIGA_FLAG_PLANE : 0;
@@ -242,7 +282,12 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
             int key = TG_KEY_DEAD;
             if (alive) {
                 double p_, w_, q_;
-                int c = tg_locate_cell<KIND>(P.f, X, Y, Z, sqrt(fma(X, X, Y * Y)), t, p_, w_, q_) >> P.key_shift;
+                int c;
+                if constexpr (KIND == 2) {         // the toroidal cell the ion carries (at most one evaluation old)
+                    const int ci = tg_locate(sqrt(fma(X, X, Y * Y)), P.f.inv_hR, P.f.offR, P.f.cR, p_);
+                    const int cj = tg_locate(Z, P.f.inv_hZ, P.f.offZ, P.f.cZ, w_);
+                    c = ((T.k * P.f.cR + ci) * P.f.cZ + cj) >> P.key_shift;
+                } else c = tg_locate_cell<KIND>(P.f, X, Y, Z, sqrt(fma(X, X, Y * Y)), t, p_, w_, q_) >> P.key_shift;
                 key = c < TG_KEY_DEAD - 1 ? c : TG_KEY_DEAD - 1;
             }
             const int mykey = (key << 8) | tid;
@@ -261,11 +306,13 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
             sh_d[6][dst] = t; sh_d[7][dst] = s0;
             if constexpr (LOSS) { sh_d[8][dst] = Lam; sh_d[9][dst] = nu0; }
             sh_u[0][dst] = idx; sh_u[1][dst] = nst; sh_u[2][dst] = alive ? 1u : 0u;
+            if constexpr (KIND == 2) sh_u[3][dst] = (uint32_t)T.K;
             __syncthreads();
             X = sh_d[0][tid]; Y = sh_d[1][tid]; Z = sh_d[2][tid]; Ux = sh_d[3][tid]; Uy = sh_d[4][tid]; Uz = sh_d[5][tid];
             t = sh_d[6][tid]; s0 = sh_d[7][tid];
             if constexpr (LOSS) { Lam = sh_d[8][tid]; nu0 = sh_d[9][tid]; }
             idx = sh_u[0][tid]; nst = sh_u[1][tid]; alive = sh_u[2][tid] != 0u;
+            if constexpr (KIND == 2) tg_tor_set(P, T, (int)sh_u[3][tid]);
         }
         since = (since + 1 >= P.regroup_every) ? 0 : since + 1;
         if (__ballot_sync(FULL, alive) == 0) continue;        // this warp idles until the next sync point
@@ -476,12 +523,38 @@ int tg_build_frag(taiga_ctx* ctx) {
     return TAIGA_OK;
 }
 
+// Number of toroidal cells around the torus, NK = 2 pi / ds, when the planes close on themselves (NK an integer multiple
+// of nS: the period nS ds divides 2 pi); 0 otherwise (then phi has a seam at +-pi and the kernel is not offered).
+static int tg_phi_cells(const FieldDev& f) {
+    const double nk = 6.283185307179586476925286766559 * f.inv_ds;
+    const long long r = llround(nk);
+    if (r < f.nS || r > (1 << 20) || fabs(nk - (double)r) > 1e-9 * nk || r % f.nS != 0) return 0;
+    return (int)r;
+}
+
 // Is the cooperative kernel offered for this field?  (cell ids are 32-bit; 2 slices / planes at least)
 bool tg_mma_supported(const taiga_ctx* ctx) {
     const FieldDev& f = ctx->field;
     if (f.kind != 1 && f.kind != 2) return false;
     const long long ncell = (long long)f.cR * f.cZ * f.nS;
+    if (f.kind == 2 && tg_phi_cells(f) == 0) return false;
     return ncell < (1ll << 31) && f.nS >= 2;
+}
+
+// (cos, sin) of the lower plane of every toroidal cell, host libm, staged like the other small tables
+static int tg_build_phi_tab(taiga_ctx* ctx, int nk) {
+    if (ctx->phi_tab_n == nk && ctx->phi_tab_s0 == ctx->field.s0 && ctx->phi_tab) return TAIGA_OK;
+    int rc = tg_reserve(ctx, &ctx->phi_tab, &ctx->cap_phi_tab, (size_t)2 * nk);
+    if (rc) return rc;
+    rc = tg_stage(ctx, (size_t)2 * nk * sizeof(double));
+    if (rc) return rc;
+    double* h = (double*)ctx->stage;
+    const double ds = 1.0 / ctx->field.inv_ds;
+    for (int K = 0; K < nk; ++K) { const double a = ctx->field.s0 + (double)K * ds; h[2 * K] = cos(a); h[2 * K + 1] = sin(a); }
+    TG_CUDA(ctx, cudaMemcpyAsync(ctx->phi_tab, h, (size_t)2 * nk * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    TG_CUDA(ctx, cudaEventRecord(ctx->stage_done, ctx->stream));
+    ctx->phi_tab_n = nk; ctx->phi_tab_s0 = ctx->field.s0;
+    return TAIGA_OK;
 }
 
 // Launch geometry: THREADS per CTA (the pool the CTA re-sorts; 32 = every warp on its own, no CTA barrier) and the
@@ -507,6 +580,13 @@ int tg_trace_mma(taiga_ctx* ctx, TraceParams& P, int solver, bool hasE, bool los
     if (rc) return rc;
     const FieldDev& f = ctx->field;
     P.frag = ctx->frag;
+    P.phi_tab = nullptr; P.phi_n = 0;
+    if (f.kind == 2) {
+        P.phi_n = tg_phi_cells(f);
+        rc = tg_build_phi_tab(ctx, P.phi_n);
+        if (rc) return rc;
+        P.phi_tab = (const double2*)ctx->phi_tab;
+    }
     long long ncell = (f.kind == 2) ? (long long)f.cR * f.cZ * f.nS : (long long)f.cR * f.cZ * (f.nS - 1);
     P.key_shift = 0;
     while ((ncell >> P.key_shift) >= TG_KEY_DEAD - 1) ++P.key_shift;
