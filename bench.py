@@ -47,6 +47,8 @@ def parse():
     ap.add_argument("--oracle-sample", type=int, default=131072)
     ap.add_argument("--solver", type=int, default=0, help="0 RKN (default, the metric), 1 printed-k3 RKN, 2 RK4, 3/4 Boris")
     ap.add_argument("--opt", action="append", default=[], help="key=value for taiga_set_option")
+    ap.add_argument("--detector", default="config", choices=["config", "gapped"],
+                    help="gapped: the config's matrix with non-uniform segments and gaps (PAPER.md L330; binary-search path of a5)")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = every rank traces the config's ions (default), strong = the config's ions are split")
     ap.add_argument("--oracle-full", action="store_true", help="time the oracle ONCE on the full config (16 threads and 1 thread on a prefix) and exit")
@@ -188,6 +190,12 @@ def main_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     from paper_2506_15812_b200 import taiga
     dev = "cuda:%d" % local
+    if args.detector == "gapped":
+        if cfg.detector is not None:
+            cfg.detector = wl.gapped_detector(cfg.detector)
+        for g in cfg.groups:
+            if g.detector is not None:
+                g.detector = wl.gapped_detector(g.detector)
     grid, nodal = cfg.field_builder()
     nodal_dev = [torch.from_numpy(np.ascontiguousarray(c)).to(dev) for c in nodal]
     nodal_pin = [torch.from_numpy(np.ascontiguousarray(c)).pin_memory() for c in nodal]
@@ -208,7 +216,7 @@ def main_ours(args):
     cd, cn = wl.depth_cdf(), wl.normal_cdf()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
     ev = lambda: torch.cuda.Event(enable_timing=True)
-    trace_ms = []
+    trace_ms, hist_ms = [], []
 
     def step(host, record=False):
         if host:
@@ -236,11 +244,12 @@ def main_ours(args):
         else:
             for v, g in spans:
                 tg.detector_histogram(v, g.detector, cfg.n_hist, counts, summary)
+        e2 = ev(); e2.record()
         sharding.allreduce_counters(dist, counts, summary)                               # exchange step: <= 0.5 MB
         if host:
             counts_pin.copy_(counts, non_blocking=True); summary_pin.copy_(summary, non_blocking=True)
         if record:
-            trace_ms.append((e0, e1))
+            trace_ms.append((e0, e1)); hist_ms.append((e1, e2))
 
     def barrier():
         if world > 1:
@@ -300,6 +309,8 @@ def main_ours(args):
                    "ion_steps_per_step": ion_steps, "ions_per_step": n_ions, "invariant_counts_sum_to_n": s_ok},
         "ions_per_s": n_ions * args.steps / (total_ms * 1e-3),
         "trace_kernel": {"ms": t_trace, "ion_steps_per_s": ion_steps_rank / (t_trace * 1e-3)},
+        "histogram_kernel": {"ms": sum(a.elapsed_time(b) for a, b in hist_ms) / len(hist_ms), "detector": args.detector,
+                             "hits_in_segments": int(summary[:, 0].sum().item()), "hits_in_gaps_or_outside": int(summary[:, 1].sum().item())},
         "e2e": {"value": ion_steps * args.steps / (total_ms_e2e * 1e-3), "unit": "ion-steps/s",
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": total_ms_e2e / args.steps,
                 "timing": "host wall clock around the C-ABI calls incl. pinned H2D of the nodal field and D2H of the counters"},

@@ -2,21 +2,23 @@
 // has no FP64 entry, so the FP64 issue rate is measured in the same run as the benchmark).
 #include "taiga_internal.h"
 
-// Four independent chains per thread, each with its own multiplicand and addend registers: eight chains sharing
-// two operand registers (the round-1 kernel) reach only 0.91 of 148 x 64 DFMA/clk because of register-bank
-// conflicts on the shared operands; this form measures 0.98-0.99 at 8-32 warps per SM (profiles/r2a_microbench.md).
+// Four independent chains per thread, each with its own multiplicand register and one shared addend: measures
+// 0.98-0.99 of 148 x 64 DFMA/clk at 8-32 warps per SM (profiles/r2a_microbench.md).  Two other forms fall short of the
+// issue limit and are NOT the roofline: eight chains sharing both operands (the round-1 kernel: 0.91, register-bank
+// conflicts on the shared pair) and chains with three distinct source registers (0.67: a DFMA reading three different
+// 64-bit registers is limited by register-file bandwidth).
 #define PEAK_CHAINS 4
 #define PEAK_INNER 64
 
-__global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters, double a0, double b0) {
-    double v[PEAK_CHAINS], a[PEAK_CHAINS], b[PEAK_CHAINS];
+__global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters, double a0, double b) {
+    double v[PEAK_CHAINS], a[PEAK_CHAINS];
 #pragma unroll
-    for (int c = 0; c < PEAK_CHAINS; ++c) { v[c] = (double)(threadIdx.x + c) * 1e-3; a[c] = a0 + c * 1e-9; b[c] = b0 + c * 1e-12; }
+    for (int c = 0; c < PEAK_CHAINS; ++c) { v[c] = (double)(threadIdx.x + c) * 1e-3; a[c] = a0 + c * 1e-9; }
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
         for (int k = 0; k < PEAK_INNER; ++k) {
 #pragma unroll
-            for (int c = 0; c < PEAK_CHAINS; ++c) v[c] = fma(v[c], a[c], b[c]);
+            for (int c = 0; c < PEAK_CHAINS; ++c) v[c] = fma(v[c], a[c], b);
         }
     }
     double s = 0.0;

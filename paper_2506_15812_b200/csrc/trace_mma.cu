@@ -203,10 +203,15 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
     constexpr int NW = THREADS / 32;
     constexpr int ND = LOSS ? 10 : 8;
     const unsigned FULL = 0xffffffffu;
-    __shared__ TgWarpBuf s_wb[NW];
-    __shared__ double sh_d[ND][THREADS];
-    __shared__ uint32_t sh_u[KIND == 2 ? 4 : 3][THREADS];
-    __shared__ __align__(16) int sh_key[THREADS];
+    // the warp buffers (evaluation) and the exchange arrays of the CTA sync point (refill + re-sort) are never live at
+    // the same time: one allocation, so that more of the SM's 256 KB stays L1 for the fragment table
+    constexpr size_t EXCH_BYTES = (size_t)ND * THREADS * 8 + (size_t)(KIND == 2 ? 4 : 3) * THREADS * 4 + (size_t)THREADS * 4;
+    constexpr size_t SMEM_BYTES = sizeof(TgWarpBuf) * NW > EXCH_BYTES ? sizeof(TgWarpBuf) * NW : EXCH_BYTES;
+    __shared__ __align__(16) unsigned char s_raw[SMEM_BYTES];
+    TgWarpBuf* s_wb = reinterpret_cast<TgWarpBuf*>(s_raw);
+    double (*sh_d)[THREADS] = reinterpret_cast<double (*)[THREADS]>(s_raw);
+    uint32_t (*sh_u)[THREADS] = reinterpret_cast<uint32_t (*)[THREADS]>(s_raw + (size_t)ND * THREADS * 8);
+    int* sh_key = reinterpret_cast<int*>(s_raw + (size_t)ND * THREADS * 8 + (size_t)(KIND == 2 ? 4 : 3) * THREADS * 4);
     __shared__ unsigned long long s_base;
     __shared__ int s_wcnt[NW];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -251,7 +256,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
             int nalive = __syncthreads_count(alive);
             if (nalive == 0 && exhausted) break;
             const int nfree = THREADS - nalive;
-            if (!exhausted && nfree >= P.refill_cta) {
+            if (!exhausted && nfree >= (P.refill_cta < THREADS ? P.refill_cta : THREADS)) {
                 unsigned dm = __ballot_sync(FULL, !alive);
                 if (lane == 0) s_wcnt[warp] = __popc(dm);
                 if (tid == 0) s_base = atomicAdd(&P.counters[0], (unsigned long long)nfree);
@@ -313,6 +318,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
             if constexpr (LOSS) { Lam = sh_d[8][tid]; nu0 = sh_d[9][tid]; }
             idx = sh_u[0][tid]; nst = sh_u[1][tid]; alive = sh_u[2][tid] != 0u;
             if constexpr (KIND == 2) tg_tor_set(P, T, (int)sh_u[3][tid]);
+            __syncthreads();                   // the exchange arrays share their memory with the warp buffers
         }
         since = (since + 1 >= P.regroup_every) ? 0 : since + 1;
         if (__ballot_sync(FULL, alive) == 0) continue;        // this warp idles until the next sync point
@@ -591,7 +597,7 @@ int tg_trace_mma(taiga_ctx* ctx, TraceParams& P, int solver, bool hasE, bool los
     P.key_shift = 0;
     while ((ncell >> P.key_shift) >= TG_KEY_DEAD - 1) ++P.key_shift;
     if (P.regroup_every < 1) P.regroup_every = 8;
-    P.refill_cta = ctx->opt_refill_cta > 0 ? ctx->opt_refill_cta : 16;
+    P.refill_cta = ctx->opt_refill_cta > 0 ? ctx->opt_refill_cta : 1024;      // default: whole-CTA tiles (clamped to THREADS in the kernel)
     const int per_sm = ctx->opt_ctas_per_sm;
     cudaStream_t st = ctx->stream;
 #define TG_MMA(K, S, E, L, B, ...) rc = tg_launch_mma_t<K, S, E, L, B, ##__VA_ARGS__>(ctx, P, per_sm, n, st)

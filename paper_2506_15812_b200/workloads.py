@@ -224,6 +224,21 @@ def uniform_detector(centre_T, centre_Z, n, pitch, x_plane=DETECTOR_X):
                     (0.0, 0.0, 1.0), lo, hi, lo.copy(), hi.copy())
 
 
+def gapped_detector(det: Detector, gap_frac: float = 0.15, jitter: float = 0.3, seed: int = 7) -> Detector:
+    """The same plane and centre as `det`, its segments made non-uniform with gaps ("optional
+    non-uniform size and gaps"): every segment keeps its centre, its width is the pitch times (1 - gap_frac) times a
+    seeded factor in [1 - jitter, 1]; segments stay ordered and disjoint.  Takes the binary-search path of a5."""
+    rng = np.random.default_rng(seed)
+
+    def axis(lo, hi):
+        c, wid = 0.5 * (lo + hi), (hi - lo) * (1.0 - gap_frac) * (1.0 - jitter * rng.random(len(lo)))
+        return np.ascontiguousarray(c - 0.5 * wid), np.ascontiguousarray(c + 0.5 * wid)
+
+    ul, uh = axis(det.u_lo, det.u_hi)
+    wl_, wh = axis(det.w_lo, det.w_hi)
+    return Detector(det.origin, det.normal, det.eu, det.ew, ul, uh, wl_, wh)
+
+
 @dataclass
 class Group:
     """One seeding call: a contiguous run of ions sharing beam, group id, birth time and
