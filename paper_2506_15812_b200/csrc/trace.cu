@@ -21,6 +21,13 @@
 //  * 1/R by MUFU.RSQ64H seed + one cubic (Halley) step: 6 FP64 instructions instead of ~30.
 #include "trace_common.cuh"
 
+#ifdef TG_EXP_RSQ
+#define TG_RSQ(a, root) tg_rsqrt_sqrt(a, root)
+#else
+__device__ __forceinline__ double tg_rsqrt_r(double a, double& root) { double y = tg_rsqrt(a); root = a * y; return y; }
+#define TG_RSQ(a, root) tg_rsqrt_r(a, root)
+#endif
+
 template <int KIND>
 struct CellCache;                              // register cache of the current cell (kind 0)
 template <>
@@ -43,7 +50,11 @@ __device__ __forceinline__ double tg_horner16(const double* c, double p, double 
     double r1 = fma(fma(fma(c[7], w, c[6]), w, c[5]), w, c[4]);
     double r2 = fma(fma(fma(c[11], w, c[10]), w, c[9]), w, c[8]);
     double r3 = fma(fma(fma(c[15], w, c[14]), w, c[13]), w, c[12]);
+#ifdef TG_EXP_ESTRIN
+    return fma(fma(r3, p, r2), p * p, fma(r1, p, r0));      // the rows are ready long before p (1/R chain): Estrin in p is one level shorter
+#else
     return fma(fma(fma(r3, p, r2), p, r1), p, r0);
+#endif
 }
 
 // Re-read the register cache for the cell that contains the global cell coordinates (pR, pZ)
@@ -370,7 +381,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
         ++warp_steps;
         if (alive) {
             // ---- stage 1 at (r, u); its grid test is the out-of-grid test of the previous step (O4)
-            double R2 = fma(X, X, Y * Y), rinv = tg_rsqrt(R2), R = R2 * rinv;
+            double R2 = fma(X, X, Y * Y), R, rinv = TG_RSQ(R2, R);
             double Bx, By, Bz, BR, Bp, tR, tZ;
             bool outside = false, dummy = false;
             double dR = 0.0, dZ = 0.0;         // predicted half-step displacement in cells
@@ -404,7 +415,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 double Xm = fma(k1x, P.a2, fma(Ux, P.a1, X)), Ym = fma(k1y, P.a2, fma(Uy, P.a1, Y)), Zm = fma(k1z, P.a2, fma(Uz, P.a1, Z));
                 double ux = fma(k1x, P.b1, Ux), uy = fma(k1y, P.b1, Uy), uz = fma(k1z, P.b1, Uz);
                 double tm = t + 0.5 * P.dt;
-                R2 = fma(Xm, Xm, Ym * Ym); rinv = tg_rsqrt(R2); R = R2 * rinv;
+                R2 = fma(Xm, Xm, Ym * Ym); rinv = TG_RSQ(R2, R);
                 if constexpr (KIND == 1 && PRED == 3) tg_field_blend<false, true>(P, cc, reloads, dummy, R, Zm, tm, t + P.dt, BR, Bz, Bp);
                 else tg_fieldCyl<KIND, CACHED, false, PRED == 2>(P, cc, reloads, dummy, Xm, Ym, Zm, tm, R, BR, Bz, Bp, tR, tZ, dR, dZ);
                 if constexpr (PRED == 1) tg_predict(P, cc, reloads, tR + dR, tZ + dZ, BR, Bz, Bp);
@@ -414,7 +425,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 ux = fma(k2x, P.b1, Ux); uy = fma(k2y, P.b1, Uy); uz = fma(k2z, P.b1, Uz);
                 if (P.variant) {               // printed Eq. 6: k3 position increment from k2
                     Xm = fma(k2x, P.a2, fma(Ux, P.a1, X)); Ym = fma(k2y, P.a2, fma(Uy, P.a1, Y)); Zm = fma(k2z, P.a2, fma(Uz, P.a1, Z));
-                    R2 = fma(Xm, Xm, Ym * Ym); rinv = tg_rsqrt(R2); R = R2 * rinv;
+                    R2 = fma(Xm, Xm, Ym * Ym); rinv = TG_RSQ(R2, R);
                     if constexpr (KIND == 1 && PRED == 3) tg_field_blend<false, false>(P, cc, reloads, dummy, R, Zm, tm, 0.0, BR, Bz, Bp);
                     else tg_fieldCyl<KIND, CACHED>(P, cc, reloads, dummy, Xm, Ym, Zm, tm, R, BR, Bz, Bp, tR, tZ);   // on-demand verify / refill
                     tg_rotate(Xm, Ym, rinv, BR, Bp, Bx, By);
@@ -425,7 +436,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 double Xe = fma(k3x, 4.0 * P.a2, fma(Ux, 2.0 * P.a1, X)), Ye = fma(k3y, 4.0 * P.a2, fma(Uy, 2.0 * P.a1, Y)),
                        Ze = fma(k3z, 4.0 * P.a2, fma(Uz, 2.0 * P.a1, Z));
                 ux = fma(k3x, 2.0 * P.b1, Ux); uy = fma(k3y, 2.0 * P.b1, Uy); uz = fma(k3z, 2.0 * P.b1, Uz);
-                R2 = fma(Xe, Xe, Ye * Ye); rinv = tg_rsqrt(R2); R = R2 * rinv;
+                R2 = fma(Xe, Xe, Ye * Ye); rinv = TG_RSQ(R2, R);
                 if constexpr (KIND == 1 && PRED == 3) tg_field_blend<false, false>(P, cc, reloads, dummy, R, Ze, t + P.dt, 0.0, BR, Bz, Bp);
                 else tg_fieldCyl<KIND, CACHED>(P, cc, reloads, dummy, Xe, Ye, Ze, t + P.dt, R, BR, Bz, Bp, tR, tZ);
                 tg_rotate(Xe, Ye, rinv, BR, Bp, Bx, By);

@@ -43,6 +43,18 @@ __device__ __forceinline__ double tg_rsqrt(double a) {
     return fma(y * e, q, y);                   // y (1 + e/2 + 3 e^2/8): cubic convergence
 }
 
+// 1/sqrt(a) and sqrt(a) together; the square root comes off the same correction one dependent operation earlier
+// (sqrt(a) = t (1 + e q) with t = a y), which is what the cell coordinate of the next Horner sum waits for
+__device__ __forceinline__ double tg_rsqrt_sqrt(double a, double& root) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+    double t = a * y;
+    double e = fma(-t, y, 1.0);
+    double q = fma(0.375, e, 0.5);
+    root = fma(t * e, q, t);
+    return fma(y * e, q, y);
+}
+
 // t in [0,1)  <=>  sign 0 and exponent < 1023  <=>  (unsigned) hi word < 0x3FF00000
 __device__ __forceinline__ bool tg_in01(double t) { return (unsigned)__double2hiint(t) < 0x3FF00000u; }
 
