@@ -233,7 +233,9 @@ int taiga_loss_statistics(const unsigned long long wsummary_host[4], double out_
  * free lanes from the queue when at least this many are free; 32 = whole tiles, default),
  * "ctas_per_sm", "variant" (kernel variant: 0 register cell cache with rolling predictive refill,
  * 8 warps/SM (default); 4 predictive refill after each evaluation; 5 refill on demand only; 3 the
- * same at 12 warps/SM; 1 / 2 no cache at 8 / 16 warps/SM), "stats" (1: read counters back,
+ * same at 12 warps/SM; 1 / 2 no cache at 8 / 16 warps/SM; time-sliced fields: 0 time-blended cell
+ * cache in registers with the slice difference in per-lane shared-memory slots (default), 6 the same
+ * with the difference gathered through L1, 4 slice cache with rolling refill), "stats" (1: read counters back,
  * default), "precision" (64 default; 32 = the fp32 variant of BASELINE config 5: kind-2 fields
  * with the RKN solver only, tricubic evaluation and its table in fp32, cell location and the ion
  * state in fp64; hit coordinates then agree with fp64 to 1e-5 m, integer outputs are not

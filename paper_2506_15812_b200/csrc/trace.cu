@@ -240,6 +240,78 @@ __device__ __forceinline__ void tg_field_blend(const TraceParams& P, CellCache<1
     BR = out[0]; BZ = out[1]; Bp = out[2];
 }
 
+// Kind 1, blended cache with the slice difference in shared memory (PRED 4).  As tg_field_blend, but D_k of the lane's
+// cell lives in the lane's own 384-B shared-memory slot (stride TG_SLOT = 400 B: the 16-B chunks of eight consecutive
+// lanes cover all 32 banks, so a warp-wide LDS.128 is 4 wavefronts whatever cells the lanes sit in).  The slot is
+// filled by cp.async when the lane enters a cell (no register staging, no write-back port), so the once-per-step stream
+// of D_k no longer goes through divergent 256-bit L1 gathers: those cost 8 / 16 / 32 wavefronts per load with 1 / 2 /
+// >= 4 cells per warp (taiga_measure_l1_gather_peak) and kept the L1 data pipe 71 % busy (profiles/r2_trace_ncu.md).
+#define TG_SLOT 400
+__device__ __forceinline__ void tg_lds2(unsigned a, double& x, double& y) {
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(x), "=d"(y) : "r"(a) : "memory");
+}
+template <bool FIRST, bool STREAM>
+__device__ __forceinline__ void tg_field_blend_sm(const TraceParams& P, CellCache<1>& cc, unsigned& reloads, bool& outside, unsigned sd,
+                                                  double R, double Z, double t, double t_next, double& BR, double& BZ, double& Bp) {
+    const double xs = (t - P.f.s0) * P.f.inv_ds;
+    const int k = tg_clampi(__double2int_rd(xs), 0, P.f.nS - 2);
+    const double tau = fmin(fmax(xs - (double)k, 0.0), 1.0);
+    double tR = fma(R, P.f.inv_hR, -cc.oR), tZ = fma(Z, P.f.inv_hZ, -cc.oZ);
+    const bool hit = tg_in01(tR) && tg_in01(tZ) && k == cc.k;
+    double out[3];
+    if (!hit) {                                // another cell or slice: D_k -> my slot (asynchronous), H_k -> C
+        if constexpr (FIRST) outside = (R < P.f.Rmin) | (R > P.f.Rmax) | (Z < P.f.Zmin) | (Z > P.f.Zmax);
+        int i = tg_clampi(__double2int_rd(fma(R, P.f.inv_hR, -P.f.offR)), 0, P.f.cR - 1);
+        int j = tg_clampi(__double2int_rd(fma(Z, P.f.inv_hZ, -P.f.offZ)), 0, P.f.cZ - 1);
+        cc.oR = P.f.offR + (double)i; cc.oZ = P.f.offZ + (double)j; cc.k = k; cc.cell = i * P.f.cZ + j;
+        tR = fma(R, P.f.inv_hR, -cc.oR); tZ = fma(Z, P.f.inv_hZ, -cc.oZ);
+        const double* hsrc = P.f.table + ((size_t)cc.cell * P.f.nS + cc.k) * 48;
+        const double* dsrc = P.f.dtable + ((size_t)cc.cell * (P.f.nS - 1) + cc.k) * 48;
+        // a copy of an earlier refill may still be in flight (a new ion starts at tau = 0 exactly and blends nothing, so its
+        // first evaluation does not wait): two copies into one slot complete in any order, the older must have landed first
+        asm volatile("cp.async.wait_all;" ::: "memory");
+#pragma unroll
+        for (int q = 0; q < 24; ++q)
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(sd + 16 * q), "l"(dsrc + 2 * q) : "memory");
+#pragma unroll
+        for (int q = 0; q < 12; ++q)
+            tg_ld4(hsrc + 4 * q, cc.c[4 * q], cc.c[4 * q + 1], cc.c[4 * q + 2], cc.c[4 * q + 3]);
+        cc.tau = 0.0;
+        ++reloads;
+    }
+    if constexpr (!STREAM) {
+        if (tau != cc.tau) {                   // bring C to this evaluation's time (after a refill: from H_k)
+            asm volatile("cp.async.wait_all;" ::: "memory");
+            const double adv = tau - cc.tau;
+#pragma unroll
+            for (int q = 0; q < 24; ++q) {
+                double d0, d1;
+                tg_lds2(sd + 16 * q, d0, d1);
+                cc.c[2 * q] = fma(adv, d0, cc.c[2 * q]); cc.c[2 * q + 1] = fma(adv, d1, cc.c[2 * q + 1]);
+            }
+            cc.tau = tau;
+        }
+#pragma unroll
+        for (int m = 0; m < 3; ++m) out[m] = tg_horner16(cc.c + m * 16, tR, tZ);
+    } else {
+        const double tau_n = fmin(fmax((t_next - P.f.s0) * P.f.inv_ds - (double)cc.k, 0.0), 1.0);
+        asm volatile("cp.async.wait_all;" ::: "memory");
+        const double adv = tau_n - cc.tau, back = tau - tau_n;
+#pragma unroll
+        for (int m = 0; m < 3; ++m) {
+            double d[16];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) tg_lds2(sd + 128 * m + 16 * q, d[2 * q], d[2 * q + 1]);
+            const double hD = tg_horner16(d, tR, tZ);
+#pragma unroll
+            for (int q = 0; q < 16; ++q) cc.c[m * 16 + q] = fma(adv, d[q], cc.c[m * 16 + q]);
+            out[m] = fma(back, hD, tg_horner16(cc.c + m * 16, tR, tZ));
+        }
+        cc.tau = tau_n;
+    }
+    BR = out[0]; BZ = out[1]; Bp = out[2];
+}
+
 // Predictive refill (kind 0, cached): right after the Horner evaluation of one stage has read the
 // cached coefficients for the last time, the in-cell coordinates of the NEXT stage are predicted
 // to ~1e-3 cell (tRp, tZp); if they fall outside the cached cell its successor is loaded now, so
@@ -288,6 +360,11 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
     unsigned reloads = 0, ion_steps = 0;       // per lane; < 2^32 for any run the queue allows
     unsigned long long warp_steps = 0;
 
+    [[maybe_unused]] unsigned sd = 0;          // PRED 4: shared address of this lane's slice-difference slot
+    if constexpr (KIND == 1 && PRED == 4) {
+        extern __shared__ __align__(16) unsigned char tg_dyn_smem[];
+        sd = (unsigned)__cvta_generic_to_shared(tg_dyn_smem) + threadIdx.x * TG_SLOT;
+    }
     [[maybe_unused]] int since = 0;            // REGROUP: iterations since the last CTA sync point
     while (true) {
       unsigned am;
@@ -387,6 +464,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
             double dR = 0.0, dZ = 0.0;         // predicted half-step displacement in cells
             if constexpr (PRED == 1 || PRED == 2) { dR = (fma(X, Ux, Y * Uy) * rinv) * P.pa1R; dZ = Uz * P.pa1Z; }
             if constexpr (KIND == 1 && PRED == 3) tg_field_blend<true, false>(P, cc, reloads, outside, R, Z, t, 0.0, BR, Bz, Bp);
+            else if constexpr (KIND == 1 && PRED == 4) tg_field_blend_sm<true, false>(P, cc, reloads, outside, sd, R, Z, t, 0.0, BR, Bz, Bp);
             else tg_fieldCyl<KIND, CACHED, true, PRED == 2>(P, cc, reloads, outside, X, Y, Z, t, R, BR, Bz, Bp, tR, tZ, dR, dZ);
             double nu1 = 0.0;
             if constexpr (LOSS) {                  // trapezoid of the step that ended at this point (not of a step that left the grid)
@@ -417,6 +495,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 double tm = t + 0.5 * P.dt;
                 R2 = fma(Xm, Xm, Ym * Ym); rinv = TG_RSQ(R2, R);
                 if constexpr (KIND == 1 && PRED == 3) tg_field_blend<false, true>(P, cc, reloads, dummy, R, Zm, tm, t + P.dt, BR, Bz, Bp);
+                else if constexpr (KIND == 1 && PRED == 4) tg_field_blend_sm<false, true>(P, cc, reloads, dummy, sd, R, Zm, tm, t + P.dt, BR, Bz, Bp);
                 else tg_fieldCyl<KIND, CACHED, false, PRED == 2>(P, cc, reloads, dummy, Xm, Ym, Zm, tm, R, BR, Bz, Bp, tR, tZ, dR, dZ);
                 if constexpr (PRED == 1) tg_predict(P, cc, reloads, tR + dR, tZ + dZ, BR, Bz, Bp);
                 tg_rotate(Xm, Ym, rinv, BR, Bp, Bx, By);
@@ -427,6 +506,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                     Xm = fma(k2x, P.a2, fma(Ux, P.a1, X)); Ym = fma(k2y, P.a2, fma(Uy, P.a1, Y)); Zm = fma(k2z, P.a2, fma(Uz, P.a1, Z));
                     R2 = fma(Xm, Xm, Ym * Ym); rinv = TG_RSQ(R2, R);
                     if constexpr (KIND == 1 && PRED == 3) tg_field_blend<false, false>(P, cc, reloads, dummy, R, Zm, tm, 0.0, BR, Bz, Bp);
+                    else if constexpr (KIND == 1 && PRED == 4) tg_field_blend_sm<false, false>(P, cc, reloads, dummy, sd, R, Zm, tm, 0.0, BR, Bz, Bp);
                     else tg_fieldCyl<KIND, CACHED>(P, cc, reloads, dummy, Xm, Ym, Zm, tm, R, BR, Bz, Bp, tR, tZ);   // on-demand verify / refill
                     tg_rotate(Xm, Ym, rinv, BR, Bp, Bx, By);
                 }
@@ -438,6 +518,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 ux = fma(k3x, 2.0 * P.b1, Ux); uy = fma(k3y, 2.0 * P.b1, Uy); uz = fma(k3z, 2.0 * P.b1, Uz);
                 R2 = fma(Xe, Xe, Ye * Ye); rinv = TG_RSQ(R2, R);
                 if constexpr (KIND == 1 && PRED == 3) tg_field_blend<false, false>(P, cc, reloads, dummy, R, Ze, t + P.dt, 0.0, BR, Bz, Bp);
+                else if constexpr (KIND == 1 && PRED == 4) tg_field_blend_sm<false, false>(P, cc, reloads, dummy, sd, R, Ze, t + P.dt, 0.0, BR, Bz, Bp);
                 else tg_fieldCyl<KIND, CACHED>(P, cc, reloads, dummy, Xe, Ye, Ze, t + P.dt, R, BR, Bz, Bp, tR, tZ);
                 tg_rotate(Xe, Ye, rinv, BR, Bp, Bx, By);
                 double k4x = fma(uy, Bz, -(uz * By)), k4y = fma(uz, Bx, -(ux * Bz)), k4z = fma(ux, By, -(uy * Bx));
@@ -553,25 +634,27 @@ __global__ void k_table_to_f32(const double* __restrict__ src, float* __restrict
 // Every instantiation of k_trace, one line each: {kind, cached, registers, PRED, SOLVER, HAS_E, LOSS, BEZ, REGROUP}.
 //   kind 0, RKN: register cell cache with rolling predictive refill (PRED 2; 2 x 128 threads/SM, 254 registers),
 //   predictive refill after each Horner (1), refill on demand (0; the 4-evaluation solvers), 168 registers, no cache;
-//   kinds 1 / 2 (option mma = 0, or precision = 32): slice cache / per-lane gathers of trace.cu; the default for these
-//   kinds is the warp-cooperative kernel of trace_mma.cu.
+//   kind 1: time-blended cell cache in registers, slice difference in per-lane shared-memory slots (PRED 4, default) or
+//   gathered through L1 (3), slice cache with rolling refill (2), no cache (0);
+//   kind 2 with option mma = 0 or precision = 32: per-lane gathers (REGROUP: CTA re-sort by cell); the default for kind 2
+//   is the warp-cooperative kernel of trace_mma.cu.
 struct TgVariant { int kind, cached, regs, pred, solver, hasE, loss, bez, regroup; void (*fn)(const TraceParams); };
 #define TG_V(K, C, R, P, S, E, L, B, G) {K, C, R, P, S, E, L, B, G, k_trace<K, (C) != 0, 128, R, P, S, (E) != 0, (L) != 0, (B) != 0, (G) != 0>}
 static const TgVariant tg_variants[] = {
     // production path: RKN, E = 0
     TG_V(0, 1, 255, 2, 0, 0, 0, 0, 0), TG_V(0, 1, 255, 1, 0, 0, 0, 0, 0), TG_V(0, 1, 255, 0, 0, 0, 0, 0, 0), TG_V(0, 1, 168, 0, 0, 0, 0, 0, 0),
     TG_V(0, 0, 128, 0, 0, 0, 0, 0, 0), TG_V(0, 0, 255, 0, 0, 0, 0, 0, 0),
-    TG_V(1, 1, 255, 3, 0, 0, 0, 0, 0), TG_V(1, 1, 255, 2, 0, 0, 0, 0, 0), TG_V(1, 0, 255, 0, 0, 0, 0, 0, 0), TG_V(1, 0, 128, 0, 0, 0, 0, 0, 0),
+    TG_V(1, 1, 255, 4, 0, 0, 0, 0, 0), TG_V(1, 1, 255, 3, 0, 0, 0, 0, 0), TG_V(1, 1, 255, 2, 0, 0, 0, 0, 0), TG_V(1, 0, 255, 0, 0, 0, 0, 0, 0), TG_V(1, 0, 128, 0, 0, 0, 0, 0, 0),
     TG_V(2, 0, 255, 0, 0, 0, 0, 0, 1), TG_V(2, 0, 255, 0, 0, 0, 0, 0, 0), TG_V(2, 0, 128, 0, 0, 0, 0, 0, 0),
     // quadratic Bezier plane interpolation
-    TG_V(0, 1, 255, 2, 0, 0, 0, 1, 0), TG_V(0, 1, 255, 0, 0, 0, 0, 1, 0), TG_V(1, 1, 255, 3, 0, 0, 0, 1, 0), TG_V(1, 0, 255, 0, 0, 0, 0, 1, 0),
+    TG_V(0, 1, 255, 2, 0, 0, 0, 1, 0), TG_V(0, 1, 255, 0, 0, 0, 0, 1, 0), TG_V(1, 1, 255, 4, 0, 0, 0, 1, 0), TG_V(1, 0, 255, 0, 0, 0, 0, 1, 0),
     TG_V(2, 0, 255, 0, 0, 0, 0, 1, 0),
     // Eq. 2 loss integral
-    TG_V(0, 1, 255, 2, 0, 0, 1, 0, 0), TG_V(0, 1, 255, 0, 0, 0, 1, 0, 0), TG_V(1, 1, 255, 3, 0, 0, 1, 0, 0), TG_V(1, 0, 255, 0, 0, 0, 1, 0, 0),
+    TG_V(0, 1, 255, 2, 0, 0, 1, 0, 0), TG_V(0, 1, 255, 0, 0, 0, 1, 0, 0), TG_V(1, 1, 255, 4, 0, 0, 1, 0, 0), TG_V(1, 0, 255, 0, 0, 0, 1, 0, 0),
     TG_V(2, 0, 255, 0, 0, 0, 1, 0, 0),
     // uniform E and / or the other solvers (Eq. 4, Eq. 7-8)
     TG_V(0, 1, 255, 2, 0, 1, 0, 0, 0), TG_V(0, 1, 255, 0, 0, 1, 0, 0, 0), TG_V(0, 1, 255, 0, 2, 1, 0, 0, 0), TG_V(0, 1, 255, 0, 3, 1, 0, 0, 0),
-    TG_V(1, 1, 255, 3, 0, 1, 0, 0, 0), TG_V(1, 0, 255, 0, 0, 1, 0, 0, 0), TG_V(1, 0, 255, 0, 2, 1, 0, 0, 0), TG_V(1, 0, 255, 0, 3, 1, 0, 0, 0),
+    TG_V(1, 1, 255, 4, 0, 1, 0, 0, 0), TG_V(1, 0, 255, 0, 0, 1, 0, 0, 0), TG_V(1, 0, 255, 0, 2, 1, 0, 0, 0), TG_V(1, 0, 255, 0, 3, 1, 0, 0, 0),
     TG_V(2, 0, 255, 0, 0, 1, 0, 0, 0), TG_V(2, 0, 255, 0, 2, 1, 0, 0, 0), TG_V(2, 0, 255, 0, 3, 1, 0, 0, 0),
 };
 #undef TG_V
@@ -657,7 +740,8 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
                 default: break;
             }
         } else if (kind == 1) {
-            if (variant == 0 && (special || kv == 0)) { k.cached = 1; k.pred = 3; }   // blended cell cache, advanced in time once per step
+            if (variant == 0 && (special || kv == 0)) { k.cached = 1; k.pred = 4; }   // blended cell cache, slice difference in per-lane shared-memory slots
+            else if (variant == 0 && kv == 6) { k.cached = 1; k.pred = 3; }           // blended cell cache, slice difference gathered through L1 (r2a)
             else if (variant == 0 && kv == 4) { k.cached = 1; k.pred = 2; }           // slice cache + rolling refill, difference gathered per evaluation (r1e)
             else if (!special && (kv == 2 || kv == 3)) k.regs = 128;
         } else {
@@ -675,7 +759,12 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         unsigned grid = (unsigned)(ctx->sm_count * per_sm);
         unsigned need = (unsigned)((ions->n + threads - 1) / threads);
         if (grid > need) grid = need;
-        sel->fn<<<grid, threads, 0, st>>>(P);
+        size_t smem = 0;
+        if (k.kind == 1 && k.pred == 4) {          // per-lane slice-difference slots: above the 48 KB static limit
+            smem = (size_t)threads * TG_SLOT;
+            TG_CUDA(ctx, cudaFuncSetAttribute((const void*)sel->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        }
+        sel->fn<<<grid, threads, smem, st>>>(P);
     }
     ++launches;
     TG_CUDA(ctx, cudaGetLastError());
