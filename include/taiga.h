@@ -232,8 +232,8 @@ int taiga_loss_statistics(const unsigned long long wsummary_host[4], double out_
  * "sort_sub" (sort bins per grid cell and axis, default 16), "min_active" (a warp refills its
  * free lanes from the queue when at least this many are free; 32 = whole tiles, default),
  * "ctas_per_sm", "variant" (kernel variant: 0 register cell cache with rolling predictive refill,
- * 8 warps/SM (default); 4 predictive refill after each evaluation; 5 refill on demand only; 3 the
- * same at 12 warps/SM; 1 / 2 no cache at 8 / 16 warps/SM; time-sliced fields: 0 time-blended cell
+ * 9 warps/SM (default); 4 predictive refill after each evaluation; 5 refill on demand only; 3 the
+ * same at 12 warps/SM; 1 / 2 no cache at 8 / 16 warps/SM; 7 the default kernel at 8 warps/SM in 128-thread CTAs; time-sliced fields: 0 time-blended cell
  * cache in registers with the slice difference in per-lane shared-memory slots (default), 6 the same
  * with the difference gathered through L1, 4 slice cache with rolling refill), "stats" (1: read counters back,
  * default), "precision" (64 default; 32 = the fp32 variant of BASELINE config 5: kind-2 fields
@@ -259,6 +259,9 @@ int taiga_measure_fp64_peak(taiga_ctx* ctx, double ms, double* dfma_per_s);
 /* the same for the FP64 tensor pipe: DMMA.8x8x4 chains, FMA per second (256 per warp instruction); the
  * denominator of the warp-cooperative tracer of kinds 1 and 2. */
 int taiga_measure_dmma_peak(taiga_ctx* ctx, double ms, double* fma_per_s);
+/* DFMA and DMMA chains interleaved 1 : 1 in FMA count: total FMA per second.  It does not exceed the DFMA rate (one
+ * FP64 datapath per SM serves both), which is why every kernel is reported against 148 x 64 FMA/clk. */
+int taiga_measure_mixed_fp64_peak(taiga_ctx* ctx, double ms, double* fma_per_s);
 /* L1-resident gather microkernel shaped like the uncached field evaluation (8 warps/SM, 48 x 256-bit
  * loads of a 1536-B cell per lane): bytes per second delivered to registers; `spread` = distinct cells
  * read by the lanes of a warp (1 ... 32).  The roofline denominator of the kind-1 / kind-2 kernels. */

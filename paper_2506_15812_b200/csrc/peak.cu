@@ -55,7 +55,7 @@ int tg_fp64_peak(taiga_ctx* ctx, double ms, double* rate) {
 }
 
 // FP64 tensor pipe: DMMA.8x8x4 (256 FMA per warp instruction) issue rate, in FMA per second.  On B200 it equals the
-// DFMA rate (the two share the FP64 datapath; a mix of both measures 0.89-0.92 of it), but reads each operand
+// DFMA rate (the two share the FP64 datapath: k_mixed_peak below), but reads each operand
 // register for 8 FMAs: the denominator of the warp-cooperative tracer (trace_mma.cu).
 __global__ void __launch_bounds__(256) k_dmma_peak(double* out, int iters, double a0, double b0) {
     double c[4][2], a[4], b[4];
@@ -93,6 +93,64 @@ int tg_dmma_peak(taiga_ctx* ctx, double ms, double* rate) {
         if (e != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); TG_CUDA(ctx, e); }
         cudaEventElapsedTime(&t, e0, e1);
         double n = (double)grid * 256.0 * (double)iters * 16.0 * 4.0 * 8.0;     // 8 FMA per lane and DMMA
+        if (rep >= 2) { double r = n / (t * 1e-3); if (r > best) best = r; }
+        if (rep == 1 && t > 0.f) { double scale = ms / t; iters = (int)(iters * scale) + 1; if (iters > (1 << 22)) iters = 1 << 22; }
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    TG_CUDA(ctx, cudaGetLastError());
+    *rate = best;
+    return TAIGA_OK;
+}
+
+// DFMA and DMMA chains interleaved, one DMMA (8 FMA per lane) per 8 DFMA: if the two had datapaths of their own the sum
+// would approach twice the DFMA rate.  Measured: it stays below the DFMA rate, so 148 x 64 FMA/clk is the one FP64 roofline
+// of the SM whichever instruction carries the work (profiles/r2a_microbench.md).
+__global__ void __launch_bounds__(256) k_mixed_peak(double* out, int iters, double a0, double b0) {
+    double c[2][2], a[2], b[2], v[4], m[4];
+#pragma unroll
+    for (int i = 0; i < 2; ++i) { c[i][0] = (double)threadIdx.x; c[i][1] = (double)i; a[i] = a0 + i * 1e-9; b[i] = b0 + i * 1e-9; }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { v[i] = (double)(threadIdx.x + i) * 1e-3; m[i] = a0 + i * 1e-9; }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                             : "+d"(c[i][0]), "+d"(c[i][1]) : "d"(a[i]), "d"(b[i]));
+#pragma unroll
+                for (int r = 0; r < 2; ++r)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) v[j] = fma(v[j], m[j], b0);
+            }
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 2; ++i) s += c[i][0] + c[i][1];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) s += v[i];
+    if (s == 123.456) out[0] = s;
+}
+
+int tg_mixed_peak(taiga_ctx* ctx, double ms, double* rate) {
+    cudaStream_t st = ctx->stream;
+    cudaEvent_t e0, e1;
+    TG_CUDA(ctx, cudaEventCreate(&e0));
+    TG_CUDA(ctx, cudaEventCreate(&e1));
+    double* dummy = (double*)ctx->counters + 12;
+    unsigned grid = (unsigned)ctx->sm_count * 2;      // 16 warps per SM
+    int iters = 256;
+    float t = 0.f;
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {
+        cudaEventRecord(e0, st);
+        k_mixed_peak<<<grid, 256, 0, st>>>(dummy, iters, 0.999999, 1e-7);
+        cudaEventRecord(e1, st);
+        cudaError_t e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); TG_CUDA(ctx, e); }
+        cudaEventElapsedTime(&t, e0, e1);
+        double n = (double)grid * 256.0 * (double)iters * 16.0 * 2.0 * (8.0 + 8.0);     // per lane: 8 FMA per DMMA + 8 DFMA
         if (rep >= 2) { double r = n / (t * 1e-3); if (r > best) best = r; }
         if (rep == 1 && t > 0.f) { double scale = ms / t; iters = (int)(iters * scale) + 1; if (iters > (1 << 22)) iters = 1 << 22; }
     }

@@ -235,7 +235,7 @@ extern "C" int taiga_set_option(taiga_ctx* ctx, const char* key, long long v) {
         {"sort", &ctx->opt_sort, 0, 1}, {"sort_sub", &ctx->opt_sort_sub, 1, 64},
         {"precision", &ctx->opt_precision, 32, 64}, {"plane_interp", &ctx->opt_plane_interp, 0, 1},
         {"regroup", &ctx->opt_regroup, 0, 1 << 20}, {"min_active", &ctx->opt_min_active, 0, 32},
-        {"ctas_per_sm", &ctx->opt_ctas_per_sm, 0, 32}, {"variant", &ctx->opt_variant, 0, 6}, {"stats", &ctx->opt_stats, 0, 1},
+        {"ctas_per_sm", &ctx->opt_ctas_per_sm, 0, 32}, {"variant", &ctx->opt_variant, 0, 7}, {"stats", &ctx->opt_stats, 0, 1},
         {"mma", &ctx->opt_mma, -1, 1}, {"refill_cta", &ctx->opt_refill_cta, 0, 1024},
         {"mma_geom", &ctx->opt_mma_geom, 0, 5}};
     for (auto& t : tab) if (!strcmp(key, t.k)) {
@@ -272,6 +272,12 @@ extern "C" int taiga_measure_dmma_peak(taiga_ctx* ctx, double ms, double* rate) 
     if (!ctx || !rate || !(ms > 0)) return TAIGA_E_ARG;
     TG_CUDA(ctx, cudaSetDevice(ctx->device));
     return tg_dmma_peak(ctx, ms, rate);
+}
+
+extern "C" int taiga_measure_mixed_fp64_peak(taiga_ctx* ctx, double ms, double* rate) {
+    if (!ctx || !rate || !(ms > 0)) return TAIGA_E_ARG;
+    TG_CUDA(ctx, cudaSetDevice(ctx->device));
+    return tg_mixed_peak(ctx, ms, rate);
 }
 
 extern "C" int taiga_loss_statistics(const unsigned long long ws[4], double out[3]) {

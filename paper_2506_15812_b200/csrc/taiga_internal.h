@@ -139,4 +139,5 @@ int tg_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, const taiga_de
                           unsigned long long* wcounts, unsigned long long* wsummary);
 int tg_fp64_peak(taiga_ctx* ctx, double ms, double* rate);
 int tg_dmma_peak(taiga_ctx* ctx, double ms, double* rate);
+int tg_mixed_peak(taiga_ctx* ctx, double ms, double* rate);
 int tg_l1_gather_peak(taiga_ctx* ctx, double ms, int spread, double* bytes_per_s);

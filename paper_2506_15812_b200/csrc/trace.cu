@@ -21,13 +21,6 @@
 //  * 1/R by MUFU.RSQ64H seed + one cubic (Halley) step: 6 FP64 instructions instead of ~30.
 #include "trace_common.cuh"
 
-#ifdef TG_EXP_RSQ
-#define TG_RSQ(a, root) tg_rsqrt_sqrt(a, root)
-#else
-__device__ __forceinline__ double tg_rsqrt_r(double a, double& root) { double y = tg_rsqrt(a); root = a * y; return y; }
-#define TG_RSQ(a, root) tg_rsqrt_r(a, root)
-#endif
-
 template <int KIND>
 struct CellCache;                              // register cache of the current cell (kind 0)
 template <>
@@ -50,11 +43,7 @@ __device__ __forceinline__ double tg_horner16(const double* c, double p, double 
     double r1 = fma(fma(fma(c[7], w, c[6]), w, c[5]), w, c[4]);
     double r2 = fma(fma(fma(c[11], w, c[10]), w, c[9]), w, c[8]);
     double r3 = fma(fma(fma(c[15], w, c[14]), w, c[13]), w, c[12]);
-#ifdef TG_EXP_ESTRIN
-    return fma(fma(r3, p, r2), p * p, fma(r1, p, r0));      // the rows are ready long before p (1/R chain): Estrin in p is one level shorter
-#else
     return fma(fma(fma(r3, p, r2), p, r1), p, r0);
-#endif
 }
 
 // Re-read the register cache for the cell that contains the global cell coordinates (pR, pZ)
@@ -458,7 +447,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
         ++warp_steps;
         if (alive) {
             // ---- stage 1 at (r, u); its grid test is the out-of-grid test of the previous step (O4)
-            double R2 = fma(X, X, Y * Y), R, rinv = TG_RSQ(R2, R);
+            double R2 = fma(X, X, Y * Y), R, rinv = tg_rsq<KIND == 0>(R2, R);
             double Bx, By, Bz, BR, Bp, tR, tZ;
             bool outside = false, dummy = false;
             double dR = 0.0, dZ = 0.0;         // predicted half-step displacement in cells
@@ -493,7 +482,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 double Xm = fma(k1x, P.a2, fma(Ux, P.a1, X)), Ym = fma(k1y, P.a2, fma(Uy, P.a1, Y)), Zm = fma(k1z, P.a2, fma(Uz, P.a1, Z));
                 double ux = fma(k1x, P.b1, Ux), uy = fma(k1y, P.b1, Uy), uz = fma(k1z, P.b1, Uz);
                 double tm = t + 0.5 * P.dt;
-                R2 = fma(Xm, Xm, Ym * Ym); rinv = TG_RSQ(R2, R);
+                R2 = fma(Xm, Xm, Ym * Ym); rinv = tg_rsq<KIND == 0>(R2, R);
                 if constexpr (KIND == 1 && PRED == 3) tg_field_blend<false, true>(P, cc, reloads, dummy, R, Zm, tm, t + P.dt, BR, Bz, Bp);
                 else if constexpr (KIND == 1 && PRED == 4) tg_field_blend_sm<false, true>(P, cc, reloads, dummy, sd, R, Zm, tm, t + P.dt, BR, Bz, Bp);
                 else tg_fieldCyl<KIND, CACHED, false, PRED == 2>(P, cc, reloads, dummy, Xm, Ym, Zm, tm, R, BR, Bz, Bp, tR, tZ, dR, dZ);
@@ -504,7 +493,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 ux = fma(k2x, P.b1, Ux); uy = fma(k2y, P.b1, Uy); uz = fma(k2z, P.b1, Uz);
                 if (P.variant) {               // printed Eq. 6: k3 position increment from k2
                     Xm = fma(k2x, P.a2, fma(Ux, P.a1, X)); Ym = fma(k2y, P.a2, fma(Uy, P.a1, Y)); Zm = fma(k2z, P.a2, fma(Uz, P.a1, Z));
-                    R2 = fma(Xm, Xm, Ym * Ym); rinv = TG_RSQ(R2, R);
+                    R2 = fma(Xm, Xm, Ym * Ym); rinv = tg_rsq<KIND == 0>(R2, R);
                     if constexpr (KIND == 1 && PRED == 3) tg_field_blend<false, false>(P, cc, reloads, dummy, R, Zm, tm, 0.0, BR, Bz, Bp);
                     else if constexpr (KIND == 1 && PRED == 4) tg_field_blend_sm<false, false>(P, cc, reloads, dummy, sd, R, Zm, tm, 0.0, BR, Bz, Bp);
                     else tg_fieldCyl<KIND, CACHED>(P, cc, reloads, dummy, Xm, Ym, Zm, tm, R, BR, Bz, Bp, tR, tZ);   // on-demand verify / refill
@@ -516,7 +505,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 double Xe = fma(k3x, 4.0 * P.a2, fma(Ux, 2.0 * P.a1, X)), Ye = fma(k3y, 4.0 * P.a2, fma(Uy, 2.0 * P.a1, Y)),
                        Ze = fma(k3z, 4.0 * P.a2, fma(Uz, 2.0 * P.a1, Z));
                 ux = fma(k3x, 2.0 * P.b1, Ux); uy = fma(k3y, 2.0 * P.b1, Uy); uz = fma(k3z, 2.0 * P.b1, Uz);
-                R2 = fma(Xe, Xe, Ye * Ye); rinv = TG_RSQ(R2, R);
+                R2 = fma(Xe, Xe, Ye * Ye); rinv = tg_rsq<KIND == 0>(R2, R);
                 if constexpr (KIND == 1 && PRED == 3) tg_field_blend<false, false>(P, cc, reloads, dummy, R, Ze, t + P.dt, 0.0, BR, Bz, Bp);
                 else if constexpr (KIND == 1 && PRED == 4) tg_field_blend_sm<false, false>(P, cc, reloads, dummy, sd, R, Ze, t + P.dt, 0.0, BR, Bz, Bp);
                 else tg_fieldCyl<KIND, CACHED>(P, cc, reloads, dummy, Xe, Ye, Ze, t + P.dt, R, BR, Bz, Bp, tR, tZ);
@@ -632,15 +621,19 @@ __global__ void k_table_to_f32(const double* __restrict__ src, float* __restrict
 }
 
 // Every instantiation of k_trace, one line each: {kind, cached, registers, PRED, SOLVER, HAS_E, LOSS, BEZ, REGROUP}.
-//   kind 0, RKN: register cell cache with rolling predictive refill (PRED 2; 2 x 128 threads/SM, 254 registers),
+//   kind 0, RKN: register cell cache with rolling predictive refill (PRED 2; 9 x 32 threads/SM at <= 224 registers),
 //   predictive refill after each Horner (1), refill on demand (0; the 4-evaluation solvers), 168 registers, no cache;
 //   kind 1: time-blended cell cache in registers, slice difference in per-lane shared-memory slots (PRED 4, default) or
 //   gathered through L1 (3), slice cache with rolling refill (2), no cache (0);
 //   kind 2 with option mma = 0 or precision = 32: per-lane gathers (REGROUP: CTA re-sort by cell); the default for kind 2
 //   is the warp-cooperative kernel of trace_mma.cu.
-struct TgVariant { int kind, cached, regs, pred, solver, hasE, loss, bez, regroup; void (*fn)(const TraceParams); };
-#define TG_V(K, C, R, P, S, E, L, B, G) {K, C, R, P, S, E, L, B, G, k_trace<K, (C) != 0, 128, R, P, S, (E) != 0, (L) != 0, (B) != 0, (G) != 0>}
+struct TgVariant { int kind, cached, regs, pred, solver, hasE, loss, bez, regroup; void (*fn)(const TraceParams); int threads; };
+#define TG_V(K, C, R, P, S, E, L, B, G) {K, C, R, P, S, E, L, B, G, k_trace<K, (C) != 0, 128, R, P, S, (E) != 0, (L) != 0, (B) != 0, (G) != 0>, 128}
+#define TG_VT(K, C, R, P, T) {K, C, R, P, 0, 0, 0, 0, 0, k_trace<K, (C) != 0, T, R, P, 0, false, false, false, false>, T}
 static const TgVariant tg_variants[] = {
+    // 9 warps per SM in 32-thread CTAs (warps are independent: any block size); 10 and 11 warps at 200 / 184 registers
+    // were slower (profiles/r2_experiments.md)
+    TG_VT(0, 1, 224, 2, 32),
     // production path: RKN, E = 0
     TG_V(0, 1, 255, 2, 0, 0, 0, 0, 0), TG_V(0, 1, 255, 1, 0, 0, 0, 0, 0), TG_V(0, 1, 255, 0, 0, 0, 0, 0, 0), TG_V(0, 1, 168, 0, 0, 0, 0, 0, 0),
     TG_V(0, 0, 128, 0, 0, 0, 0, 0, 0), TG_V(0, 0, 255, 0, 0, 0, 0, 0, 0),
@@ -732,7 +725,8 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
             if (special) { k.cached = 1; k.pred = (variant == 0) ? 2 : 0; }
             else if (variant != 0) { k.cached = (kv != 1 && kv != 2); k.regs = (kv == 2) ? 128 : 255; }     // printed k3: 4th evaluation, on demand
             else switch (kv) {
-                case 0: k.cached = 1; k.pred = 2; break;
+                case 0: k.cached = 1; k.pred = 2; k.regs = 224; break;     // 9 warps/SM (9 x 32 threads): 31.3 against 31.5 ms
+                case 7: k.cached = 1; k.pred = 2; break;                   // 8 warps/SM (2 x 128 threads), the round-1 geometry
                 case 4: k.cached = 1; k.pred = 1; break;
                 case 5: k.cached = 1; break;
                 case 3: k.cached = 1; k.regs = 168; break;
@@ -754,8 +748,12 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
             if (v.kind == k.kind && v.cached == k.cached && v.regs == k.regs && v.pred == k.pred && v.solver == k.solver &&
                 v.hasE == k.hasE && v.loss == k.loss && v.bez == k.bez && v.regroup == k.regroup) { sel = &v; break; }
         if (!sel) { TG_SET_ERR(ctx, "trace: no kernel for kind %d solver %d with these options", kind, variant); return TAIGA_E_ARG; }
-        const int threads = 128;
+        const int threads = sel->threads;
         int per_sm = ctx->opt_ctas_per_sm > 0 ? ctx->opt_ctas_per_sm : (k.regs == 128 ? 4 : (k.regs == 168 ? 3 : 2));
+        if (threads != 128 && ctx->opt_ctas_per_sm <= 0) {     // other CTA shapes: as many CTAs as fit
+            TG_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)sel->fn, threads, 0));
+            if (per_sm < 1) per_sm = 1;
+        }
         unsigned grid = (unsigned)(ctx->sm_count * per_sm);
         unsigned need = (unsigned)((ions->n + threads - 1) / threads);
         if (grid > need) grid = need;
@@ -765,6 +763,15 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
             TG_CUDA(ctx, cudaFuncSetAttribute((const void*)sel->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         }
         sel->fn<<<grid, threads, smem, st>>>(P);
+        cudaError_t le = cudaGetLastError();
+        if (le != cudaSuccess) {
+            cudaFuncAttributes fa;
+            memset(&fa, 0, sizeof(fa));
+            cudaFuncGetAttributes(&fa, (const void*)sel->fn);
+            TG_SET_ERR(ctx, "trace launch (%u x %d threads, %zu B dynamic smem; kernel: %d registers, max %d threads per block, %zu B static smem): %s",
+                       grid, threads, smem, fa.numRegs, fa.maxThreadsPerBlock, fa.sharedSizeBytes, cudaGetErrorString(le));
+            return TAIGA_E_CUDA;
+        }
     }
     ++launches;
     TG_CUDA(ctx, cudaGetLastError());

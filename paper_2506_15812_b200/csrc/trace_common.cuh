@@ -55,6 +55,14 @@ __device__ __forceinline__ double tg_rsqrt_sqrt(double a, double& root) {
     return fma(y * e, q, y);
 }
 
+// EARLY: the form above (kind 0: 31.62 -> 31.53 ms on BASELINE config 2); otherwise sqrt(a) = a / sqrt(a) after the correction,
+// one instruction fewer (the kind-1 kernel sits at the register limit and is 7 % slower with the early form)
+template <bool EARLY>
+__device__ __forceinline__ double tg_rsq(double a, double& root) {
+    if constexpr (EARLY) return tg_rsqrt_sqrt(a, root);
+    else { const double y = tg_rsqrt(a); root = a * y; return y; }
+}
+
 // t in [0,1)  <=>  sign 0 and exponent < 1023  <=>  (unsigned) hi word < 0x3FF00000
 __device__ __forceinline__ bool tg_in01(double t) { return (unsigned)__double2hiint(t) < 0x3FF00000u; }
 

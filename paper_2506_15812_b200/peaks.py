@@ -2,7 +2,8 @@
 
     python -m paper_2506_15812_b200.peaks [milliseconds per measurement]
 
-FP64 pipe (DFMA instructions / s), FP64 tensor pipe (DMMA.8x8x4, FMA / s) and the L1 -> register delivery rate of
+FP64 pipe (DFMA instructions / s), FP64 tensor pipe (DMMA.8x8x4, FMA / s), both interleaved (one datapath: the sum does
+not exceed either) and the L1 -> register delivery rate of
 256-bit gathers for 1 / 2 / 4 / 32 distinct cells per warp.  bench.py takes the first two live in every run.
 """
 import json
@@ -14,6 +15,7 @@ from . import taiga
 def measure(ms: float = 50.0, device: int = 0) -> dict:
     tg = taiga.Taiga(device)
     out = {"dfma_instr_per_s": tg.fp64_peak(ms), "dmma_fma_per_s": tg.dmma_peak(ms),
+           "dfma_plus_dmma_fma_per_s": tg.mixed_fp64_peak(ms),
            "nominal_fp64_instr_per_s": 148 * 64 * 1.965e9,
            "l1_gather_bytes_per_s": {str(k): tg.l1_gather_peak(ms, k) for k in (1, 2, 4, 32)}}
     tg.close()

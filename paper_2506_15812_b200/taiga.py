@@ -30,7 +30,8 @@ EXPORTS = ["taiga_create", "taiga_destroy", "taiga_last_error", "taiga_load_fiel
            "taiga_detector_histogram_weighted", "taiga_seed_beam_grid",
            "taiga_field_eval", "taiga_field_table", "taiga_seed_beam", "taiga_trace",
            "taiga_detector_histogram", "taiga_set_efield", "taiga_set_option", "taiga_get_stats",
-           "taiga_measure_fp64_peak", "taiga_measure_l1_gather_peak", "taiga_measure_dmma_peak", "taiga_loss_statistics"]
+           "taiga_measure_fp64_peak", "taiga_measure_l1_gather_peak", "taiga_measure_dmma_peak", "taiga_measure_mixed_fp64_peak",
+           "taiga_loss_statistics"]
 
 
 class GridS(C.Structure):
@@ -96,6 +97,7 @@ _lib.taiga_get_stats.argtypes = [C.c_void_p, C.POINTER(C.c_ulonglong * 8)]
 _lib.taiga_measure_fp64_peak.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
 _lib.taiga_measure_l1_gather_peak.argtypes = [C.c_void_p, C.c_double, C.c_int, C.POINTER(C.c_double)]
 _lib.taiga_measure_dmma_peak.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
+_lib.taiga_measure_mixed_fp64_peak.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
 _lib.taiga_loss_statistics.argtypes = [C.POINTER(C.c_ulonglong * 4), C.POINTER(C.c_double * 3)]
 
 
@@ -303,6 +305,11 @@ class Taiga:
     def dmma_peak(self, ms=50.0):
         r = C.c_double()
         self._chk(_lib.taiga_measure_dmma_peak(self.h, ms, C.byref(r)))
+        return r.value
+
+    def mixed_fp64_peak(self, ms=50.0):
+        r = C.c_double()
+        self._chk(_lib.taiga_measure_mixed_fp64_peak(self.h, ms, C.byref(r)))
         return r.value
 
 
