@@ -232,8 +232,8 @@ int taiga_loss_statistics(const unsigned long long wsummary_host[4], double out_
  * "sort_sub" (sort bins per grid cell and axis, default 16), "min_active" (a warp refills its
  * free lanes from the queue when at least this many are free; 32 = whole tiles, default),
  * "ctas_per_sm", "variant" (kernel variant: 0 register cell cache with rolling predictive refill,
- * 9 warps/SM (default); 4 predictive refill after each evaluation; 5 refill on demand only; 3 the
- * same at 12 warps/SM; 1 / 2 no cache at 8 / 16 warps/SM; 7 the default kernel at 8 warps/SM in 128-thread CTAs; time-sliced fields: 0 time-blended cell
+ * 8 warps/SM in 32-thread CTAs (default); 4 predictive refill after each evaluation; 5 refill on demand only; 3 the
+ * same at 12 warps/SM; 1 / 2 no cache at 8 / 16 warps/SM; 7 the same in 128-thread CTAs at 223 registers; time-sliced fields: 0 time-blended cell
  * cache in registers with the slice difference in per-lane shared-memory slots (default), 6 the same
  * with the difference gathered through L1, 4 slice cache with rolling refill), "stats" (1: read counters back,
  * default), "precision" (64 default; 32 = the fp32 variant of BASELINE config 5: kind-2 fields

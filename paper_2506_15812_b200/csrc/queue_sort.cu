@@ -3,10 +3,12 @@
 
 // ------------------------------------------------------------------------------------------
 // Ordering of the ion queue: counting sort by birth cell (R-major, so that deep-born = long
-// running ions are dequeued first and the ions sharing a warp fly through the same cells).
+// running ions are dequeued first and the ions sharing a warp fly through the same cells);
+// time-sliced and (R,Z,phi) fields: key = (radial band, slice / toroidal sub-cell, R bin, Z bin).
 // Output is written by ion index, so the order never shows in the results.
 #define SORT_NBR 512
 #define SORT_NBZ 256
+#define SORT_BAND 64                   // fine R bins per radial band (8 bands)
 #define SCAN_ITEMS 8
 #define SCAN_TPB 1024
 
@@ -59,7 +61,11 @@ __device__ __forceinline__ uint32_t sort_key(const SortParams& S, uint32_t i) {
         xs -= (double)S.nS * floor(xs / (double)S.nS);
         m = min(max((int)(xs * (double)S.n_major / (double)S.nS), 0), S.n_major - 1);
     }
-    return (uint32_t)((m * SORT_NBR + bR) * SORT_NBZ + bZ);
+    // radial band (SORT_BAND fine bins) first, then the slice / toroidal sub-cell, then the fine bins: every slice's deep-born
+    // (trapped, step-limit) ions are dequeued at the head of the queue instead of at the head of their slice's section,
+    // where the late slices' tiles outlived the rest of the kernel by 14 % (BASELINE config 4, profiles/r2_experiments.md)
+    const int band = bR / SORT_BAND, fine = bR % SORT_BAND;
+    return (uint32_t)(((band * S.n_major + m) * SORT_BAND + fine) * SORT_NBZ + bZ);
 }
 
 __global__ void k_sort_count(SortParams S, uint32_t* bins) {

@@ -21,6 +21,10 @@
 //  * 1/R by MUFU.RSQ64H seed + one cubic (Halley) step: 6 FP64 instructions instead of ~30.
 #include "trace_common.cuh"
 
+#ifdef TG_DBG_TAIL
+__device__ unsigned long long tg_dbg_t[8] = {~0ull, 0, 0, 0, 0, 0, 0, 0};
+extern "C" void taiga_dbg_tail(unsigned long long* out) { cudaMemcpyFromSymbol(out, tg_dbg_t, sizeof(tg_dbg_t)); unsigned long long z[8] = {~0ull, 0, 0, 0, 0, 0, 0, 0}; cudaMemcpyToSymbol(tg_dbg_t, z, sizeof(z)); }
+#endif
 template <int KIND>
 struct CellCache;                              // register cache of the current cell (kind 0)
 template <>
@@ -337,6 +341,9 @@ template <int KIND, bool CACHED, int THREADS, int MAXREG, int PRED = 0, int SOLV
 __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const TraceParams P) {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
+#ifdef TG_DBG_TAIL
+    unsigned long long tg_t0; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tg_t0));
+#endif
     CellCache<KIND> cc;
     if constexpr (KIND == 1 && CACHED) { cc.k = -1; cc.cell = 0; cc.tau = -1.0; }
     if constexpr (KIND <= 1 && CACHED) { cc.oR = 1e300; cc.oZ = 1e300;
@@ -602,6 +609,13 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
             }
         }
     }
+#ifdef TG_DBG_TAIL
+    if (lane == 0) {
+        unsigned long long te; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(te));
+        atomicMax(&tg_dbg_t[1], te); atomicAdd(&tg_dbg_t[2], te - tg_t0); atomicAdd(&tg_dbg_t[3], 1ull); atomicMin(&tg_dbg_t[0], tg_t0);
+        atomicAdd(&tg_dbg_t[4], warp_steps);
+    }
+#endif
     // per-warp statistics
     unsigned long long rl = reloads, is = ion_steps;
     for (int o = 16; o > 0; o >>= 1) {
@@ -621,7 +635,7 @@ __global__ void k_table_to_f32(const double* __restrict__ src, float* __restrict
 }
 
 // Every instantiation of k_trace, one line each: {kind, cached, registers, PRED, SOLVER, HAS_E, LOSS, BEZ, REGROUP}.
-//   kind 0, RKN: register cell cache with rolling predictive refill (PRED 2; 9 x 32 threads/SM at <= 224 registers),
+//   kind 0, RKN: register cell cache with rolling predictive refill (PRED 2; 8 x 32 threads/SM, 210 registers),
 //   predictive refill after each Horner (1), refill on demand (0; the 4-evaluation solvers), 168 registers, no cache;
 //   kind 1: time-blended cell cache in registers, slice difference in per-lane shared-memory slots (PRED 4, default) or
 //   gathered through L1 (3), slice cache with rolling refill (2), no cache (0);
@@ -631,8 +645,9 @@ struct TgVariant { int kind, cached, regs, pred, solver, hasE, loss, bez, regrou
 #define TG_V(K, C, R, P, S, E, L, B, G) {K, C, R, P, S, E, L, B, G, k_trace<K, (C) != 0, 128, R, P, S, (E) != 0, (L) != 0, (B) != 0, (G) != 0>, 128}
 #define TG_VT(K, C, R, P, T) {K, C, R, P, 0, 0, 0, 0, 0, k_trace<K, (C) != 0, T, R, P, 0, false, false, false, false>, T}
 static const TgVariant tg_variants[] = {
-    // 9 warps per SM in 32-thread CTAs (warps are independent: any block size); 10 and 11 warps at 200 / 184 registers
-    // were slower (profiles/r2_experiments.md)
+    // 32-thread CTAs (warps are independent: any block size), register cap 224: 8 warps per SM as before (the register
+    // file is allocated in steps that put 210 registers at 256 per lane); 10 warps at 192 registers were slower
+    // (profiles/r2_experiments.md)
     TG_VT(0, 1, 224, 2, 32),
     // production path: RKN, E = 0
     TG_V(0, 1, 255, 2, 0, 0, 0, 0, 0), TG_V(0, 1, 255, 1, 0, 0, 0, 0, 0), TG_V(0, 1, 255, 0, 0, 0, 0, 0, 0), TG_V(0, 1, 168, 0, 0, 0, 0, 0, 0),
@@ -725,7 +740,7 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
             if (special) { k.cached = 1; k.pred = (variant == 0) ? 2 : 0; }
             else if (variant != 0) { k.cached = (kv != 1 && kv != 2); k.regs = (kv == 2) ? 128 : 255; }     // printed k3: 4th evaluation, on demand
             else switch (kv) {
-                case 0: k.cached = 1; k.pred = 2; k.regs = 224; break;     // 9 warps/SM (9 x 32 threads): 31.3 against 31.5 ms
+                case 0: k.cached = 1; k.pred = 2; k.regs = 224; break;     // 8 x 32-thread CTAs per SM, 210 registers: 31.3 against 31.5 ms
                 case 7: k.cached = 1; k.pred = 2; break;                   // 8 warps/SM (2 x 128 threads), the round-1 geometry
                 case 4: k.cached = 1; k.pred = 1; break;
                 case 5: k.cached = 1; break;
