@@ -330,7 +330,11 @@ def main_ours(args):
         out["roofline"]["dmma_peak"] = 2e-12 * tg.dmma_peak(50.0)
         out["roofline"]["note"] = ("field evaluation on the FP64 tensor pipe (DMMA.8x8x4, same FMA rate as DFMA on B200: dmma_peak); "
                                    "frac counts the method's %d FP64 instructions per ion-step, not the padded tensor work" % int(alg))
-    if kind != 0 and not args.solver and not mma_on:
+    opts = {kv.split("=")[0].strip(): kv.split("=")[1].strip() for kv in args.opt}
+    # the kernels that still gather coefficients per lane through L1 (kind 2 with mma=0 / precision=32; kind 1 with the r1 / r2a
+    # variants) are reported against the measured L1 delivery rate; the default kernels against the FP64 rate
+    gathers = (kind == 2 and not mma_on) or (kind == 1 and not mma_on and opts.get("variant", "0") != "0")
+    if gathers and not args.solver:
         f32 = any(kv.strip() == "precision=32" for kv in args.opt)
         l1_peak = tg.l1_gather_peak(50.0, 1)
         l1_bytes = ALG_L1_BYTES_PER_ION_STEP[kind] * (0.5 if f32 else 1.0)

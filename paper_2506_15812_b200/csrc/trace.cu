@@ -21,10 +21,6 @@
 //  * 1/R by MUFU.RSQ64H seed + one cubic (Halley) step: 6 FP64 instructions instead of ~30.
 #include "trace_common.cuh"
 
-#ifdef TG_DBG_TAIL
-__device__ unsigned long long tg_dbg_t[8] = {~0ull, 0, 0, 0, 0, 0, 0, 0};
-extern "C" void taiga_dbg_tail(unsigned long long* out) { cudaMemcpyFromSymbol(out, tg_dbg_t, sizeof(tg_dbg_t)); unsigned long long z[8] = {~0ull, 0, 0, 0, 0, 0, 0, 0}; cudaMemcpyToSymbol(tg_dbg_t, z, sizeof(z)); }
-#endif
 template <int KIND>
 struct CellCache;                              // register cache of the current cell (kind 0)
 template <>
@@ -341,9 +337,6 @@ template <int KIND, bool CACHED, int THREADS, int MAXREG, int PRED = 0, int SOLV
 __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const TraceParams P) {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
-#ifdef TG_DBG_TAIL
-    unsigned long long tg_t0; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tg_t0));
-#endif
     CellCache<KIND> cc;
     if constexpr (KIND == 1 && CACHED) { cc.k = -1; cc.cell = 0; cc.tau = -1.0; }
     if constexpr (KIND <= 1 && CACHED) { cc.oR = 1e300; cc.oZ = 1e300;
@@ -609,13 +602,6 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
             }
         }
     }
-#ifdef TG_DBG_TAIL
-    if (lane == 0) {
-        unsigned long long te; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(te));
-        atomicMax(&tg_dbg_t[1], te); atomicAdd(&tg_dbg_t[2], te - tg_t0); atomicAdd(&tg_dbg_t[3], 1ull); atomicMin(&tg_dbg_t[0], tg_t0);
-        atomicAdd(&tg_dbg_t[4], warp_steps);
-    }
-#endif
     // per-warp statistics
     unsigned long long rl = reloads, is = ion_steps;
     for (int o = 16; o > 0; o >>= 1) {

@@ -28,10 +28,6 @@
 // birth-cell-ordered queue, so all warps stay full through the tail.
 #include "trace_common.cuh"
 
-#ifdef TG_DBG_CELLS
-__device__ unsigned long long tg_dbg[32];
-extern "C" void taiga_dbg_read(unsigned long long* out) { cudaMemcpyFromSymbol(out, tg_dbg, sizeof(tg_dbg)); unsigned long long z[32] = {0}; cudaMemcpyToSymbol(tg_dbg, z, sizeof(z)); }
-#endif
 #define TG_IDX(L) ((L) + 2 * ((L) >> 4))          // skewed slot of lane L: quad-strided 64-bit reads hit distinct banks
 #define TG_ROW 35                                 // row stride of the per-warp buffer: 34 slots; 35 = 3 mod 16 keeps the 16 lanes
                                                   // of a half-warp (rows r = 0..3 or 4..7, t = 0..3) on distinct 8-byte banks
@@ -155,14 +151,6 @@ __device__ __forceinline__ void tg_eval_mma(const TgLane& L, int cell, double p,
     __syncwarp();
     const int n_items = __popc(leaders);
     sets += n_items;
-#ifdef TG_DBG_CELLS
-    {   // distinct cells of this warp-evaluation and a histogram of the items per evaluation (debug statistics)
-        const unsigned mc = __match_any_sync(FULL, cell);
-        const unsigned lc = __ballot_sync(FULL, cell >= 0 && (mc & (0u - mc)) == (1u << L.lane));
-        if (L.lane == 0) { atomicAdd(&tg_dbg[0], (unsigned long long)__popc(lc)); atomicAdd(&tg_dbg[1], 1ull);
-                           atomicAdd(&tg_dbg[2 + (n_items < 29 ? n_items : 29)], 1ull); }
-    }
-#endif
     double b[KS][3], a[KS], qg = 0.0;
     int cs = 0;
     unsigned mem = 0, gofs = 0;
