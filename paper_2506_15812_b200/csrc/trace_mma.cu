@@ -565,7 +565,7 @@ static int tg_build_phi_tab(taiga_ctx* ctx, int nk) {
 
 // Launch geometry: THREADS per CTA (the pool the CTA re-sorts; 32 = every warp on its own, no CTA barrier) and the
 // register cap.  The kernel is latency-bound (throughput scales with resident warps up to the point where ptxas
-// spills: profiles/r2b_mma_kernel.md), so the grid is one persistent CTA per resident slot.
+// spills: profiles/r2_experiments.md), so the grid is one persistent CTA per resident slot.
 template <int KIND, int SOLVER, bool HAS_E, bool LOSS, bool BEZ, int THREADS = 128, int MAXREG = 168>
 static int tg_launch_mma_t(taiga_ctx* ctx, const TraceParams& P, int per_sm, uint64_t n, cudaStream_t st) {
     auto kern = k_trace_mma<KIND, THREADS, MAXREG, SOLVER, HAS_E, LOSS, BEZ>;
