@@ -248,7 +248,9 @@ int taiga_loss_statistics(const unsigned long long wsummary_host[4], double out_
  * every this many steps, so that the lanes of a warp / of an 8-ion group share cells; default 8; with mma = 0, 0 = off:
  * per-warp tiles), "refill_cta" (mma: the CTA refills its finished lanes from the queue at a re-sort point once this
  * many are free; default: all of them, i.e. whole tiles of consecutive queue entries, which keeps the ions of a CTA
- * in few cells -- 9.4e9 against 7.5e9 ion-steps/s with 16 on BASELINE config 5).  Values out of range are refused with TAIGA_E_ARG when set. */
+ * in few cells -- 9.4e9 against 7.5e9 ion-steps/s with 16 on BASELINE config 5), "mma_geom" (mma, plain RKN kernel: threads per
+ * CTA x register cap: 0 = 128 x 128, four CTAs per SM (default); 1 = 128 x 168; 2 = 64 x 144; 3 = 32 x 144; 4 = 32 x 128;
+ * 5 = 64 x 128).  Values out of range are refused with TAIGA_E_ARG when set. */
 int taiga_set_option(taiga_ctx* ctx, const char* key, long long value);
 /* counters of the last taiga_trace (valid with "stats" on): [0] ion-steps, [1] warp-steps*32
  * (lane slots issued), [2] 1, [3] kernel launches, [4] cell refills, [5..7] 0. */

@@ -564,8 +564,9 @@ static int tg_build_phi_tab(taiga_ctx* ctx, int nk) {
 }
 
 // Launch geometry: THREADS per CTA (the pool the CTA re-sorts; 32 = every warp on its own, no CTA barrier) and the
-// register cap.  The kernel is latency-bound (throughput scales with resident warps up to the point where ptxas
-// spills: profiles/r2_experiments.md), so the grid is one persistent CTA per resident slot.
+// register cap.  The kernel is latency-bound: throughput follows the resident warps, and 4 CTAs of 128 threads at 128
+// registers (40 B of spills) beat 3 at 148 registers by 6 % on BASELINE config 5 (profiles/r2_experiments.md), so the
+// production RKN kernel is capped at 128; the grid is one persistent CTA per resident slot.
 template <int KIND, int SOLVER, bool HAS_E, bool LOSS, bool BEZ, int THREADS = 128, int MAXREG = 168>
 static int tg_launch_mma_t(taiga_ctx* ctx, const TraceParams& P, int per_sm, uint64_t n, cudaStream_t st) {
     auto kern = k_trace_mma<KIND, THREADS, MAXREG, SOLVER, HAS_E, LOSS, BEZ>;
@@ -608,12 +609,12 @@ int tg_trace_mma(taiga_ctx* ctx, TraceParams& P, int solver, bool hasE, bool los
         else if (solver == 0 && hasE) TG_MMA(K, 0, true, false, false);       \
         else if (solver == 0) {                                               \
             switch (ctx->opt_mma_geom) {                                      \
-                case 1: TG_MMA(K, 0, false, false, false, 128, 128); break;   \
+                case 1: TG_MMA(K, 0, false, false, false, 128, 168); break;   \
                 case 2: TG_MMA(K, 0, false, false, false, 64, 144); break;    \
                 case 3: TG_MMA(K, 0, false, false, false, 32, 144); break;    \
                 case 4: TG_MMA(K, 0, false, false, false, 32, 128); break;    \
                 case 5: TG_MMA(K, 0, false, false, false, 64, 128); break;    \
-                default: TG_MMA(K, 0, false, false, false); break;            \
+                default: TG_MMA(K, 0, false, false, false, 128, 128); break;  \
             }                                                                 \
         } else if (solver == 2) TG_MMA(K, 2, true, false, false);             \
         else TG_MMA(K, 3, true, false, false);                                \
