@@ -134,6 +134,47 @@ def test_prefix_parity(tg, icfg, n):
     assert ngpu > 0
 
 
+@pytest.mark.parametrize("icfg,n,opts", [
+    (4, 96, dict(variant=6)),                      # kind 1: blended cache, slice difference gathered through L1 (r2a)
+    (4, 96, dict(variant=4)),                      # kind 1: slice cache with rolling refill (r1e)
+    (4, 96, dict(variant=1)),                      # kind 1: no cache
+    (4, 96, dict(mma=1)),                          # kind 1 on the DMMA tracer
+    (4, 96, dict(sort=0)),                         # queue in ion-index order (slices interleaved per tile boundary)
+    (5, 4096 + 5, dict(mma=0)),                    # kind 2: per-lane gathers with the CTA re-sort (r1e)
+    (5, 4096 + 5, dict(mma=0, regroup=0)),         # ... per-warp tiles
+    (5, 4096 + 5, dict(mma_geom=1)), (5, 4096 + 5, dict(mma_geom=2)), (5, 4096 + 5, dict(mma_geom=3)),
+    (5, 4096 + 5, dict(mma_geom=5)),
+    (5, 4096 + 5, dict(refill_cta=16, regroup=3)), (5, 4096 + 5, dict(sort=0)),
+])
+def test_kernel_options_of_the_sliced_fields(tg, icfg, n, opts):
+    """Every kernel variant and launch geometry `taiga_set_option` offers for the time-sliced and (R, Z, phi) tables
+    gives the oracle's result (the defaults are covered by the prefix and full-histogram tests)."""
+    from paper_2506_15812_b200 import taiga
+    for k, v in opts.items():
+        tg.set_option(k, v)
+    cfg = wl.config(icfg, n_override=n)
+    ions, counts, summary = taiga.run_config(tg, cfg)
+    torch.cuda.synchronize()
+    ref = orc.run_config(cfg)
+    st = compare_groups(ions, ref, "%s %s" % (cfg.name, opts))
+    check_histogram(cfg, ions, counts, summary, ref)
+    assert st["flagged"] <= 8, st
+
+
+def test_roofline_denominators_are_consistent(tg):
+    """The microkernels behind bench.py's roofline: the DFMA and DMMA issue rates are within 3 % of 148 x 64 FMA per clock
+    at the clock nvidia-smi reports as maximum, and interleaving both does not exceed either (one FP64 datapath)."""
+    import subprocess
+    mhz = float(subprocess.run(["nvidia-smi", "-i", "0", "--query-gpu=clocks.max.sm", "--format=csv,noheader,nounits"],
+                               capture_output=True, text=True).stdout.strip().splitlines()[0])
+    sm = torch.cuda.get_device_properties(0).multi_processor_count
+    nominal = sm * 64 * mhz * 1e6
+    dfma, dmma, mixed = tg.fp64_peak(30.0), tg.dmma_peak(30.0), tg.mixed_fp64_peak(30.0)
+    assert 0.90 * nominal < dfma < 1.03 * nominal, (dfma, nominal)
+    assert 0.90 * nominal < dmma < 1.03 * nominal, (dmma, nominal)
+    assert 0.5 * dfma < mixed < 1.03 * max(dfma, dmma), (mixed, dfma, dmma)
+
+
 @pytest.mark.parametrize("icfg,n", [(2, None), (3, 65536 + 21), (4, 2048 + 3), (5, 65536 + 77)])
 def test_full_histogram_parity(tg, icfg, n):
     """The method's output is the counters.  COMPLETE detector histograms + summary, bit for bit
