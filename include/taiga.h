@@ -167,7 +167,7 @@ typedef struct {
  *             v(t0) moved to t0 - dt/2 by one Boris push at the start (reading R2: "a
  *             second-order Verlet solver"),
  *         4 = Boris with Eq. 8 exactly as printed: r(t0+dt) = r(t0) + v(t0) dt (first order).
- * E of Eq. 3 is the uniform field set by taiga_set_efield (default 0). */
+ * E of Eq. 3 is the uniform field set by taiga_set_efield (default 0) plus the gridded field of taiga_load_efield (default none). */
 int taiga_trace(taiga_ctx* ctx, taiga_ions* ions, double q_over_m, double dt,
                 uint32_t max_steps, const taiga_detector* det, int solver);
 
@@ -175,6 +175,18 @@ int taiga_trace(taiga_ctx* ctx, taiga_ions* ions, double q_over_m, double dt,
  * for it"; verification scenarios 2 and 5, L279, L282).  Host pointer, copied.  Applies to all
  * later taiga_trace calls of this ctx; (0,0,0) restores the E = 0 production kernels. */
 int taiga_set_efield(taiga_ctx* ctx, const double E_V_per_m[3]);
+
+/* Gridded electric field E(R, Z) [V/m] of Eq. 3 (E(r); L177: the Cartesian coordinates "are mapped to a
+ * poloidal cross-section plane in each iteration step.  That is how the local magnetic and electric field is given"; L175:
+ * a parametric model of E near the wall is tabulated on the grid by the caller).  Reading E1: nodal values
+ * E_R, E_Z, E_phi on the (R, Z) nodes of the LOADED magnetic field's grid, c->form = 0, arrays [nR][nZ] (one static slice
+ * whatever the kind of B) in c->BR, c->BZ, c->Bphi, host or device (c->on_device); interpolated by the same not-a-knot
+ * bicubic spline as B (a1's kernels), the boundary cell extrapolating outside the grid, rotated to Cartesian components like
+ * B and ADDED to the uniform field of taiga_set_efield at every stage of every solver (Boris: at r(t0), as B).  c == NULL
+ * removes it.  Must follow taiga_load_field (TAIGA_E_STATE otherwise); a later taiga_load_field removes it.  The table is
+ * gathered per evaluation (48 coefficients through L1, no register cache): meant for edge studies, not for the production
+ * E = 0 path, whose kernels are unchanged.  Same restrictions as the uniform E (no loss model, no Bezier, fp64). */
+int taiga_load_efield(taiga_ctx* ctx, const taiga_coeffs* c);
 
 /* ---- a5: binning + histogram (segment ID per ion; atomically summed
  * per-segment counters; only the compact counter array is returned).

@@ -27,7 +27,7 @@ class Field(C.Structure):
     _fields_ = [("kind", C.c_int), ("nR", C.c_int), ("nZ", C.c_int), ("nS", C.c_int),
                 ("Rmin", C.c_double), ("Rmax", C.c_double), ("Zmin", C.c_double),
                 ("Zmax", C.c_double), ("s0", C.c_double), ("ds", C.c_double),
-                ("coef", _dp * 3), ("par", C.c_double * 8), ("E", C.c_double * 3)]
+                ("coef", _dp * 3), ("par", C.c_double * 8), ("E", C.c_double * 3), ("ecoef", _dp * 3)]
 
 
 class DetectorS(C.Structure):
@@ -98,9 +98,23 @@ def spline_periodic(y):
 class OracleField:
     """Spline-table field (kind 0/1/2) built from nodal grids, or an analytic pin field."""
 
-    def __init__(self, grid=None, nodal=None, kind=None, par=(), E=(0.0, 0.0, 0.0)):
+    def __init__(self, grid=None, nodal=None, kind=None, par=(), E=(0.0, 0.0, 0.0), E_nodal=None, E_grid=None):
+        """E: uniform electric field; E_nodal: (E_R, E_Z, E_phi) nodal values [nR][nZ] of a static gridded field on the
+        (R, Z) grid of `grid` (or of `E_grid` for the analytic pin fields)."""
         self.s = Field()
         self._keep = []
+        if E_nodal is not None:
+            g = grid if grid is not None else E_grid
+            self.etables = []
+            for c in range(3):
+                nod = np.ascontiguousarray(np.asarray(E_nodal[c], dtype=np.float64).reshape(1, g.nR, g.nZ))
+                tab = np.empty((1, g.nR - 1, g.nZ - 1, 16))
+                assert _lib.orc_build_tables(C.c_int(0), C.c_int(g.nR), C.c_int(g.nZ), C.c_int(1), _p(nod), _p(tab)) == 0
+                self.etables.append(tab)
+                self.s.ecoef[c] = _p(tab)
+            if grid is None:
+                self.s.nR, self.s.nZ, self.s.nS = g.nR, g.nZ, 1
+                self.s.Rmin, self.s.Rmax, self.s.Zmin, self.s.Zmax = g.Rmin, g.Rmax, g.Zmin, g.Zmax
         if grid is not None:
             g = grid
             self.s.kind, self.s.nR, self.s.nZ, self.s.nS = g.kind, g.nR, g.nZ, g.nS
@@ -127,6 +141,11 @@ class OracleField:
     def B(self, r, t=0.0):
         out = D3()
         _lib.orc_field_B(C.byref(self.s), D3(*r), C.c_double(t), out)
+        return np.array(out[:])
+
+    def E(self, r):
+        out = D3()
+        _lib.orc_field_E(C.byref(self.s), D3(*r), out)
         return np.array(out[:])
 
     def cyl(self, R, Z, s=0.0):

@@ -336,13 +336,35 @@ extern "C" void orc_field_B(const orc_field* f, const double r[3], double t, dou
     B[2] = Bc[1];
 }
 
+/* E(r) of Eq. 3 (L177: "mapped to a poloidal cross-section plane ... That is how the local magnetic
+ * and electric field is given"): the uniform vector plus, when given, a static field tabulated like B -- E_R, E_Z, E_phi
+ * on the (R, Z) grid, the same bicubic spline, the boundary cell extrapolating outside the grid (A12), rotated to
+ * Cartesian components like B (O0).  Reading E1 in DESIGN.md.                                                       */
+extern "C" void orc_field_E(const orc_field* f, const double r[3], double E[3]) {
+    E[0] = f->E[0]; E[1] = f->E[1]; E[2] = f->E[2];
+    if (!f->ecoef[0]) return;
+    const int cR = f->nR - 1, cZ = f->nZ - 1;
+    double hR = (f->Rmax - f->Rmin) / (double)cR, hZ = (f->Zmax - f->Zmin) / (double)cZ;
+    double R = std::sqrt(r[0] * r[0] + r[1] * r[1]);
+    double c = r[0] / R, s = r[1] / R;
+    double p, w, Ec[3];
+    int i = cell_index(R, f->Rmin, hR, f->nR, &p);
+    int j = cell_index(r[2], f->Zmin, hZ, f->nZ, &w);
+    size_t cell = (size_t)i * cZ + j;
+    for (int m = 0; m < 3; ++m) Ec[m] = bicubic(f->ecoef[m] + cell * 16, p, w);
+    E[0] = E[0] + (Ec[0] * c - Ec[2] * s);
+    E[1] = E[1] + (Ec[0] * s + Ec[2] * c);
+    E[2] = E[2] + Ec[1];
+}
+
 /* Eq. 3: a = (q/m)(E + v x B) */
 static inline void accel(const orc_field* f, double qm, const double r[3], const double v[3], double t, double a[3]) {
-    double B[3];
+    double B[3], E[3];
     orc_field_B(f, r, t, B);
-    a[0] = qm * (f->E[0] + (v[1] * B[2] - v[2] * B[1]));
-    a[1] = qm * (f->E[1] + (v[2] * B[0] - v[0] * B[2]));
-    a[2] = qm * (f->E[2] + (v[0] * B[1] - v[1] * B[0]));
+    orc_field_E(f, r, E);
+    a[0] = qm * (E[0] + (v[1] * B[2] - v[2] * B[1]));
+    a[1] = qm * (E[1] + (v[2] * B[0] - v[0] * B[2]));
+    a[2] = qm * (E[2] + (v[0] * B[1] - v[1] * B[0]));
 }
 
 /* O3  one Runge-Kutta-Nystrom step, Eq. 5-6 under readings A1-A3:
@@ -402,15 +424,16 @@ static inline void cross3(const double a[3], const double b[3], double c[3]) {
  *  v+ = v- + v* x s;  v' = v+ + (q/m) E h/2   (first line of Eq. 8).                         */
 static inline void boris_velocity(const orc_field* f, double qm, const double r[3], const double v[3],
                                   double t, double h, double vn[3]) {
-    double B[3], vm[3], tv[3], sv[3], vs[3], vp[3], c1[3], c2[3];
+    double B[3], E[3], vm[3], tv[3], sv[3], vs[3], vp[3], c1[3], c2[3];
     orc_field_B(f, r, t, B);
+    orc_field_E(f, r, E);
     double tt = 0.0;
-    for (int c = 0; c < 3; ++c) { vm[c] = v[c] + qm * f->E[c] * (h / 2.0); tv[c] = qm * B[c] * (h / 2.0); tt += tv[c] * tv[c]; }
+    for (int c = 0; c < 3; ++c) { vm[c] = v[c] + qm * E[c] * (h / 2.0); tv[c] = qm * B[c] * (h / 2.0); tt += tv[c] * tv[c]; }
     for (int c = 0; c < 3; ++c) sv[c] = 2.0 * tv[c] / (1.0 + tt);
     cross3(vm, tv, c1);
     for (int c = 0; c < 3; ++c) vs[c] = vm[c] + c1[c];
     cross3(vs, sv, c2);
-    for (int c = 0; c < 3; ++c) { vp[c] = vm[c] + c2[c]; vn[c] = vp[c] + qm * f->E[c] * (h / 2.0); }
+    for (int c = 0; c < 3; ++c) { vp[c] = vm[c] + c2[c]; vn[c] = vp[c] + qm * E[c] * (h / 2.0); }
 }
 /* Eq. 8, second line (L266): position.  As printed, r(t0+dt) = r(t0) + v(t0) dt uses the OLD
  * velocity: explicit Euler in r, first order, while the text calls the solver "a second-order

@@ -19,7 +19,7 @@
  * P18 Bezier plane interpolation: exact on parabolas, order 3; P19 weighted-grid seeding:
  * weights sum to 1, marginals = CDF increments, weighted detector image = stochastic image;
  * P20 stage times in a time-linear uniform field (closed-form rotation), Boris B(t_n), trace vs an ODE
- * solution; P21 weight domain of the fixed-point counters; P22 uniform-disc cross-section: radius bound,
+ * solution; P21 weight domain of the fixed-point counters; P23 gridded E: central-force invariants, constant grid = uniform E; P22 uniform-disc cross-section: radius bound,
  * r^2 law, uniform azimuth, second moments R^2/4, acceptance pi/4, retry counters.
  * Parity unpinned: nothing in this file; the paper's own figures that cannot be pinned
  * (Fig. 10 loss rate, Table 1, Fig. 12 curves) are listed in DESIGN.md.
@@ -47,6 +47,9 @@ typedef struct {
     const double* coef[3];   /* BR, BZ, Bphi per-cell power-basis tables (orc_build_tables) */
     double par[8];           /* analytic-field parameters */
     double E[3];             /* uniform electric field (Eq. 3; L175 "parametric modeling")  */
+    const double* ecoef[3];  /* gridded E_R, E_Z, E_phi (Eq. 3 E(r); L177: given on the poloidal plane like B): per-cell
+                              * power-basis tables of a static 2-D spline on the (R, Z) grid above, layout of kind 0
+                              * (orc_build_tables with kind 0, one slice); all three null = none (reading E1)            */
 } orc_field;
 
 /* secondary-ionisation loss inputs (Eq. 2): psi spline table of ONE component in
@@ -98,6 +101,8 @@ int orc_spline_periodic(int n, const double* y, double* c);
 int orc_build_tables(int kind, int nR, int nZ, int nS, const double* nodal, double* coef);
 /* O0/O1 field at a Cartesian point and time: B Cartesian */
 void orc_field_B(const orc_field* f, const double r[3], double t, double B[3]);
+/* E(r) of Eq. 3 in Cartesian components: the uniform vector plus the gridded field (reading E1) */
+void orc_field_E(const orc_field* f, const double r[3], double E[3]);
 /* field components in the poloidal plane, (B_R,B_Z,B_phi), s = time or phi */
 void orc_field_cyl(const orc_field* f, double R, double Z, double s, double Bc[3]);
 

@@ -270,7 +270,7 @@ int tg_precompute(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c) {
     f.inv_hR = 1.0 / hR; f.inv_hZ = 1.0 / hZ;
     f.offR = g->Rmin / hR; f.offZ = g->Zmin / hZ;
     f.s0 = g->s0; f.inv_ds = (g->kind == 0) ? 0.0 : 1.0 / g->ds;
-    f.table = ctx->table; f.table32 = nullptr; f.dtable = nullptr;
+    f.table = ctx->table; f.table32 = nullptr; f.dtable = nullptr; f.etable = nullptr;
     return TAIGA_OK;
 }
 
@@ -316,6 +316,42 @@ int tg_load_loss(taiga_ctx* ctx, const double* psi_nodal, int on_device, const t
     TG_CUDA(ctx, cudaStreamSynchronize(st));          // host profile arrays may be freed by the caller
     ctx->loss.psi = ctx->psi_table; ctx->loss.rate = ctx->loss_rate; ctx->loss.n = prof->n;
     ctx->loss.psi0 = prof->psi0; ctx->loss.inv_dpsi = 1.0 / prof->dpsi;
+    return TAIGA_OK;
+}
+
+// Gridded electric field (taiga_load_efield): three static 2-D components on the loaded grid, the kind-0 table layout,
+// built by the same stencil and assembly kernels as B.
+int tg_load_efield(taiga_ctx* ctx, const taiga_coeffs* c) {
+    FieldDev& f = ctx->field;
+    if (!c) { f.etable = nullptr; return TAIGA_OK; }
+    const int nR = f.nR, nZ = f.nZ;
+    const long long nnode = (long long)nR * nZ, ncell = (long long)f.cR * f.cZ;
+    cudaStream_t st = ctx->stream;
+    const int TPB = 128;
+    int rc = tg_reserve(ctx, &ctx->etable, &ctx->cap_etable, (size_t)ncell * 48);
+    if (rc) return rc;
+    size_t need = 12 * (size_t)nnode, scap = ctx->scratch_bytes / sizeof(double);
+    rc = tg_reserve(ctx, &ctx->scratch, &scap, need);
+    ctx->scratch_bytes = scap * sizeof(double);
+    if (rc) return rc;
+    double *y = ctx->scratch, *Mz = y + 3 * nnode, *Myr = Mz + 3 * nnode, *Mzr = Myr + 3 * nnode;
+    for (int ax = 0; ax < 2; ++ax) { rc = tg_ensure_band(ctx, ax, ax ? nR : nZ); if (rc) return rc; }
+    const double* src[3] = {c->BR, c->BZ, c->Bphi};
+    for (int m = 0; m < 3; ++m)
+        TG_CUDA(ctx, cudaMemcpyAsync(y + (size_t)m * nnode, src[m], nnode * sizeof(double),
+                                     c->on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+    long long tot = 3 * nnode;
+    unsigned gb = (unsigned)((tot + TPB - 1) / TPB);
+    k_second_deriv<<<gb, TPB, 0, st>>>(y, Mz, ctx->band[0], nZ, 1, tot);
+    k_second_deriv<<<gb, TPB, 0, st>>>(y, Myr, ctx->band[1], nR, nZ, tot);
+    k_second_deriv<<<gb, TPB, 0, st>>>(Mz, Mzr, ctx->band[1], nR, nZ, tot);
+    for (int m = 0; m < 3; ++m) {
+        size_t o = (size_t)m * nnode;
+        k_assemble<<<(unsigned)((ncell + TPB - 1) / TPB), TPB, 0, st>>>(y + o, Mz + o, Myr + o, Mzr + o, ctx->etable, 1, nR, nZ, m, 0);
+    }
+    TG_CUDA(ctx, cudaGetLastError());
+    if (!c->on_device) TG_CUDA(ctx, cudaStreamSynchronize(st));      // pageable or pinned host arrays may be reused by the caller
+    f.etable = ctx->etable;
     return TAIGA_OK;
 }
 

@@ -54,7 +54,7 @@ extern "C" int taiga_destroy(taiga_ctx* ctx) {
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     void* bufs[] = {ctx->table, ctx->scratch, ctx->band[0], ctx->band[1], ctx->cdf_depth, ctx->cdf_normal, ctx->edges, ctx->order,
-                    ctx->bins, ctx->counters, ctx->table32, ctx->psi_table, ctx->loss_rate, ctx->dtable, ctx->frag, ctx->phi_tab};
+                    ctx->bins, ctx->counters, ctx->table32, ctx->psi_table, ctx->loss_rate, ctx->dtable, ctx->frag, ctx->phi_tab, ctx->etable};
     for (void* b : bufs) if (b) cudaFree(b);
     if (ctx->counters_host) cudaFreeHost(ctx->counters_host);
     if (ctx->stage) cudaFreeHost(ctx->stage);
@@ -214,6 +214,17 @@ extern "C" int taiga_set_efield(taiga_ctx* ctx, const double E[3]) {
     for (int c = 0; c < 3; ++c) if (!isfinite(E[c])) { TG_SET_ERR(ctx, "set_efield: non-finite component"); return TAIGA_E_ARG; }
     for (int c = 0; c < 3; ++c) ctx->E[c] = E[c];
     return TAIGA_OK;
+}
+
+extern "C" int taiga_load_efield(taiga_ctx* ctx, const taiga_coeffs* c) {
+    if (!ctx) return TAIGA_E_ARG;
+    if (!ctx->field_loaded) { TG_SET_ERR(ctx, "load_efield: no magnetic field loaded (its grid carries E)"); return TAIGA_E_STATE; }
+    if (c && (c->form != 0 || !c->BR || !c->BZ || !c->Bphi)) {
+        TG_SET_ERR(ctx, "load_efield: nodal values (form 0) of E_R, E_Z, E_phi on the (R, Z) grid");
+        return TAIGA_E_ARG;
+    }
+    TG_CUDA(ctx, cudaSetDevice(ctx->device));
+    return tg_load_efield(ctx, c);
 }
 
 extern "C" int taiga_detector_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,

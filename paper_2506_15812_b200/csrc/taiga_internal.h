@@ -21,6 +21,7 @@ struct FieldDev {
     const double* table;
     const double* dtable;            // kind 1: slice differences [iR][iZ][k < nS-1][comp][16] = table[k+1] - table[k]
     const float* table32;            // kind 2, "precision" = 32: the same table rounded to fp32 (else null)
+    const double* etable;            // gridded E (taiga_load_efield): [iR][iZ][comp E_R, E_Z, E_phi][16], else null
 };
 
 // secondary-ionisation loss model (taiga_load_loss); psi == nullptr: none
@@ -53,6 +54,7 @@ struct taiga_ctx {
     double* band[2];          size_t band_cap[2]; int band_n[2];   // y -> y'' band operators (Z, R)
 
     double E[3];                                         // uniform electric field (taiga_set_efield), V/m
+    double* etable;           size_t cap_etable;         // gridded electric field (taiga_load_efield); field.etable = null: none
 
     // loss model
     LossDev loss;
@@ -135,6 +137,7 @@ int tg_field_eval(taiga_ctx* ctx, uint64_t n, const double* R, const double* Z, 
                   double* BR, double* BZ, double* Bp);
 int tg_field_table(taiga_ctx* ctx, int comp, double* host);
 int tg_load_loss(taiga_ctx* ctx, const double* psi_nodal, int on_device, const taiga_loss_profile* prof);
+int tg_load_efield(taiga_ctx* ctx, const taiga_coeffs* c);        // field_precompute.cu
 int tg_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
                           unsigned long long* wcounts, unsigned long long* wsummary);
 int tg_fp64_peak(taiga_ctx* ctx, double ms, double* rate);

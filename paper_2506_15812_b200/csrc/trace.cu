@@ -477,7 +477,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 if constexpr (PRED == 1) tg_predict(P, cc, reloads, tR + dR, tZ + dZ, BR, Bz, Bp);
                 tg_rotate(X, Y, rinv, BR, Bp, Bx, By);
                 double k1x = fma(Uy, Bz, -(Uz * By)), k1y = fma(Uz, Bx, -(Ux * Bz)), k1z = fma(Ux, By, -(Uy * Bx));
-                if constexpr (HAS_E) { k1x += P.qE[0]; k1y += P.qE[1]; k1z += P.qE[2]; }
+                if constexpr (HAS_E) tg_add_qE(P, X, Y, Z, k1x, k1y, k1z);
                 // ---- stage 2 (and 3, classical: same position)
                 double Xm = fma(k1x, P.a2, fma(Ux, P.a1, X)), Ym = fma(k1y, P.a2, fma(Uy, P.a1, Y)), Zm = fma(k1z, P.a2, fma(Uz, P.a1, Z));
                 double ux = fma(k1x, P.b1, Ux), uy = fma(k1y, P.b1, Uy), uz = fma(k1z, P.b1, Uz);
@@ -489,7 +489,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 if constexpr (PRED == 1) tg_predict(P, cc, reloads, tR + dR, tZ + dZ, BR, Bz, Bp);
                 tg_rotate(Xm, Ym, rinv, BR, Bp, Bx, By);
                 double k2x = fma(uy, Bz, -(uz * By)), k2y = fma(uz, Bx, -(ux * Bz)), k2z = fma(ux, By, -(uy * Bx));
-                if constexpr (HAS_E) { k2x += P.qE[0]; k2y += P.qE[1]; k2z += P.qE[2]; }
+                if constexpr (HAS_E) tg_add_qE(P, Xm, Ym, Zm, k2x, k2y, k2z);
                 ux = fma(k2x, P.b1, Ux); uy = fma(k2y, P.b1, Uy); uz = fma(k2z, P.b1, Uz);
                 if (P.variant) {               // printed Eq. 6: k3 position increment from k2
                     Xm = fma(k2x, P.a2, fma(Ux, P.a1, X)); Ym = fma(k2y, P.a2, fma(Uy, P.a1, Y)); Zm = fma(k2z, P.a2, fma(Uz, P.a1, Z));
@@ -500,7 +500,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                     tg_rotate(Xm, Ym, rinv, BR, Bp, Bx, By);
                 }
                 double k3x = fma(uy, Bz, -(uz * By)), k3y = fma(uz, Bx, -(ux * Bz)), k3z = fma(ux, By, -(uy * Bx));
-                if constexpr (HAS_E) { k3x += P.qE[0]; k3y += P.qE[1]; k3z += P.qE[2]; }
+                if constexpr (HAS_E) tg_add_qE(P, Xm, Ym, Zm, k3x, k3y, k3z);
                 // ---- stage 4
                 double Xe = fma(k3x, 4.0 * P.a2, fma(Ux, 2.0 * P.a1, X)), Ye = fma(k3y, 4.0 * P.a2, fma(Uy, 2.0 * P.a1, Y)),
                        Ze = fma(k3z, 4.0 * P.a2, fma(Uz, 2.0 * P.a1, Z));
@@ -511,7 +511,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 else tg_fieldCyl<KIND, CACHED>(P, cc, reloads, dummy, Xe, Ye, Ze, t + P.dt, R, BR, Bz, Bp, tR, tZ);
                 tg_rotate(Xe, Ye, rinv, BR, Bp, Bx, By);
                 double k4x = fma(uy, Bz, -(uz * By)), k4y = fma(uz, Bx, -(ux * Bz)), k4z = fma(ux, By, -(uy * Bx));
-                if constexpr (HAS_E) { k4x += P.qE[0]; k4y += P.qE[1]; k4z += P.qE[2]; }
+                if constexpr (HAS_E) tg_add_qE(P, Xe, Ye, Ze, k4x, k4y, k4z);
                 // ---- Eq. 5
                 double Tx = k2x + k3x, Ty = k2y + k3y, Tz = k2z + k3z;
                 Xn = fma(k1x + Tx, P.c6, fma(Ux, P.dtq, X)); Yn = fma(k1y + Ty, P.c6, fma(Uy, P.dtq, Y));
@@ -525,18 +525,23 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                     // ---- Eq. 4: classical RK4 on y = (r, v); with u = (q/m) v and k = dv/dt:
                     //  r2 = r + v dt/2;            r3 = r + v dt/2 + k1 dt^2/4;   r4 = r + v dt + k2 dt^2/2
                     //  r' = r + v dt + (k1+k2+k3) dt^2/6;   v' = v + (k1+2k2+2k3+k4) dt/6
-                    double k1x = fma(Uy, Bz, -(Uz * By)) + P.qE[0], k1y = fma(Uz, Bx, -(Ux * Bz)) + P.qE[1], k1z = fma(Ux, By, -(Uy * Bx)) + P.qE[2];
+                    double k1x = fma(Uy, Bz, -(Uz * By)), k1y = fma(Uz, Bx, -(Ux * Bz)), k1z = fma(Ux, By, -(Uy * Bx));
+                    tg_add_qE(P, X, Y, Z, k1x, k1y, k1z);
                     double ux = fma(k1x, P.b1, Ux), uy = fma(k1y, P.b1, Uy), uz = fma(k1z, P.b1, Uz);
-                    tg_fieldXYZ<KIND, CACHED>(P, cc, reloads, fma(Ux, P.a1, X), fma(Uy, P.a1, Y), fma(Uz, P.a1, Z), t + 0.5 * P.dt, Bx, By, Bz);
-                    double k2x = fma(uy, Bz, -(uz * By)) + P.qE[0], k2y = fma(uz, Bx, -(ux * Bz)) + P.qE[1], k2z = fma(ux, By, -(uy * Bx)) + P.qE[2];
+                    double Xs = fma(Ux, P.a1, X), Ys = fma(Uy, P.a1, Y), Zs = fma(Uz, P.a1, Z);
+                    tg_fieldXYZ<KIND, CACHED>(P, cc, reloads, Xs, Ys, Zs, t + 0.5 * P.dt, Bx, By, Bz);
+                    double k2x = fma(uy, Bz, -(uz * By)), k2y = fma(uz, Bx, -(ux * Bz)), k2z = fma(ux, By, -(uy * Bx));
+                    tg_add_qE(P, Xs, Ys, Zs, k2x, k2y, k2z);
                     ux = fma(k2x, P.b1, Ux); uy = fma(k2y, P.b1, Uy); uz = fma(k2z, P.b1, Uz);
-                    tg_fieldXYZ<KIND, CACHED>(P, cc, reloads, fma(k1x, 2.0 * P.a2, fma(Ux, P.a1, X)), fma(k1y, 2.0 * P.a2, fma(Uy, P.a1, Y)),
-                            fma(k1z, 2.0 * P.a2, fma(Uz, P.a1, Z)), t + 0.5 * P.dt, Bx, By, Bz);
-                    double k3x = fma(uy, Bz, -(uz * By)) + P.qE[0], k3y = fma(uz, Bx, -(ux * Bz)) + P.qE[1], k3z = fma(ux, By, -(uy * Bx)) + P.qE[2];
+                    Xs = fma(k1x, 2.0 * P.a2, fma(Ux, P.a1, X)); Ys = fma(k1y, 2.0 * P.a2, fma(Uy, P.a1, Y)); Zs = fma(k1z, 2.0 * P.a2, fma(Uz, P.a1, Z));
+                    tg_fieldXYZ<KIND, CACHED>(P, cc, reloads, Xs, Ys, Zs, t + 0.5 * P.dt, Bx, By, Bz);
+                    double k3x = fma(uy, Bz, -(uz * By)), k3y = fma(uz, Bx, -(ux * Bz)), k3z = fma(ux, By, -(uy * Bx));
+                    tg_add_qE(P, Xs, Ys, Zs, k3x, k3y, k3z);
                     ux = fma(k3x, 2.0 * P.b1, Ux); uy = fma(k3y, 2.0 * P.b1, Uy); uz = fma(k3z, 2.0 * P.b1, Uz);
-                    tg_fieldXYZ<KIND, CACHED>(P, cc, reloads, fma(k2x, 4.0 * P.a2, fma(Ux, 2.0 * P.a1, X)), fma(k2y, 4.0 * P.a2, fma(Uy, 2.0 * P.a1, Y)),
-                            fma(k2z, 4.0 * P.a2, fma(Uz, 2.0 * P.a1, Z)), t + P.dt, Bx, By, Bz);
-                    double k4x = fma(uy, Bz, -(uz * By)) + P.qE[0], k4y = fma(uz, Bx, -(ux * Bz)) + P.qE[1], k4z = fma(ux, By, -(uy * Bx)) + P.qE[2];
+                    Xs = fma(k2x, 4.0 * P.a2, fma(Ux, 2.0 * P.a1, X)); Ys = fma(k2y, 4.0 * P.a2, fma(Uy, 2.0 * P.a1, Y)); Zs = fma(k2z, 4.0 * P.a2, fma(Uz, 2.0 * P.a1, Z));
+                    tg_fieldXYZ<KIND, CACHED>(P, cc, reloads, Xs, Ys, Zs, t + P.dt, Bx, By, Bz);
+                    double k4x = fma(uy, Bz, -(uz * By)), k4y = fma(uz, Bx, -(ux * Bz)), k4z = fma(ux, By, -(uy * Bx));
+                    tg_add_qE(P, Xs, Ys, Zs, k4x, k4y, k4z);
                     double Tx = k2x + k3x, Ty = k2y + k3y, Tz = k2z + k3z;
                     Xn = fma(k1x + Tx, P.c6, fma(Ux, P.dtq, X)); Yn = fma(k1y + Ty, P.c6, fma(Uy, P.dtq, Y));
                     Zn = fma(k1z + Tz, P.c6, fma(Uz, P.dtq, Z));
@@ -546,15 +551,21 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 } else {
                     // ---- Eq. 7-8: Boris push with B, E at r(t0).  In u = (q/m) v units:
                     //  u- = u + eh;  t = B (q/m) h/2;  s = 2t/(1+t.t);  u* = u- + u- x t;  u+ = u- + u* x s;  u' = u+ + eh
+                    double eh0 = P.eh[0], eh1 = P.eh[1], eh2 = P.eh[2];      // half kick (q/m)^2 E dt/2 with E at r(t0)
+                    if (P.f.etable) {
+                        double gx = 0.0, gy = 0.0, gz = 0.0;
+                        tg_add_qE(P, X, Y, Z, gx, gy, gz);
+                        eh0 = gx * P.b1; eh1 = gy * P.b1; eh2 = gz * P.b1;
+                    }
                     auto push = [&](double hb, double he) {      // hb = (q/m) h/2, he = h/dt
-                        double ax = fma(he, P.eh[0], Ux), ay = fma(he, P.eh[1], Uy), az = fma(he, P.eh[2], Uz);
+                        double ax = fma(he, eh0, Ux), ay = fma(he, eh1, Uy), az = fma(he, eh2, Uz);
                         double tx = Bx * hb, ty = By * hb, tz = Bz * hb;
                         double sc = 2.0 / (1.0 + fma(tx, tx, fma(ty, ty, tz * tz)));
                         double bx = ax + fma(ay, tz, -(az * ty)), by = ay + fma(az, tx, -(ax * tz)), bz = az + fma(ax, ty, -(ay * tx));
                         double sx = tx * sc, sy = ty * sc, sz = tz * sc;
-                        Ux = fma(he, P.eh[0], ax + fma(by, sz, -(bz * sy)));
-                        Uy = fma(he, P.eh[1], ay + fma(bz, sx, -(bx * sz)));
-                        Uz = fma(he, P.eh[2], az + fma(bx, sy, -(by * sx)));
+                        Ux = fma(he, eh0, ax + fma(by, sz, -(bz * sy)));
+                        Uy = fma(he, eh1, ay + fma(bz, sx, -(bx * sz)));
+                        Uz = fma(he, eh2, az + fma(bx, sy, -(by * sx)));
                     };
                     if (nst == 0 && P.variant == 3) push(-0.5 * P.b1, -0.5);   // leap-frog start: v(t0) -> v(t0 - dt/2)
                     double ox = Ux, oy = Uy, oz = Uz;
@@ -661,6 +672,7 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     const bool f32 = ctx->opt_precision == 32;
     bool hasE = false;
     for (int c = 0; c < 3; ++c) hasE |= ctx->E[c] != 0.0;
+    hasE |= ctx->field.etable != nullptr;          // gridded E (taiga_load_efield)
     // ---- what is offered (checked before anything is enqueued)
     if (f32 && (kind != 2 || variant > 1)) {
         TG_SET_ERR(ctx, "precision=32 is offered for kind-2 (R,Z,phi) fields with the RKN solver only");

@@ -73,6 +73,25 @@ __device__ __forceinline__ void tg_rotate(double X, double Y, double rinv, doubl
     By = fma(BR, s_, Bp * c);
 }
 
+// Acceleration (q/m) E(r) of Eq. 3 added to (ax, ay, az): the uniform field (P.qE) plus, when loaded, the gridded
+// E_R, E_Z, E_phi of taiga_load_efield: located and gathered per evaluation (boundary cell extrapolates), rotated to
+// Cartesian components like B (O0).  PAPER.md L172-177, reading E1.
+__device__ __forceinline__ void tg_add_qE(const TraceParams& P, double Xs, double Ys, double Zs, double& ax, double& ay, double& az) {
+    double ex = P.qE[0], ey = P.qE[1], ez = P.qE[2];
+    if (P.f.etable) {
+        const double R2 = fma(Xs, Xs, Ys * Ys), ri = tg_rsqrt(R2), Rs = R2 * ri;
+        double p, w;
+        const int i = tg_locate(Rs, P.f.inv_hR, P.f.offR, P.f.cR, p);
+        const int j = tg_locate(Zs, P.f.inv_hZ, P.f.offZ, P.f.cZ, w);
+        const double* c = P.f.etable + ((size_t)i * P.f.cZ + j) * 48;
+        const double eR = tg_bicubic(c, p, w), eZ = tg_bicubic(c + 16, p, w), eP = tg_bicubic(c + 32, p, w);
+        double gx, gy;
+        tg_rotate(Xs, Ys, ri, eR, eP, gx, gy);
+        ex = fma(P.qm, gx, ex); ey = fma(P.qm, gy, ey); ez = fma(P.qm, eZ, ez);
+    }
+    ax += ex; ay += ey; az += ez;
+}
+
 // nu(psi(R,Z)): psi from its bicubic table (boundary cell extrapolates), the rate
 // profile linear in psi between its points, held constant outside.
 __device__ __forceinline__ double tg_loss_rate(const TraceParams& P, double R, double Z) {

@@ -353,7 +353,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
             double Xm = 0, Ym = 0, Zm = 0, ux = 0, uy = 0, uz = 0, Rd;
             if (alive) {
                 k1x = fma(Uy, Bz, -(Uz * By)); k1y = fma(Uz, Bx, -(Ux * Bz)); k1z = fma(Ux, By, -(Uy * Bx));
-                if constexpr (HAS_E) { k1x += P.qE[0]; k1y += P.qE[1]; k1z += P.qE[2]; }
+                if constexpr (HAS_E) tg_add_qE(P, X, Y, Z, k1x, k1y, k1z);
                 Xm = fma(k1x, P.a2, fma(Ux, P.a1, X)); Ym = fma(k1y, P.a2, fma(Uy, P.a1, Y)); Zm = fma(k1z, P.a2, fma(Uz, P.a1, Z));
                 ux = fma(k1x, P.b1, Ux); uy = fma(k1y, P.b1, Uy); uz = fma(k1z, P.b1, Uz);
             }
@@ -361,7 +361,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
             field(Xm, Ym, Zm, tm, Bx, By, Bz, Rd);             // stage 2 (and 3, classical: same position)
             if (alive) {
                 k2x = fma(uy, Bz, -(uz * By)); k2y = fma(uz, Bx, -(ux * Bz)); k2z = fma(ux, By, -(uy * Bx));
-                if constexpr (HAS_E) { k2x += P.qE[0]; k2y += P.qE[1]; k2z += P.qE[2]; }
+                if constexpr (HAS_E) tg_add_qE(P, Xm, Ym, Zm, k2x, k2y, k2z);
                 ux = fma(k2x, P.b1, Ux); uy = fma(k2y, P.b1, Uy); uz = fma(k2z, P.b1, Uz);
             }
             if (P.variant) {                   // printed Eq. 6: k3 position increment from k2 (kernel-uniform)
@@ -371,7 +371,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
             double Xe = 0, Ye = 0, Ze = 0;
             if (alive) {
                 k3x = fma(uy, Bz, -(uz * By)); k3y = fma(uz, Bx, -(ux * Bz)); k3z = fma(ux, By, -(uy * Bx));
-                if constexpr (HAS_E) { k3x += P.qE[0]; k3y += P.qE[1]; k3z += P.qE[2]; }
+                if constexpr (HAS_E) tg_add_qE(P, Xm, Ym, Zm, k3x, k3y, k3z);
                 Xe = fma(k3x, 4.0 * P.a2, fma(Ux, 2.0 * P.a1, X)); Ye = fma(k3y, 4.0 * P.a2, fma(Uy, 2.0 * P.a1, Y));
                 Ze = fma(k3z, 4.0 * P.a2, fma(Uz, 2.0 * P.a1, Z));
                 ux = fma(k3x, 2.0 * P.b1, Ux); uy = fma(k3y, 2.0 * P.b1, Uy); uz = fma(k3z, 2.0 * P.b1, Uz);
@@ -379,7 +379,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
             field(Xe, Ye, Ze, t + P.dt, Bx, By, Bz, Rd);       // stage 4
             if (alive) {
                 double k4x = fma(uy, Bz, -(uz * By)), k4y = fma(uz, Bx, -(ux * Bz)), k4z = fma(ux, By, -(uy * Bx));
-                if constexpr (HAS_E) { k4x += P.qE[0]; k4y += P.qE[1]; k4z += P.qE[2]; }
+                if constexpr (HAS_E) tg_add_qE(P, Xe, Ye, Ze, k4x, k4y, k4z);
                 double Tx = k2x + k3x, Ty = k2y + k3y, Tz = k2z + k3z;
                 Xn = fma(k1x + Tx, P.c6, fma(Ux, P.dtq, X)); Yn = fma(k1y + Ty, P.c6, fma(Uy, P.dtq, Y));
                 Zn = fma(k1z + Tz, P.c6, fma(Uz, P.dtq, Z));
@@ -392,25 +392,29 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
             double k1x = 0, k1y = 0, k1z = 0, k2x = 0, k2y = 0, k2z = 0, k3x = 0, k3y = 0, k3z = 0;
             double Xs = 0, Ys = 0, Zs = 0, ux = 0, uy = 0, uz = 0, Rd;
             if (alive) {
-                k1x = fma(Uy, Bz, -(Uz * By)) + P.qE[0]; k1y = fma(Uz, Bx, -(Ux * Bz)) + P.qE[1]; k1z = fma(Ux, By, -(Uy * Bx)) + P.qE[2];
+                k1x = fma(Uy, Bz, -(Uz * By)); k1y = fma(Uz, Bx, -(Ux * Bz)); k1z = fma(Ux, By, -(Uy * Bx));
+                tg_add_qE(P, X, Y, Z, k1x, k1y, k1z);
                 ux = fma(k1x, P.b1, Ux); uy = fma(k1y, P.b1, Uy); uz = fma(k1z, P.b1, Uz);
                 Xs = fma(Ux, P.a1, X); Ys = fma(Uy, P.a1, Y); Zs = fma(Uz, P.a1, Z);
             }
             field(Xs, Ys, Zs, t + 0.5 * P.dt, Bx, By, Bz, Rd);
             if (alive) {
-                k2x = fma(uy, Bz, -(uz * By)) + P.qE[0]; k2y = fma(uz, Bx, -(ux * Bz)) + P.qE[1]; k2z = fma(ux, By, -(uy * Bx)) + P.qE[2];
+                k2x = fma(uy, Bz, -(uz * By)); k2y = fma(uz, Bx, -(ux * Bz)); k2z = fma(ux, By, -(uy * Bx));
+                tg_add_qE(P, Xs, Ys, Zs, k2x, k2y, k2z);
                 ux = fma(k2x, P.b1, Ux); uy = fma(k2y, P.b1, Uy); uz = fma(k2z, P.b1, Uz);
                 Xs = fma(k1x, 2.0 * P.a2, fma(Ux, P.a1, X)); Ys = fma(k1y, 2.0 * P.a2, fma(Uy, P.a1, Y)); Zs = fma(k1z, 2.0 * P.a2, fma(Uz, P.a1, Z));
             }
             field(Xs, Ys, Zs, t + 0.5 * P.dt, Bx, By, Bz, Rd);
             if (alive) {
-                k3x = fma(uy, Bz, -(uz * By)) + P.qE[0]; k3y = fma(uz, Bx, -(ux * Bz)) + P.qE[1]; k3z = fma(ux, By, -(uy * Bx)) + P.qE[2];
+                k3x = fma(uy, Bz, -(uz * By)); k3y = fma(uz, Bx, -(ux * Bz)); k3z = fma(ux, By, -(uy * Bx));
+                tg_add_qE(P, Xs, Ys, Zs, k3x, k3y, k3z);
                 ux = fma(k3x, 2.0 * P.b1, Ux); uy = fma(k3y, 2.0 * P.b1, Uy); uz = fma(k3z, 2.0 * P.b1, Uz);
                 Xs = fma(k2x, 4.0 * P.a2, fma(Ux, 2.0 * P.a1, X)); Ys = fma(k2y, 4.0 * P.a2, fma(Uy, 2.0 * P.a1, Y)); Zs = fma(k2z, 4.0 * P.a2, fma(Uz, 2.0 * P.a1, Z));
             }
             field(Xs, Ys, Zs, t + P.dt, Bx, By, Bz, Rd);
             if (alive) {
-                double k4x = fma(uy, Bz, -(uz * By)) + P.qE[0], k4y = fma(uz, Bx, -(ux * Bz)) + P.qE[1], k4z = fma(ux, By, -(uy * Bx)) + P.qE[2];
+                double k4x = fma(uy, Bz, -(uz * By)), k4y = fma(uz, Bx, -(ux * Bz)), k4z = fma(ux, By, -(uy * Bx));
+                tg_add_qE(P, Xs, Ys, Zs, k4x, k4y, k4z);
                 double Tx = k2x + k3x, Ty = k2y + k3y, Tz = k2z + k3z;
                 Xn = fma(k1x + Tx, P.c6, fma(Ux, P.dtq, X)); Yn = fma(k1y + Ty, P.c6, fma(Uy, P.dtq, Y));
                 Zn = fma(k1z + Tz, P.c6, fma(Uz, P.dtq, Z));
@@ -421,15 +425,21 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
         } else {
             // Eq. 7-8: Boris push with B, E at r(t0); see trace.cu
             if (alive) {
+                double eh0 = P.eh[0], eh1 = P.eh[1], eh2 = P.eh[2];      // half kick (q/m)^2 E dt/2 with E at r(t0)
+                if (P.f.etable) {
+                    double gx = 0.0, gy = 0.0, gz = 0.0;
+                    tg_add_qE(P, X, Y, Z, gx, gy, gz);
+                    eh0 = gx * P.b1; eh1 = gy * P.b1; eh2 = gz * P.b1;
+                }
                 auto push = [&](double hb, double he) {      // hb = (q/m) h/2, he = h/dt
-                    double ax = fma(he, P.eh[0], Ux), ay = fma(he, P.eh[1], Uy), az = fma(he, P.eh[2], Uz);
+                    double ax = fma(he, eh0, Ux), ay = fma(he, eh1, Uy), az = fma(he, eh2, Uz);
                     double tx = Bx * hb, ty = By * hb, tz = Bz * hb;
                     double sc = 2.0 / (1.0 + fma(tx, tx, fma(ty, ty, tz * tz)));
                     double bx = ax + fma(ay, tz, -(az * ty)), by = ay + fma(az, tx, -(ax * tz)), bz = az + fma(ax, ty, -(ay * tx));
                     double sx = tx * sc, sy = ty * sc, sz = tz * sc;
-                    Ux = fma(he, P.eh[0], ax + fma(by, sz, -(bz * sy)));
-                    Uy = fma(he, P.eh[1], ay + fma(bz, sx, -(bx * sz)));
-                    Uz = fma(he, P.eh[2], az + fma(bx, sy, -(by * sx)));
+                    Ux = fma(he, eh0, ax + fma(by, sz, -(bz * sy)));
+                    Uy = fma(he, eh1, ay + fma(bz, sx, -(bx * sz)));
+                    Uz = fma(he, eh2, az + fma(bx, sy, -(by * sx)));
                 };
                 if (nst == 0 && P.variant == 3) push(-0.5 * P.b1, -0.5);   // leap-frog start: v(t0) -> v(t0 - dt/2)
                 double ox = Ux, oy = Uy, oz = Uz;

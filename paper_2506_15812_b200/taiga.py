@@ -29,7 +29,7 @@ FLAG_EDGE, FLAG_PLANE, FLAG_GRID = 1, 2, 4
 EXPORTS = ["taiga_create", "taiga_destroy", "taiga_last_error", "taiga_load_field", "taiga_load_loss",
            "taiga_detector_histogram_weighted", "taiga_seed_beam_grid",
            "taiga_field_eval", "taiga_field_table", "taiga_seed_beam", "taiga_trace",
-           "taiga_detector_histogram", "taiga_set_efield", "taiga_set_option", "taiga_get_stats",
+           "taiga_detector_histogram", "taiga_set_efield", "taiga_load_efield", "taiga_set_option", "taiga_get_stats",
            "taiga_measure_fp64_peak", "taiga_measure_l1_gather_peak", "taiga_measure_dmma_peak", "taiga_measure_mixed_fp64_peak",
            "taiga_loss_statistics"]
 
@@ -92,6 +92,7 @@ _lib.taiga_load_loss.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(Loss
 _lib.taiga_detector_histogram_weighted.argtypes = [C.c_void_p, C.POINTER(IonsS), C.POINTER(DetS), C.c_int,
                                                    C.c_void_p, C.c_void_p]
 _lib.taiga_set_efield.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+_lib.taiga_load_efield.argtypes = [C.c_void_p, C.POINTER(CoeffsS)]
 _lib.taiga_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_longlong]
 _lib.taiga_get_stats.argtypes = [C.c_void_p, C.POINTER(C.c_ulonglong * 8)]
 _lib.taiga_measure_fp64_peak.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
@@ -192,6 +193,23 @@ class Taiga:
         self._chk(_lib.taiga_load_field(self.h, C.byref(g), C.byref(co)))
         if on_dev:
             self._keep = keep            # device inputs are read asynchronously
+
+    def load_efield(self, comps):
+        """comps: (E_R, E_Z, E_phi) nodal arrays [nR][nZ] on the loaded grid (numpy or torch cuda), or None to remove."""
+        if comps is None:
+            self._chk(_lib.taiga_load_efield(self.h, None))
+            return
+        on_dev = isinstance(comps[0], torch.Tensor)
+        if on_dev:
+            keep = [c.contiguous() for c in comps]
+            ptrs = [c.data_ptr() for c in keep]
+        else:
+            keep = [_host(c) for c in comps]
+            ptrs = [c.ctypes.data for c in keep]
+        co = CoeffsS(0, ptrs[0], ptrs[1], ptrs[2], 1 if on_dev else 0)
+        self._chk(_lib.taiga_load_efield(self.h, C.byref(co)))
+        if on_dev:
+            self._keep_e = keep
 
     def field_eval(self, R, Z, s=None):
         R, Z = R.contiguous(), Z.contiguous()

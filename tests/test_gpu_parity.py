@@ -544,6 +544,40 @@ def test_uniform_E_field_parity(tg, solver):
     assert np.abs(g["w"][cr] - g0["w"][cr]).max() > 1e-5
 
 
+@pytest.mark.parametrize("icfg,n,solver", [(1, 1200 + 7, 0), (1, 1200 + 7, 1), (1, 1200 + 7, 2), (1, 1200 + 7, 3), (1, 1200 + 7, 4),
+                                           (4, 48, 0), (4, 48, 3), (5, 1024 + 3, 0), (5, 1024 + 3, 2), (5, 1024 + 3, 3)])
+def test_gridded_E_field_parity(tg, icfg, n, solver):
+    """Eq. 3 with E(R, Z) given on the poloidal grid like B (taiga_load_efield, reading E1), added to a uniform E, through
+    every solver and all three kinds of B (kind 2: the DMMA tracer).  Sheath-like radial field growing towards the outer
+    wall, a vertical field linear in Z and a constant toroidal component: tens of kV/m, which move the hits by far more
+    than the tolerance."""
+    from paper_2506_15812_b200 import taiga
+    cfg = wl.config(icfg, n_override=n)
+    grid, nodal = cfg.field_builder()
+    R = np.linspace(grid.Rmin, grid.Rmax, grid.nR)[:, None] * np.ones((1, grid.nZ))
+    Z = np.ones((grid.nR, 1)) * np.linspace(grid.Zmin, grid.Zmax, grid.nZ)[None, :]
+    En = (4.0e4 * np.exp((R - 0.8) / 0.05) - 1.0e4 * 0.56 / R, 6.0e4 * Z, 2.0e4 + 0.0 * R)
+    Eu = (1.0e4, 0.0, -5.0e3)
+    tg.load_field(grid, nodal)
+    tg.load_efield(En)
+    tg.set_efield(Eu)
+    ions, counts, summary = taiga.run_config(tg, cfg, field_loaded=True, rkn_variant=solver)
+    torch.cuda.synchronize()
+    fE = orc.OracleField(grid, nodal, E=Eu, E_nodal=En)
+    ref = orc.run_config(cfg, field=fE, variant=solver)
+    compare_groups(ions, ref, "%s gridded E solver %d" % (cfg.name, solver))
+    check_histogram(cfg, ions, counts, summary, ref)
+    # the gridded part is live, and removing it restores the uniform-E result
+    tg.load_efield(None)
+    ions2, _, _ = taiga.run_config(tg, cfg, field_loaded=True, rkn_variant=solver)
+    torch.cuda.synchronize()
+    ref2 = orc.run_config(cfg, field=orc.OracleField(grid, nodal, E=Eu), variant=solver)
+    compare_groups(ions2, ref2, "%s uniform E after removing the grid" % cfg.name)
+    a, b = ref["groups"][0], ref2["groups"][0]
+    cr = (a["status"] == 0) & (b["status"] == 0)
+    assert np.abs(a["w"][cr] - b["w"][cr]).max() > 1e-5
+
+
 def test_cfg5_fp32_variant(tg):
     """BASELINE config 5 'fp32 variant' (reading A19): the tricubic field evaluation and its table
     in fp32, the ion state integrated in fp64.  north_star: hit coordinates within 1e-5 m of the
@@ -770,6 +804,9 @@ def test_error_paths_of_the_widened_entry_points(tg):
     t2 = taiga.Taiga(0)
     with pytest.raises(taiga.TaigaError) as e:
         t2.load_loss(wl.nodal_psi(grid), psi0, dpsi, ne, te, wl.E12_LI)            # before load_field
+    assert e.value.code == taiga.E_STATE
+    with pytest.raises(taiga.TaigaError) as e:
+        t2.load_efield([nodal[0][0], nodal[1][0], nodal[2][0]])                    # the grid of B carries E: before load_field
     assert e.value.code == taiga.E_STATE
     t2.load_field(grid, nodal)
     for bad in (dict(dpsi=0.0), dict(E12=-1.0), dict(ne=-ne), dict(ne=ne[:1], te=te[:1])):
