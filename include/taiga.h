@@ -185,7 +185,7 @@ int taiga_set_efield(taiga_ctx* ctx, const double E_V_per_m[3]);
  * B and ADDED to the uniform field of taiga_set_efield at every stage of every solver (Boris: at r(t0), as B).  c == NULL
  * removes it.  Must follow taiga_load_field (TAIGA_E_STATE otherwise); a later taiga_load_field removes it.  The table is
  * gathered per evaluation (48 coefficients through L1, no register cache): meant for edge studies, not for the production
- * E = 0 path, whose kernels are unchanged.  Same restrictions as the uniform E (no loss model, no Bezier, fp64). */
+ * E = 0 path, whose kernels are unchanged.  fp64 only, like the uniform E. */
 int taiga_load_efield(taiga_ctx* ctx, const taiga_coeffs* c);
 
 /* ---- a5: binning + histogram (segment ID per ion; atomically summed
@@ -203,7 +203,7 @@ int taiga_detector_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga
  * [nR][nZ] on the (R,Z) grid of the field loaded before (any kind; psi is static and axisymmetric),
  * (ii) the rate profile nu_k = n_e,k sqrt(t) exp(-1/t) / (E12^1.5 (6+t)) 1e-11 [1/s], t = T_e,k/E12
  * (Eq. 2) at psi0 + k dpsi, k < n; nu(psi) is linear in between and held constant outside.
- * While a loss model is loaded and ions->weight is not null, taiga_trace (RKN solvers, E = 0)
+ * While a loss model is loaded and ions->weight is not null, taiga_trace (every solver, with or without E; fp64)
  * also writes weight = w0 exp(-integral of nu dt) (w0 = 1 when ions->w0 is null), the integral taken
  * by the trapezoidal rule over the step end points, the crossing step counted up to the plane with nu
  * interpolated linearly
@@ -254,7 +254,7 @@ int taiga_loss_statistics(const unsigned long long wsummary_host[4], double out_
  * bit-exact; taiga_trace returns TAIGA_E_ARG for other kinds / solvers), "plane_interp" (0 default:
  * linear interpolation to the detector plane; 1: quadratic Bezier through r_n, r_n+1 with the
  * control point at the mean of r_n + v_n dt/2 and r_n+1 - v_n+1 dt/2, reading Z1;
- * RKN solvers, E = 0, no loss model), "mma" (kinds 1 and 2, fp64: 1 = warp-cooperative evaluation on the FP64
+ * RKN solvers (the Boris velocities live at half steps), with or without E, no loss model), "mma" (kinds 1 and 2, fp64: 1 = warp-cooperative evaluation on the FP64
  * tensor pipe (trace_mma.cu; default for kind 2), 0 = one lane evaluates its own ion (trace.cu; default for kind 1),
  * -1 = the default of the kind), "regroup" (kinds 1 / 2: the CTA re-sorts its 128 ions over its lanes by field cell
  * every this many steps, so that the lanes of a warp / of an 8-ion group share cells; default 8; with mma = 0, 0 = off:

@@ -657,6 +657,12 @@ static const TgVariant tg_variants[] = {
     // Eq. 2 loss integral
     TG_V(0, 1, 255, 2, 0, 0, 1, 0, 0), TG_V(0, 1, 255, 0, 0, 0, 1, 0, 0), TG_V(1, 1, 255, 4, 0, 0, 1, 0, 0), TG_V(1, 0, 255, 0, 0, 0, 1, 0, 0),
     TG_V(2, 0, 255, 0, 0, 0, 1, 0, 0),
+    // the loss integral and the Bezier interpolation with an electric field; the loss integral with the other solvers
+    TG_V(0, 1, 255, 2, 0, 1, 1, 0, 0), TG_V(0, 1, 255, 0, 0, 1, 1, 0, 0), TG_V(0, 1, 255, 0, 2, 1, 1, 0, 0), TG_V(0, 1, 255, 0, 3, 1, 1, 0, 0),
+    TG_V(0, 1, 255, 2, 0, 1, 0, 1, 0), TG_V(0, 1, 255, 0, 0, 1, 0, 1, 0),
+    TG_V(1, 1, 255, 4, 0, 1, 1, 0, 0), TG_V(1, 0, 255, 0, 0, 1, 1, 0, 0), TG_V(1, 0, 255, 0, 2, 1, 1, 0, 0), TG_V(1, 0, 255, 0, 3, 1, 1, 0, 0),
+    TG_V(1, 1, 255, 4, 0, 1, 0, 1, 0), TG_V(1, 0, 255, 0, 0, 1, 0, 1, 0),
+    TG_V(2, 0, 255, 0, 0, 1, 1, 0, 0), TG_V(2, 0, 255, 0, 2, 1, 1, 0, 0), TG_V(2, 0, 255, 0, 3, 1, 1, 0, 0), TG_V(2, 0, 255, 0, 0, 1, 0, 1, 0),
     // uniform E and / or the other solvers (Eq. 4, Eq. 7-8)
     TG_V(0, 1, 255, 2, 0, 1, 0, 0, 0), TG_V(0, 1, 255, 0, 0, 1, 0, 0, 0), TG_V(0, 1, 255, 0, 2, 1, 0, 0, 0), TG_V(0, 1, 255, 0, 3, 1, 0, 0, 0),
     TG_V(1, 1, 255, 4, 0, 1, 0, 0, 0), TG_V(1, 0, 255, 0, 0, 1, 0, 0, 0), TG_V(1, 0, 255, 0, 2, 1, 0, 0, 0), TG_V(1, 0, 255, 0, 3, 1, 0, 0, 0),
@@ -678,12 +684,12 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         TG_SET_ERR(ctx, "precision=32 is offered for kind-2 (R,Z,phi) fields with the RKN solver only");
         return TAIGA_E_ARG;
     }
-    if (bez && (variant > 1 || hasE || loss || f32)) {
-        TG_SET_ERR(ctx, "plane_interp=1 (Bezier) is offered with the RKN solvers, E = 0, no loss model, fp64");
+    if (bez && (variant > 1 || loss || f32)) {
+        TG_SET_ERR(ctx, "plane_interp=1 (Bezier) is offered with the RKN solvers (Boris velocities live at half steps), no loss model, fp64");
         return TAIGA_E_ARG;
     }
-    if (loss && (variant > 1 || hasE || f32)) {
-        TG_SET_ERR(ctx, "the loss model is offered with the RKN solvers, E = 0, fp64");
+    if (loss && f32) {
+        TG_SET_ERR(ctx, "the loss model is offered in fp64");
         return TAIGA_E_ARG;
     }
     TraceParams P;

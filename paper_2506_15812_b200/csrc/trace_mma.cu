@@ -591,7 +591,7 @@ static int tg_launch_mma_t(taiga_ctx* ctx, const TraceParams& P, int per_sm, uin
     return TAIGA_OK;
 }
 
-// solver: 0 RKN (P.variant 0 / 1), 2 RK4, 3 Boris (P.variant 3 / 4).  loss / bez: with RKN and E = 0 only (as trace.cu).
+// solver: 0 RKN (P.variant 0 / 1), 2 RK4, 3 Boris (P.variant 3 / 4).  bez: RKN only; loss: any solver (as trace.cu).
 int tg_trace_mma(taiga_ctx* ctx, TraceParams& P, int solver, bool hasE, bool loss, bool bez, uint64_t n) {
     int rc = tg_build_frag(ctx);
     if (rc) return rc;
@@ -614,7 +614,11 @@ int tg_trace_mma(taiga_ctx* ctx, TraceParams& P, int solver, bool hasE, bool los
 #define TG_MMA(K, S, E, L, B, ...) rc = tg_launch_mma_t<K, S, E, L, B, ##__VA_ARGS__>(ctx, P, per_sm, n, st)
 #define TG_MMA_KIND(K)                                                        \
     do {                                                                      \
-        if (bez) TG_MMA(K, 0, false, false, true);                            \
+        if (bez && hasE) TG_MMA(K, 0, true, false, true);                     \
+        else if (bez) TG_MMA(K, 0, false, false, true);                       \
+        else if (loss && solver == 2) TG_MMA(K, 2, true, true, false);        \
+        else if (loss && solver == 3) TG_MMA(K, 3, true, true, false);        \
+        else if (loss && hasE) TG_MMA(K, 0, true, true, false);               \
         else if (loss) TG_MMA(K, 0, false, true, false);                      \
         else if (solver == 0 && hasE) TG_MMA(K, 0, true, false, false);       \
         else if (solver == 0) {                                               \

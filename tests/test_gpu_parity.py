@@ -722,6 +722,59 @@ def test_bezier_plane_interpolation_parity(tg, icfg, n):
     assert 1e-8 < d < 1e-3                    # micrometres (more at grazing incidence): the switch is live
 
 
+@pytest.mark.parametrize("icfg,n,solver,mode", [
+    (1, 1500 + 3, 0, "loss+E"), (1, 1500 + 3, 1, "loss+E"), (1, 1500 + 3, 2, "loss"), (1, 1500 + 3, 3, "loss"), (1, 1500 + 3, 4, "loss+E"),
+    (1, 1500 + 3, 0, "bezier+E"), (1, 1500 + 3, 1, "bezier+E"),
+    (4, 40, 0, "loss+E"), (4, 40, 2, "loss"), (4, 40, 0, "bezier+E"),
+    (5, 1024 + 9, 0, "loss+E"), (5, 1024 + 9, 2, "loss"), (5, 1024 + 9, 3, "loss+E"), (5, 1024 + 9, 0, "bezier+E"),
+])
+def test_loss_and_bezier_with_E_and_the_other_solvers(tg, icfg, n, solver, mode):
+    """The loss integral (Eq. 2) along trajectories of every solver, with or without an electric field, and the Bezier
+    plane interpolation (L338) with an electric field: the combinations round 1 refused."""
+    from paper_2506_15812_b200 import taiga
+    cfg = wl.config(icfg, n_override=n)
+    grid, nodal = cfg.field_builder()
+    E = (2.0e4, -1.0e4, 3.0e4) if "+E" in mode else (0.0, 0.0, 0.0)
+    tg.load_field(grid, nodal)
+    tg.set_efield(E)
+    f = orc.OracleField(grid, nodal, E=E)
+    cd, cn = wl.depth_cdf(), wl.normal_cdf()
+    if mode.startswith("bezier"):
+        tg.set_option("plane_interp", 1)
+        ions, counts, summary = taiga.run_config(tg, cfg, field_loaded=True, rkn_variant=solver)
+        torch.cuda.synchronize()
+        ref = orc.run_config(cfg, field=f, variant=solver, interp=1)
+        compare_groups(ions, ref, "%s %s solver %d" % (cfg.name, mode, solver))
+        check_histogram(cfg, ions, counts, summary, ref)
+        return
+    species_E12 = wl.E12_NA if icfg == 4 else wl.E12_LI
+    psi0, dpsi, ne, te = wl.loss_profile_inputs()
+    psi_nodal = wl.nodal_psi(grid)
+    tg.load_loss(psi_nodal, psi0, dpsi, ne, te, species_E12)
+    ions, counts, summary = taiga.run_config(tg, cfg, field_loaded=True, rkn_variant=solver)
+    torch.cuda.synchronize()
+    L = orc.OracleLoss(grid, psi_nodal, psi0, dpsi, orc.mcwhirter_rate(ne, te, species_E12))
+    off, worst, ncross = 0, 0.0, 0
+    for g in cfg.groups:
+        det = g.detector or cfg.detector
+        st = orc.seed(g.beam, cd, cn, cfg.seed, g.first_index, g.n_ions)
+        res = orc.trace_loss(f, L, g.beam.charge_C / g.beam.mass_kg, st, np.full(g.n_ions, g.t0), cfg.dt, cfg.max_steps, det, variant=solver)
+        orc.histogram(res, np.full(g.n_ions, g.group, dtype=np.uint16), det, cfg.n_hist)
+        v = ions.view(off, off + g.n_ions)
+        ok = ((_np(v.flags) | res["flags"]) == 0)
+        assert np.array_equal(_np(v.cell)[ok], res["cell"][ok]) and np.array_equal(_np(v.steps)[ok].astype(np.uint32), res["steps"][ok])
+        cr = ok & (res["status"] == 0)
+        if cr.any():
+            assert np.abs(_np(v.hit_u)[cr] - res["u"][cr]).max() < TOL_UW and np.abs(_np(v.hit_w)[cr] - res["w"][cr]).max() < TOL_UW
+        wg, wr = _np(v.weight), res["weight"]
+        assert np.all((wg > 0) & (wg <= 1.0))
+        worst = max(worst, np.abs(wg[ok] / wr[ok] - 1).max())
+        ncross += int(cr.sum())
+        off += g.n_ions
+    assert worst < 1e-12, worst
+    assert ncross > 0
+
+
 def test_deterministic_grid_seeding_parity(tg):
     """weighted-grid initialisation, bit-exact against the
     oracle (positions, velocities, weights), incl. sub-ranges (sharding) and a tilted beam frame;
@@ -822,14 +875,15 @@ def test_error_paths_of_the_widened_entry_points(tg):
     with pytest.raises(taiga.TaigaError):
         t2.set_efield((float("nan"), 0.0, 0.0))
     t2.load_loss(wl.nodal_psi(grid), psi0, dpsi, ne, te, wl.E12_LI)
-    for setup in (lambda: t2.set_option("plane_interp", 1), lambda: t2.set_efield((1e3, 0, 0))):
-        setup()
-        with pytest.raises(taiga.TaigaError) as e:
-            t2.trace(ions, qm, cfg.dt, 100, cfg.detector)                           # loss + Bezier / loss + E
-        assert e.value.code == taiga.E_ARG
-        t2.set_option("plane_interp", 0); t2.set_efield((0, 0, 0))
-    with pytest.raises(taiga.TaigaError):
-        t2.trace(ions, qm, cfg.dt, 100, cfg.detector, 3)                            # loss + Boris
+    t2.set_option("plane_interp", 1)
+    with pytest.raises(taiga.TaigaError) as e:
+        t2.trace(ions, qm, cfg.dt, 100, cfg.detector)                               # loss + Bezier: the one combination not offered
+    assert e.value.code == taiga.E_ARG
+    t2.set_option("plane_interp", 0)
+    t2.set_efield((1e3, 0, 0))
+    t2.trace(ions, qm, cfg.dt, 100, cfg.detector)                                   # loss + E and loss + Boris are (round 2)
+    t2.trace(ions, qm, cfg.dt, 100, cfg.detector, 3)
+    t2.set_efield((0, 0, 0))
     t2.load_loss(None)
     t2.set_option("plane_interp", 1)
     with pytest.raises(taiga.TaigaError):
