@@ -254,7 +254,8 @@ int taiga_loss_statistics(const unsigned long long wsummary_host[4], double out_
  * bit-exact; taiga_trace returns TAIGA_E_ARG for other kinds / solvers), "plane_interp" (0 default:
  * linear interpolation to the detector plane; 1: quadratic Bezier through r_n, r_n+1 with the
  * control point at the mean of r_n + v_n dt/2 and r_n+1 - v_n+1 dt/2, reading Z1;
- * RKN solvers (the Boris velocities live at half steps), with or without E, no loss model), "mma" (kinds 1 and 2, fp64: 1 = warp-cooperative evaluation on the FP64
+ * RKN solvers (the Boris velocities live at half steps), with or without E and the loss model (whose crossing step then
+ * counts up to the curve parameter of the hit)), "mma" (kinds 1 and 2, fp64: 1 = warp-cooperative evaluation on the FP64
  * tensor pipe (trace_mma.cu; default for kind 2), 0 = one lane evaluates its own ion (trace.cu; default for kind 1),
  * -1 = the default of the kind), "regroup" (kinds 1 / 2: the CTA re-sorts its 128 ions over its lanes by field cell
  * every this many steps, so that the lanes of a warp / of an 8-ion group share cells; default 8; with mma = 0, 0 = off:

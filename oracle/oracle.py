@@ -304,7 +304,7 @@ class OracleLoss:
         self.s = LossS(_p(self.table), len(self.rate), float(psi0), float(dpsi), _p(self.rate))
 
 
-def trace_loss(field: OracleField, loss: OracleLoss, qm, state, t0, dt, max_steps, det, variant=0, nthreads=0, w0=None):
+def trace_loss(field: OracleField, loss: OracleLoss, qm, state, t0, dt, max_steps, det, variant=0, nthreads=0, w0=None, interp=0):
     x, y, z, vx, vy, vz = [np.ascontiguousarray(a, dtype=np.float64) for a in state]
     n = len(x)
     d, keep = _det_struct(det)
@@ -313,7 +313,7 @@ def trace_loss(field: OracleField, loss: OracleLoss, qm, state, t0, dt, max_step
     steps = np.empty(n, dtype=np.uint32)
     flags = np.empty(n, dtype=np.uint8)
     t0a = None if t0 is None else np.ascontiguousarray(t0, dtype=np.float64)
-    _lib.orc_trace_loss(C.byref(field.s), C.byref(loss.s), C.c_double(qm), C.c_int(variant), C.c_uint64(n),
+    _lib.orc_trace_loss_interp(C.byref(field.s), C.byref(loss.s), C.c_double(qm), C.c_int(variant), C.c_int(interp), C.c_uint64(n),
                         _p(x), _p(y), _p(z), _p(vx), _p(vy), _p(vz),
                         _p(t0a) if t0a is not None else None,
                         C.c_double(dt), C.c_uint32(max_steps), C.byref(d),

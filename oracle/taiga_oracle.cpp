@@ -495,8 +495,8 @@ static inline bool in_grid(const orc_field* f, const double r[3], bool* graze) {
  * plane distance s(tau) = (1-tau)^2 s0 + 2 (1-tau) tau sc + tau^2 s1 vanishes in [0,1]
  * (sc = n.(P1 - r_D)); tau* = 2 s0 / (2 s0 - 2 sc - sqrt(4 sc^2 - 4 s0 s1))... written below in
  * the cancellation-free form.  Exact for uniformly accelerated motion.                       */
-static inline void bezier_hit(const double r[3], const double v[3], const double rn[3], const double vn[3],
-                              double dt, double s0, double s1, const orc_detector* det, double p[3]) {
+static inline double bezier_hit(const double r[3], const double v[3], const double rn[3], const double vn[3],
+                                double dt, double s0, double s1, const orc_detector* det, double p[3]) {
     double P1[3], sc = 0.0;
     for (int c = 0; c < 3; ++c) {
         P1[c] = 0.5 * ((r[c] + v[c] * (dt / 2.0)) + (rn[c] - vn[c] * (dt / 2.0)));
@@ -515,6 +515,7 @@ static inline void bezier_hit(const double r[3], const double v[3], const double
     if (tau > 1.0) tau = 1.0;
     double w0 = (1.0 - tau) * (1.0 - tau), w1 = 2.0 * (1.0 - tau) * tau, w2 = tau * tau;
     for (int k = 0; k < 3; ++k) p[k] = w0 * r[k] + w1 * P1[k] + w2 * rn[k];
+    return tau;                                             /* the curve parameter of the hit (reading L2': loss integral) */
 }
 
 extern "C" void orc_trace(const orc_field* f, double qm, int variant, uint64_t n,
@@ -628,8 +629,20 @@ extern "C" void orc_trace_loss(const orc_field* f, const orc_loss* L, double qm,
                                double dt, uint32_t max_steps, const orc_detector* det,
                                int32_t* status, double* hit_u, double* hit_w,
                                uint32_t* steps, uint8_t* flags, const double* w0, double* weight, int nthreads) {
-    orc_trace(f, qm, variant, n, x, y, z, vx, vy, vz, t0, dt, max_steps, det, status, hit_u, hit_w, nullptr,
-              steps, flags, nthreads);
+    orc_trace_loss_interp(f, L, qm, variant, 0, n, x, y, z, vx, vy, vz, t0, dt, max_steps, det, status, hit_u, hit_w, steps,
+                          flags, w0, weight, nthreads);
+}
+
+/* The same with the plane interpolation of orc_trace_interp.  interp = 1 (Bezier, reading Z1): the fraction of the crossing
+ * step that counts is the curve parameter tau of the hit instead of lam, nu interpolated linearly in tau (reading L2'). */
+extern "C" void orc_trace_loss_interp(const orc_field* f, const orc_loss* L, double qm, int variant, int interp, uint64_t n,
+                                      const double* x, const double* y, const double* z,
+                                      const double* vx, const double* vy, const double* vz, const double* t0,
+                                      double dt, uint32_t max_steps, const orc_detector* det,
+                                      int32_t* status, double* hit_u, double* hit_w,
+                                      uint32_t* steps, uint8_t* flags, const double* w0, double* weight, int nthreads) {
+    orc_trace_interp(f, qm, variant, interp, n, x, y, z, vx, vy, vz, t0, dt, max_steps, det, status, hit_u, hit_w, nullptr,
+                     steps, flags, nthreads);
 #ifdef _OPENMP
     if (nthreads <= 0) nthreads = omp_get_max_threads();
 #pragma omp parallel for schedule(dynamic, 16) num_threads(nthreads)
@@ -652,6 +665,7 @@ extern "C" void orc_trace_loss(const orc_field* f, const orc_loss* L, double qm,
                 double s1 = det->normal[0] * (rn[0] - det->origin[0]) + det->normal[1] * (rn[1] - det->origin[1]) +
                             det->normal[2] * (rn[2] - det->origin[2]);
                 double lam = s0 / (s0 - s1);
+                if (interp == 1) { double p[3]; lam = bezier_hit(r, v, rn, vn, dt, s0, s1, det, p); }
                 double nuh = nu0 + lam * (nu1 - nu0);
                 Lam += lam * dt * (nu0 + nuh) / 2.0;
                 break;

@@ -147,6 +147,14 @@ void orc_trace_loss(const orc_field* f, const orc_loss* L, double qm, int varian
                     double dt, uint32_t max_steps, const orc_detector* det,
                     int32_t* status, double* hit_u, double* hit_w,
                     uint32_t* steps, uint8_t* flags, const double* w0 /* or 0 */, double* weight, int nthreads);
+/* the same with the plane interpolation of orc_trace_interp (interp = 1: Bezier; the crossing step counts up to the curve
+ * parameter of the hit, reading L2') */
+void orc_trace_loss_interp(const orc_field* f, const orc_loss* L, double qm, int variant, int interp, uint64_t n,
+                    const double* x, const double* y, const double* z,
+                    const double* vx, const double* vy, const double* vz, const double* t0,
+                    double dt, uint32_t max_steps, const orc_detector* det,
+                    int32_t* status, double* hit_u, double* hit_w,
+                    uint32_t* steps, uint8_t* flags, const double* w0 /* or 0 */, double* weight, int nthreads);
 void orc_histogram_weighted(uint64_t n, const int32_t* cell, const double* weight, const uint16_t* group,
                             const orc_detector* det, int n_hist, uint64_t* wcounts, uint64_t* wsummary);
 

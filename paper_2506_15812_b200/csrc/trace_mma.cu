@@ -458,6 +458,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
         }
         if (crossed) {                         // O4: s0 < 0 <= s1
             lam = s0 / (s0 - s1);
+            [[maybe_unused]] double frac = lam;     // fraction of the crossing step up to the plane (Bezier: its tau)
             double px = fma(lam, Xn - X, X) - P.det.origin[0], py = fma(lam, Yn - Y, Y) - P.det.origin[1],
                    pz = fma(lam, Zn - Z, Z) - P.det.origin[2];
             if constexpr (BEZ) {
@@ -469,6 +470,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
                     tau = (qb >= 0.0) ? (-2.0 * s0) / (qb + sq) : (sq - qb) / (2.0 * qa);
                 }
                 tau = fmin(fmax(tau, 0.0), 1.0);
+                frac = tau;
                 double w0 = (1.0 - tau) * (1.0 - tau), w1 = 2.0 * (1.0 - tau) * tau, w2 = tau * tau;
                 px = fma(w0, X, fma(w1, qx, w2 * Xn)) - P.det.origin[0];
                 py = fma(w0, Y, fma(w1, qy, w2 * Yn)) - P.det.origin[1];
@@ -479,8 +481,8 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace_mma(const
             P.cell[idx] = TAIGA_CELL_MISS;      // segment assigned by the histogram kernel (a5)
             if constexpr (LOSS) {               // crossing step: up to the plane, nu interpolated linearly (reading L2)
                 double nun = tg_loss_rate(P, sqrt(fma(Xn, Xn, Yn * Yn)), Zn);
-                double nuh = fma(lam, nun - nu1, nu1);
-                P.weight[idx] = (P.w0 ? P.w0[idx] : 1.0) * exp(-fma(lam * P.hdt, nu1 + nuh, Lam));
+                double nuh = fma(frac, nun - nu1, nu1);
+                P.weight[idx] = (P.w0 ? P.w0[idx] : 1.0) * exp(-fma(frac * P.hdt, nu1 + nuh, Lam));
             }
             P.steps[idx] = nst;
             P.flags[idx] = (fabs(s0) < TG_GRAZE || fabs(s1) < TG_GRAZE) ? TAIGA_FLAG_PLANE : 0;
@@ -614,7 +616,9 @@ int tg_trace_mma(taiga_ctx* ctx, TraceParams& P, int solver, bool hasE, bool los
 #define TG_MMA(K, S, E, L, B, ...) rc = tg_launch_mma_t<K, S, E, L, B, ##__VA_ARGS__>(ctx, P, per_sm, n, st)
 #define TG_MMA_KIND(K)                                                        \
     do {                                                                      \
-        if (bez && hasE) TG_MMA(K, 0, true, false, true);                     \
+        if (bez && loss && hasE) TG_MMA(K, 0, true, true, true);              \
+        else if (bez && loss) TG_MMA(K, 0, false, true, true);                \
+        else if (bez && hasE) TG_MMA(K, 0, true, false, true);                \
         else if (bez) TG_MMA(K, 0, false, false, true);                       \
         else if (loss && solver == 2) TG_MMA(K, 2, true, true, false);        \
         else if (loss && solver == 3) TG_MMA(K, 3, true, true, false);        \

@@ -727,10 +727,13 @@ def test_bezier_plane_interpolation_parity(tg, icfg, n):
     (1, 1500 + 3, 0, "bezier+E"), (1, 1500 + 3, 1, "bezier+E"),
     (4, 40, 0, "loss+E"), (4, 40, 2, "loss"), (4, 40, 0, "bezier+E"),
     (5, 1024 + 9, 0, "loss+E"), (5, 1024 + 9, 2, "loss"), (5, 1024 + 9, 3, "loss+E"), (5, 1024 + 9, 0, "bezier+E"),
+    (1, 1500 + 3, 0, "loss+bezier"), (1, 1500 + 3, 1, "loss+bezier+E"), (4, 40, 0, "loss+bezier+E"), (5, 1024 + 9, 0, "loss+bezier"),
+    (5, 1024 + 9, 0, "loss+bezier+E"),
 ])
 def test_loss_and_bezier_with_E_and_the_other_solvers(tg, icfg, n, solver, mode):
     """The loss integral (Eq. 2) along trajectories of every solver, with or without an electric field, and the Bezier
-    plane interpolation (L338) with an electric field: the combinations round 1 refused."""
+    plane interpolation (L338) with an electric field and with the loss integral (the crossing step counts up to the curve
+    parameter of the hit, reading L2'): the combinations round 1 refused."""
     from paper_2506_15812_b200 import taiga
     cfg = wl.config(icfg, n_override=n)
     grid, nodal = cfg.field_builder()
@@ -739,8 +742,9 @@ def test_loss_and_bezier_with_E_and_the_other_solvers(tg, icfg, n, solver, mode)
     tg.set_efield(E)
     f = orc.OracleField(grid, nodal, E=E)
     cd, cn = wl.depth_cdf(), wl.normal_cdf()
+    interp = 1 if "bezier" in mode else 0
+    tg.set_option("plane_interp", interp)
     if mode.startswith("bezier"):
-        tg.set_option("plane_interp", 1)
         ions, counts, summary = taiga.run_config(tg, cfg, field_loaded=True, rkn_variant=solver)
         torch.cuda.synchronize()
         ref = orc.run_config(cfg, field=f, variant=solver, interp=1)
@@ -758,7 +762,8 @@ def test_loss_and_bezier_with_E_and_the_other_solvers(tg, icfg, n, solver, mode)
     for g in cfg.groups:
         det = g.detector or cfg.detector
         st = orc.seed(g.beam, cd, cn, cfg.seed, g.first_index, g.n_ions)
-        res = orc.trace_loss(f, L, g.beam.charge_C / g.beam.mass_kg, st, np.full(g.n_ions, g.t0), cfg.dt, cfg.max_steps, det, variant=solver)
+        res = orc.trace_loss(f, L, g.beam.charge_C / g.beam.mass_kg, st, np.full(g.n_ions, g.t0), cfg.dt, cfg.max_steps, det, variant=solver,
+                             interp=interp)
         orc.histogram(res, np.full(g.n_ions, g.group, dtype=np.uint16), det, cfg.n_hist)
         v = ions.view(off, off + g.n_ions)
         ok = ((_np(v.flags) | res["flags"]) == 0)
@@ -876,14 +881,17 @@ def test_error_paths_of_the_widened_entry_points(tg):
         t2.set_efield((float("nan"), 0.0, 0.0))
     t2.load_loss(wl.nodal_psi(grid), psi0, dpsi, ne, te, wl.E12_LI)
     t2.set_option("plane_interp", 1)
-    with pytest.raises(taiga.TaigaError) as e:
-        t2.trace(ions, qm, cfg.dt, 100, cfg.detector)                               # loss + Bezier: the one combination not offered
-    assert e.value.code == taiga.E_ARG
+    t2.trace(ions, qm, cfg.dt, 100, cfg.detector)                                   # loss + Bezier, loss + E, loss + Boris: offered since round 2
     t2.set_option("plane_interp", 0)
     t2.set_efield((1e3, 0, 0))
-    t2.trace(ions, qm, cfg.dt, 100, cfg.detector)                                   # loss + E and loss + Boris are (round 2)
+    t2.trace(ions, qm, cfg.dt, 100, cfg.detector)
     t2.trace(ions, qm, cfg.dt, 100, cfg.detector, 3)
     t2.set_efield((0, 0, 0))
+    t2.set_option("precision", 32)
+    with pytest.raises(taiga.TaigaError) as e:
+        t2.trace(ions, qm, cfg.dt, 100, cfg.detector)                               # fp32 is kind 2 + RKN, no loss model
+    assert e.value.code == taiga.E_ARG
+    t2.set_option("precision", 64)
     t2.load_loss(None)
     t2.set_option("plane_interp", 1)
     with pytest.raises(taiga.TaigaError):

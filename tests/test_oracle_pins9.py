@@ -98,3 +98,31 @@ def test_p23_central_force_conserves_angular_momentum_and_energy():
         assert 0.3 < math.hypot(r[0], r[1]) < 0.85 and np.abs(r - r0).max() > 0.1    # it moved, inside the grid
     assert dW[0] < 5e-6 and dW[2] < 3e-8, dW
     assert dW[0] / dW[1] > 8 and dW[1] / dW[2] > 8, dW
+
+
+# ---- P24: loss integral with the Bezier plane interpolation (reading L2') -----------------------------------
+def test_p24_bezier_fraction_of_the_crossing_step_is_the_exact_time_fraction_on_a_parabola():
+    """Uniform E, B = 0: the trajectory is a parabola, which the quadratic Bezier curve through (r_n, v_n), (r_n+1, v_n+1)
+    reproduces with tau = (t - t_n)/dt exactly.  With a constant rate every trapezoid is exact, so with the Bezier
+    interpolation weight = exp(-nu t_hit) for the EXACT crossing time at any dt, while the linear interpolation's fraction
+    lam is off by O(dt^2 a / v) and shows it."""
+    grid, nodal = wl.nodal_field_2d(33, 65)
+    Ex = 4.0e6                                                   # strong enough to bend the parabola within a step
+    f = orc.OracleField(grid, [0.0 * c for c in nodal], E=(Ex, 0.0, 0.0))
+    nu0 = 2.5e6
+    L = orc.OracleLoss(grid, wl.nodal_psi(grid), 0.0, 1e-3, np.full(5, nu0))
+    V0 = math.sqrt(2 * 60e3 * wl.E_CHARGE / wl.MASS_LI7)
+    x0 = np.array([0.70, 0.61, 0.8123])
+    state = [x0, np.zeros(3), np.array([0.0, 0.01, -0.02]), np.full(3, 0.2 * V0), np.zeros(3), np.zeros(3)]
+    det = wl.uniform_detector(0.0, 0.0, 8, 2.5e-3, x_plane=0.82)
+    a = QM * Ex
+    v0 = 0.2 * V0
+    t_hit = (-v0 + np.sqrt(v0 * v0 + 2.0 * a * (0.82 - x0))) / a          # x0 + v0 t + a t^2 / 2 = 0.82
+    dev_lin = []
+    for dt in (4e-9, 1.3e-9):
+        rb = orc.trace_loss(f, L, QM, state, None, dt, 100000, det, interp=1)
+        rl = orc.trace_loss(f, L, QM, state, None, dt, 100000, det, interp=0)
+        assert np.all(rb["status"] == 0) and np.array_equal(rb["steps"], rl["steps"])
+        assert np.abs(rb["weight"] / np.exp(-nu0 * t_hit) - 1).max() < 2e-13
+        dev_lin.append(np.abs(rl["weight"] / np.exp(-nu0 * t_hit) - 1).max())
+    assert dev_lin[0] > 1e-7 and dev_lin[0] > 4 * dev_lin[1] > 0, dev_lin
