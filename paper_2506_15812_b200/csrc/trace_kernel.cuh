@@ -29,6 +29,7 @@ template <>
 struct CellCache<0> {
     double c[48];
     double oR, oZ;                             // offR + i, offZ + j of the cached cell
+    int i, j;                                  // its indices
 };
 template <>
 struct CellCache<1> {                          // slice k of the current cell (PRED 2: the slice difference is gathered per
@@ -52,7 +53,7 @@ __device__ __forceinline__ double tg_horner16(const double* c, double p, double 
 // (clamped to the grid: outside it the boundary cell extrapolates, reading A12).
 __device__ __forceinline__ void tg_refill(const TraceParams& P, CellCache<0>& cc, unsigned& reloads, double pR, double pZ) {
     int i = tg_clampi(__double2int_rd(pR), 0, P.f.cR - 1), j = tg_clampi(__double2int_rd(pZ), 0, P.f.cZ - 1);
-    cc.oR = P.f.offR + (double)i; cc.oZ = P.f.offZ + (double)j;
+    cc.oR = P.f.offR + (double)i; cc.oZ = P.f.offZ + (double)j; cc.i = i; cc.j = j;
     const double* src = P.f.table + ((size_t)i * P.f.cZ + j) * 48;      // 384-B aligned
 #pragma unroll
     for (int k = 0; k < 12; ++k)       // 12 x LDG.E.256 (sm_100: 256-bit global loads)
@@ -106,15 +107,17 @@ __device__ __forceinline__ void tg_fieldCyl(const TraceParams& P, CellCache<KIND
             tR = fma(R, P.f.inv_hR, -cc.oR); tZ = fma(Z, P.f.inv_hZ, -cc.oZ);
         }
         double tRp = tR + dR, tZp = tZ + dZ;
-        int need = !(tg_in01(tRp) && tg_in01(tZp));
-        const double* src = P.f.table;
-        if (need) {
-            int i = tg_clampi(__double2int_rd(tRp + (cc.oR - P.f.offR)), 0, P.f.cR - 1);
-            int j = tg_clampi(__double2int_rd(tZp + (cc.oZ - P.f.offZ)), 0, P.f.cZ - 1);
-            cc.oR = P.f.offR + (double)i; cc.oZ = P.f.offZ + (double)j;
-            src += ((size_t)i * P.f.cZ + j) * 48;
-            ++reloads;
-        }
+        // Branch-free (30.6 against 31.5 ms with a divergent block, profiles/r2_experiments.md): the predicted point is at most
+        // one cell away in each direction, so the successor's indices are the cached ones -1 / 0 / +1 from the sign and the
+        // exponent of the predicted coordinates; a wrong guess is corrected by the next stage's verify.
+        const unsigned hR = (unsigned)__double2hiint(tRp), hZ = (unsigned)__double2hiint(tZp);
+        const int i2 = tg_clampi(cc.i + (int)(hR >= 0x3FF00000u) - 2 * (int)(hR >> 31), 0, P.f.cR - 1);
+        const int j2 = tg_clampi(cc.j + (int)(hZ >= 0x3FF00000u) - 2 * (int)(hZ >> 31), 0, P.f.cZ - 1);
+        const int need = (i2 != cc.i) | (j2 != cc.j);
+        cc.i = i2; cc.j = j2;
+        cc.oR = P.f.offR + (double)i2; cc.oZ = P.f.offZ + (double)j2;
+        const double* src = P.f.table + ((size_t)i2 * P.f.cZ + j2) * 48;
+        reloads += need;
         BR = tg_horner16(cc.c, tR, tZ);      tg_ldpred16(src, need, cc.c);
         BZ = tg_horner16(cc.c + 16, tR, tZ); tg_ldpred16(src + 16, need, cc.c + 16);
         Bp = tg_horner16(cc.c + 32, tR, tZ); tg_ldpred16(src + 32, need, cc.c + 32);
@@ -341,6 +344,7 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
     const int lane = threadIdx.x & 31;
     CellCache<KIND> cc;
     if constexpr (KIND == 1 && CACHED) { cc.k = -1; cc.cell = 0; cc.tau = -1.0; }
+    if constexpr (KIND == 0 && CACHED) { cc.i = 0; cc.j = 0; }
     if constexpr (KIND <= 1 && CACHED) { cc.oR = 1e300; cc.oZ = 1e300;
 #pragma unroll
         for (int k = 0; k < 48; ++k) cc.c[k] = 0.0; }
