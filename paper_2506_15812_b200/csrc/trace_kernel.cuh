@@ -450,6 +450,11 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
         }
         if (am == 0) { if (exhausted) break; else continue; }
       }
+      // Steps repeat here until a lane of the warp finishes: the loop head above (vote, queue refill, exit test) has nothing
+      // to decide before that and costs 13 control instructions per step (profiles/r2_experiments.md)
+      bool again;
+      do {
+        const bool was_alive = alive;
         ++warp_steps;
         if (alive) {
             // ---- stage 1 at (r, u); its grid test is the out-of-grid test of the previous step (O4)
@@ -620,6 +625,8 @@ __global__ void __launch_bounds__(THREADS) __maxnreg__(MAXREG) k_trace(const Tra
                 if constexpr (LOSS) nu0 = nu1;
             }
         }
+        again = !REGROUP && __all_sync(FULL, was_alive == alive);
+      } while (again);
     }
     // per-warp statistics
     unsigned long long rl = reloads, is = ion_steps;
