@@ -29,7 +29,7 @@ sys.path.insert(0, ROOT)
 ALG_FP64_INSTR_PER_ION_STEP = {0: 252.0, 1: 402.0, 2: 840.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel at the FULL size of the config, from
 # the latest `ncu --set full` capture of that kernel (not measured by this run): {config: (bytes, capture)}
-NCU_DRAM_BYTES_PER_LAUNCH = {2: (176.4e6, "profiles/r2_trace_ncu.md"), 4: (1686e6, "profiles/r2_trace_ncu.md")}
+NCU_DRAM_BYTES_PER_LAUNCH = {2: (175.2e6, "profiles/r2_trace_ncu.md"), 4: (1686e6, "profiles/r2_trace_ncu.md")}
 NOMINAL_FP64_INSTR_PER_S = 148 * 64 * 1.965e9      # B200: 148 SMs x 64 FP64 lanes x 1965 MHz
 # kinds 1 and 2 are bound by the L1 -> register delivery of the gathered coefficients:
 # bytes per ion-step = 3 evaluations x (384: slice difference, kind 1 | 1536: tricubic cell, kind 2; fp32 halves it)
