@@ -9,10 +9,11 @@
  *    "host" pointers are ordinary host memory, read during the call only.  The ctx owns only
  *    its internal tables / scratch and frees them in taiga_destroy.
  *  - All kernels are enqueued on the ctx's stream and the caller synchronises.  Exceptions:
- *    taiga_load_field synchronises once the first time it sees a new grid line length (it
- *    uploads a host-built band operator); taiga_trace synchronises at its end only while the
- *    "stats" option is on (default; it reads the counters back), taiga_field_table and
- *    taiga_measure_fp64_peak / taiga_measure_dmma_peak / taiga_measure_l1_gather_peak always do.
+ *    taiga_load_field / taiga_load_efield / taiga_load_loss wait for the upload of HOST input arrays (so that the
+ *    caller may reuse them on return; device inputs are not synchronised, and every table is built on the device);
+ *    taiga_trace synchronises at its end only while the "stats" option is on (default; it reads the counters back);
+ *    taiga_field_table and the taiga_measure_* calls always do.  Small host tables (CDFs, detector edges) are staged
+ *    through a pinned buffer of the ctx and never synchronise.
  *  - Coordinates: right-handed Cartesian (X,Y,Z), Z vertical, torus axis = Z,
  *    R = sqrt(X^2+Y^2); (R,phi,Z) right-handed; SI units.
  *  - There is no CPU fallback: every entry point needs an sm_100 device.

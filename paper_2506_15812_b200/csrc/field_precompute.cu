@@ -230,6 +230,7 @@ int tg_precompute(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c) {
             if (!c->on_device) { TG_CUDA(ctx, cudaMemcpyAsync(ctx->scratch, src[m], need * sizeof(double), cudaMemcpyHostToDevice, st)); s = ctx->scratch; }
             k_relayout<<<(unsigned)((need + TPB - 1) / TPB), TPB, 0, st>>>(s, ctx->table, g->kind, nS, ncell, m, 1);
         }
+        if (!c->on_device) TG_CUDA(ctx, cudaStreamSynchronize(st));      // host arrays: read during the call only
     } else {
         // scratch: y[3] | Mz[3] | Myr[3] | Mzr[3] (3 components) | temp bicubic (kind 2) | G
         size_t n_tmp = (g->kind == 2) ? (size_t)ncell * nS * 48 : 0;
@@ -245,6 +246,9 @@ int tg_precompute(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c) {
         for (int m = 0; m < 3; ++m)
             TG_CUDA(ctx, cudaMemcpyAsync(y + (size_t)m * nnode, src[m], nnode * sizeof(double),
                                          c->on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+        // host arrays are "read during the call only" (taiga.h): a copy from pinned or registered host memory is truly
+        // asynchronous, so wait for it here; device inputs (the timed paths) are not synchronised
+        if (!c->on_device) TG_CUDA(ctx, cudaStreamSynchronize(st));
         long long tot = 3 * nnode;
         unsigned gb = (unsigned)((tot + TPB - 1) / TPB);
         k_second_deriv<<<gb, TPB, 0, st>>>(y, Mz, ctx->band[0], nZ, 1, tot);          // y_zz
