@@ -55,7 +55,7 @@ struct TgLane {
 __device__ __forceinline__ double tg_lds(unsigned a) { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a)); return v; }
 __device__ __forceinline__ void tg_sts(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
 __device__ __forceinline__ void tg_lds4(unsigned a, int& x, unsigned& y, unsigned& z) {
-    int w;
+    [[maybe_unused]] int w;                   // fourth word of the descriptor: padding
     asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(x), "=r"(y), "=r"(z), "=r"(w) : "r"(a));
 }
 __device__ __forceinline__ void tg_sts4(unsigned a, int x, unsigned y, unsigned z) {
