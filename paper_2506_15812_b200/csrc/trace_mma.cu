@@ -88,7 +88,7 @@ __device__ __forceinline__ int tg_locate_cell(const FieldDev& f, double X, doubl
 }
 
 // Kind 2 without atan2.  The ion carries K, the global index of the toroidal cell it is in (K ds <= phi - s0 < (K+1) ds,
-// NK = 2 pi / ds cells around the torus), and (c0, s0) = (cos, sin) of that cell's lower plane from a host-built table.
+// NK = 2 pi / ds cells around the torus), and (c0, s0) = (cos, sin) of that cell's lower plane from a table (k_phi_tab).
 // For a point (X, Y) the angle past the plane is small, delta = asin((Y c0 - X s0) / R) with |delta| <~ ds, so
 // q = delta / ds is a 4-term series in s = (Y c0 - X s0) / R (1/R is needed anyway): 10 FP64 instructions instead of the
 // ~65 of atan2 + modulo.  A point beyond the cell moves K (and the frame) by floor(q) and is evaluated again.
@@ -559,18 +559,21 @@ bool tg_mma_supported(const taiga_ctx* ctx) {
     return ncell < (1ll << 31) && f.nS >= 2;
 }
 
-// (cos, sin) of the lower plane of every toroidal cell, host libm, staged like the other small tables
+// (cos, sin) of the lower plane of every toroidal cell, built on the device
+__global__ void k_phi_tab(double* __restrict__ tab, int nk, double s0, double ds) {
+    const int K = blockIdx.x * blockDim.x + threadIdx.x;
+    if (K >= nk) return;
+    double sn, cs;
+    sincos(s0 + (double)K * ds, &sn, &cs);
+    tab[2 * K] = cs; tab[2 * K + 1] = sn;
+}
+
 static int tg_build_phi_tab(taiga_ctx* ctx, int nk) {
     if (ctx->phi_tab_n == nk && ctx->phi_tab_s0 == ctx->field.s0 && ctx->phi_tab) return TAIGA_OK;
     int rc = tg_reserve(ctx, &ctx->phi_tab, &ctx->cap_phi_tab, (size_t)2 * nk);
     if (rc) return rc;
-    rc = tg_stage(ctx, (size_t)2 * nk * sizeof(double));
-    if (rc) return rc;
-    double* h = (double*)ctx->stage;
-    const double ds = 1.0 / ctx->field.inv_ds;
-    for (int K = 0; K < nk; ++K) { const double a = ctx->field.s0 + (double)K * ds; h[2 * K] = cos(a); h[2 * K + 1] = sin(a); }
-    TG_CUDA(ctx, cudaMemcpyAsync(ctx->phi_tab, h, (size_t)2 * nk * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
-    TG_CUDA(ctx, cudaEventRecord(ctx->stage_done, ctx->stream));
+    k_phi_tab<<<(nk + 127) / 128, 128, 0, ctx->stream>>>(ctx->phi_tab, nk, ctx->field.s0, 1.0 / ctx->field.inv_ds);
+    TG_CUDA(ctx, cudaGetLastError());
     ctx->phi_tab_n = nk; ctx->phi_tab_s0 = ctx->field.s0;
     return TAIGA_OK;
 }
