@@ -198,6 +198,31 @@ int taiga_detector_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga
                              int n_hist, unsigned long long* counts_dev,
                              unsigned long long* summary_dev);
 
+/* The same binning for callers that are not allowed to allocate GPU or pinned memory.  taiga_detector_histogram keeps a
+ * device copy of the segment edges in a buffer of the context that it creates on first use and replaces when a larger
+ * detector arrives (cudaMalloc / cudaFree), and stages the edges through a pinned buffer (cudaMallocHost).  That rules it
+ * out in two places this library is meant for: a between-shot or in-shot evaluation loop that shares the GPU with other
+ * streams and must never stall them (cudaMalloc and cudaFree make the whole device wait), and a process whose memory pool
+ * -- torch's caching allocator, a control system's fixed partition -- already owns the device's memory, where a late
+ * cudaMalloc just fails.  This entry point calls no cudaMalloc, cudaMallocHost, cudaFree or any other allocating routine:
+ * its edge table is a fixed array inside the library image, TAIGA_STATIC_MAX_SEGMENTS * 2 doubles = 32 KB, which every GPU
+ * that loads libtaiga.so holds until the process exits.  Arguments, outputs, accumulation and results are exactly those of
+ * taiga_detector_histogram (same kernel); ions, counts_dev and summary_dev remain the caller's.
+ *  - Limit: det->nu + det->nw <= TAIGA_STATIC_MAX_SEGMENTS, else TAIGA_E_ARG with a message naming the limit (nothing
+ *    is enqueued).
+ *  - First call on a device: looks up the device address of the array (cudaGetSymbolAddress, no allocation).  Make that
+ *    first call during set-up, before any stream capture is begun.
+ *  - The edge arrays are copied from the caller's host memory by four cudaMemcpyAsync on the ctx's stream; ordinary
+ *    (pageable) arrays have been read when the call returns, pinned ones must stay valid until the stream reaches the copy.
+ *  - The array is shared by every context and every call on that GPU and keeps what the last call wrote.  Nothing in
+ *    it has to start at zero -- each call rewrites every entry its kernel reads -- but two calls that overlap on the GPU
+ *    (different streams, or host threads with different contexts on one device) race on it: keep all calls on one
+ *    device in one stream, or order them with events. */
+#define TAIGA_STATIC_MAX_SEGMENTS 2048
+int taiga_detector_histogram_static(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det,
+                                    int n_hist, unsigned long long* counts_dev,
+                                    unsigned long long* summary_dev);
+
 /* ---- secondary-ionisation loss (PAPER.md III.C, Eq. 2; L177: "numerically integrated with
  * every step using the one-dimensional secondary ionization profile"; L350 weighting).
  * taiga_load_loss builds (i) the bicubic spline table of the poloidal flux psi(R,Z) from nodal values

@@ -164,3 +164,60 @@ int tg_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, const taiga_de
     TG_CUDA(ctx, cudaGetLastError());
     return TAIGA_OK;
 }
+
+// ------------------------------------------------------------------------------------------
+// taiga_detector_histogram_static (include/taiga.h): k_histogram again, for callers that must not allocate.
+//
+// tg_histogram above keeps its device copy of the segment edges in ctx->edges (cudaMalloc on the first call and
+// whenever a larger detector comes along) and stages the host arrays through ctx->stage (cudaMallocHost).  A caller
+// that runs the binning inside a loop it has promised to keep free of allocations -- a between-shot evaluation that
+// shares the GPU with other streams (cudaMalloc / cudaFree stall every stream of the device), or a process whose
+// memory pool has already taken the device's memory, where a late cudaMalloc simply fails -- cannot use that.
+// Here the edge copy lives in the fixed array below, part of the library image: every GPU that loads libtaiga.so
+// holds these 32 KB until the process exits, whether or not this entry point is ever called.
+#define TG_STATIC_EDGE_DOUBLES 4096                       // 2 (nu + nw) doubles: nu + nw <= TAIGA_STATIC_MAX_SEGMENTS = 2048
+#define TG_STATIC_MAX_DEVICES 64
+static __device__ __align__(256) double g_static_edges[TG_STATIC_EDGE_DOUBLES];
+// Device address of g_static_edges per CUDA ordinal.  In host code `g_static_edges` is only a handle for the symbol
+// API, not an address a kernel may be given; the address is asked for once per device, with that device current.
+static double* g_static_edges_dev[TG_STATIC_MAX_DEVICES];
+
+int tg_histogram_static(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
+                        unsigned long long* counts, unsigned long long* summary) {
+    const size_t nu = (size_t)det->nu, nw = (size_t)det->nw, ne = 2 * (nu + nw);
+    if (ne > TG_STATIC_EDGE_DOUBLES) {
+        TG_SET_ERR(ctx, "histogram_static: nu + nw = %zu segments exceed the fixed edge table (TAIGA_STATIC_MAX_SEGMENTS = %d); "
+                        "use taiga_detector_histogram, which allocates", nu + nw, TG_STATIC_EDGE_DOUBLES / 2);
+        return TAIGA_E_ARG;
+    }
+    if (ctx->device < 0 || ctx->device >= TG_STATIC_MAX_DEVICES) {
+        TG_SET_ERR(ctx, "histogram_static: device ordinal %d outside [0, %d)", ctx->device, TG_STATIC_MAX_DEVICES);
+        return TAIGA_E_ARG;
+    }
+    double* e = g_static_edges_dev[ctx->device];
+    if (!e) {          // first call on this device (the caller has made ctx->device current): resolve the symbol
+        TG_CUDA(ctx, cudaGetSymbolAddress((void**)&e, g_static_edges));
+        g_static_edges_dev[ctx->device] = e;           // every thread that gets here stores the same value
+    }
+    cudaStream_t st = ctx->stream;
+    // Straight from the caller's arrays, in stream order behind earlier users of the table on this stream; the runtime
+    // has read a pageable source by the time each call returns.  Every entry the kernel reads is rewritten here, so
+    // nothing in the array has to start at zero and the previous call's contents do not matter.
+    TG_CUDA(ctx, cudaMemcpyAsync(e, det->u_lo, nu * sizeof(double), cudaMemcpyHostToDevice, st));
+    TG_CUDA(ctx, cudaMemcpyAsync(e + nu, det->u_hi, nu * sizeof(double), cudaMemcpyHostToDevice, st));
+    TG_CUDA(ctx, cudaMemcpyAsync(e + 2 * nu, det->w_lo, nw * sizeof(double), cudaMemcpyHostToDevice, st));
+    TG_CUDA(ctx, cudaMemcpyAsync(e + 2 * nu + nw, det->w_hi, nw * sizeof(double), cudaMemcpyHostToDevice, st));
+    HistParams P;
+    P.hit_u = ions->hit_u; P.hit_w = ions->hit_w; P.cell = ions->cell; P.flags = ions->flags; P.group = ions->group;
+    P.n = ions->n;
+    P.u_lo = e; P.u_hi = e + nu; P.w_lo = e + 2 * nu; P.w_hi = e + 2 * nu + nw;
+    P.nu = det->nu; P.nw = det->nw; P.n_hist = n_hist;
+    P.inv_pu = uniform_inv_pitch(det->u_lo, det->u_hi, det->nu);
+    P.inv_pw = uniform_inv_pitch(det->w_lo, det->w_hi, det->nw);
+    P.counts = counts; P.summary = summary;
+    unsigned blocks = (unsigned)((ions->n + 255) / 256);
+    if ((long long)n_hist * det->nw * det->nu <= HIST_SMEM_BINS) k_histogram<true><<<blocks, 256, 0, st>>>(P);
+    else k_histogram<false><<<blocks, 256, 0, st>>>(P);
+    TG_CUDA(ctx, cudaGetLastError());
+    return TAIGA_OK;
+}

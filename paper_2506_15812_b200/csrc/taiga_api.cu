@@ -240,6 +240,26 @@ extern "C" int taiga_detector_histogram(taiga_ctx* ctx, const taiga_ions* ions, 
     return tg_histogram(ctx, ions, det, n_hist, counts, summary);
 }
 
+// The binning of taiga_detector_histogram for callers that must not allocate (include/taiga.h): same checks, same kernel,
+// the edge table in a fixed device array of the library instead of a buffer of the context.
+extern "C" int taiga_detector_histogram_static(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
+                                               unsigned long long* counts, unsigned long long* summary) {
+    if (!ctx) return TAIGA_E_ARG;
+    int rc = check_ions(ctx, ions, true);
+    if (rc) return rc;
+    rc = check_det(ctx, det, true);
+    if (rc) return rc;
+    if (n_hist < 1 || n_hist > 65536 || !counts || !summary) { TG_SET_ERR(ctx, "histogram_static: bad n_hist / null output"); return TAIGA_E_ARG; }
+    if (det->nu + det->nw > TAIGA_STATIC_MAX_SEGMENTS) {
+        TG_SET_ERR(ctx, "histogram_static: nu + nw = %d segments exceed TAIGA_STATIC_MAX_SEGMENTS = %d (the fixed edge table); "
+                        "use taiga_detector_histogram, which allocates", det->nu + det->nw, TAIGA_STATIC_MAX_SEGMENTS);
+        return TAIGA_E_ARG;
+    }
+    if (ions->n == 0) return TAIGA_OK;
+    TG_CUDA(ctx, cudaSetDevice(ctx->device));
+    return tg_histogram_static(ctx, ions, det, n_hist, counts, summary);
+}
+
 extern "C" int taiga_set_option(taiga_ctx* ctx, const char* key, long long v) {
     if (!ctx || !key) return TAIGA_E_ARG;
     struct { const char* k; int* p; long long lo, hi; } tab[] = {

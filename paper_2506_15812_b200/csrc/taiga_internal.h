@@ -133,6 +133,8 @@ bool tg_mma_supported(const taiga_ctx* ctx);
 int tg_build_dtable(taiga_ctx* ctx);                             // field_precompute.cu
 int tg_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
                  unsigned long long* counts, unsigned long long* summary);
+int tg_histogram_static(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
+                        unsigned long long* counts, unsigned long long* summary);       // histogram.cu: no allocation
 int tg_field_eval(taiga_ctx* ctx, uint64_t n, const double* R, const double* Z, const double* s,
                   double* BR, double* BZ, double* Bp);
 int tg_field_table(taiga_ctx* ctx, int comp, double* host);

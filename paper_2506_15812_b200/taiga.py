@@ -25,13 +25,14 @@ D3 = C.c_double * 3
 OK, E_ARG, E_STATE, E_CUDA, E_NOMEM = 0, -1, -2, -3, -4
 CELL_MISS, CELL_MAXSTEPS, CELL_OUT, CELL_BADSTART = -1, -2, -3, -4
 FLAG_EDGE, FLAG_PLANE, FLAG_GRID = 1, 2, 4
+STATIC_MAX_SEGMENTS = 2048       # TAIGA_STATIC_MAX_SEGMENTS
 
 EXPORTS = ["taiga_create", "taiga_destroy", "taiga_last_error", "taiga_load_field", "taiga_load_loss",
            "taiga_detector_histogram_weighted", "taiga_seed_beam_grid",
            "taiga_field_eval", "taiga_field_table", "taiga_seed_beam", "taiga_trace",
            "taiga_detector_histogram", "taiga_set_efield", "taiga_load_efield", "taiga_set_option", "taiga_get_stats",
            "taiga_measure_fp64_peak", "taiga_measure_l1_gather_peak", "taiga_measure_dmma_peak", "taiga_measure_mixed_fp64_peak",
-           "taiga_loss_statistics"]
+           "taiga_loss_statistics", "taiga_detector_histogram_static"]
 
 
 class GridS(C.Structure):
@@ -87,6 +88,7 @@ _lib.taiga_trace.argtypes = [C.c_void_p, C.POINTER(IonsS), C.c_double, C.c_doubl
                              C.POINTER(DetS), C.c_int]
 _lib.taiga_detector_histogram.argtypes = [C.c_void_p, C.POINTER(IonsS), C.POINTER(DetS), C.c_int,
                                           C.c_void_p, C.c_void_p]
+_lib.taiga_detector_histogram_static.argtypes = _lib.taiga_detector_histogram.argtypes
 _lib.taiga_seed_beam_grid.argtypes = [C.c_void_p, C.POINTER(BeamS), C.POINTER(SeedGridS), C.POINTER(IonsS)]
 _lib.taiga_load_loss.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(LossProfileS)]
 _lib.taiga_detector_histogram_weighted.argtypes = [C.c_void_p, C.POINTER(IonsS), C.POINTER(DetS), C.c_int,
@@ -301,6 +303,18 @@ class Taiga:
         assert counts.numel() == n_hist * d.nu * d.nw and summary.numel() == n_hist * 6
         self._chk(_lib.taiga_detector_histogram(self.h, C.byref(s), C.byref(d), int(n_hist),
                                                 counts.data_ptr(), summary.data_ptr()))
+
+    def detector_histogram_static(self, ions, det, n_hist, counts, summary):
+        """detector_histogram without any allocation inside the library (taiga_detector_histogram_static): for loops that
+        must not stall the device's other streams or that run under a memory pool owning the GPU.  The segment edges go to
+        a fixed 32 KB array of the library, so det.nu + det.nw <= STATIC_MAX_SEGMENTS (TaigaError otherwise), and calls
+        on one device must not overlap on the GPU."""
+        d, keep = self._det(det)
+        s = ions.struct()
+        assert counts.dtype == torch.int64 and summary.dtype == torch.int64
+        assert counts.numel() == n_hist * d.nu * d.nw and summary.numel() == n_hist * 6
+        self._chk(_lib.taiga_detector_histogram_static(self.h, C.byref(s), C.byref(d), int(n_hist),
+                                                       counts.data_ptr(), summary.data_ptr()))
 
     def set_option(self, key, value):
         self._chk(_lib.taiga_set_option(self.h, key.encode(), int(value)))
