@@ -27,9 +27,41 @@ sys.path.insert(0, ROOT)
 # FP64-pipe instructions per ion-step of the classical RKN step on a 2-D bicubic field
 # (3 field evaluations x 61 + 4 cross products x 6 + stage/Eq.5/plane 45).
 ALG_FP64_INSTR_PER_ION_STEP = {0: 252.0, 1: 402.0, 2: 840.0}
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel at the FULL size of the config, from
-# the latest `ncu --set full` capture of that kernel (not measured by this run): {config: (bytes, capture)}
-NCU_DRAM_BYTES_PER_LAUNCH = {2: (175.2e6, "profiles/r2_trace_ncu.md"), 4: (1686e6, "profiles/r2_trace_ncu.md")}
+# roofline.traffic (dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel at the FULL size of the
+# config) is not measured by this run: it is read from profiles/traffic.json, which names the `ncu --set full` capture each
+# figure comes from and the hash of the kernel sources it was taken at (csrc_hash below); any later change under csrc/
+# makes the figure stale and the line prints traffic = null.
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "traffic.json")
+
+
+def csrc_hash():
+    """sha256 (first 16 hex digits) over the names and contents of paper_2506_15812_b200/csrc/*.{cu,cuh,h}."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2506_15812_b200", "csrc")
+    for f in sorted(glob.glob(os.path.join(d, "*"))):
+        if f.endswith((".cu", ".cuh", ".h")):
+            h.update(os.path.basename(f).encode())
+            h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(config, default_run):
+    """(bytes per launch | None, source string | None) for `config` at its default launch configuration."""
+    if not default_run:
+        return None, "not the configuration the capture was taken in (options / size / detector / solver changed)"
+    try:
+        ent = json.load(open(TRAFFIC_JSON))["configs"].get(str(config))
+    except (OSError, ValueError, KeyError):
+        ent = None
+    if not ent:
+        return None, "no ncu --set full capture recorded for config %d in profiles/traffic.json" % config
+    if ent.get("csrc_hash") != csrc_hash():
+        return None, "stale: %s was taken at csrc hash %s, the sources are now %s" % (ent.get("capture"), ent.get("csrc_hash"), csrc_hash())
+    return float(ent["dram_bytes_per_launch"]), "per launch, from the ncu --set full capture in %s (not measured by this run)" % ent["capture"]
+
+
 NOMINAL_FP64_INSTR_PER_S = 148 * 64 * 1.965e9      # B200: 148 SMs x 64 FP64 lanes x 1965 MHz
 # kinds 1 and 2 are bound by the L1 -> register delivery of the gathered coefficients (DESIGN.md section 6):
 # bytes per ion-step = 3 evaluations x (384: slice difference, kind 1 | 1536: tricubic cell, kind 2; fp32 halves it)
@@ -52,6 +84,7 @@ def parse():
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = every rank traces the config's ions (default), strong = the config's ions are split")
     ap.add_argument("--oracle-full", action="store_true", help="time the oracle ONCE on the full config (16 threads and 1 thread on a prefix) and exit")
+    ap.add_argument("--csrc-hash", action="store_true", help="print the hash of the kernel sources that profiles/traffic.json entries carry, and exit")
     ap.add_argument("--dry-run-ranks", action="store_true", help="stop after the rank / shard set-up (CPU test of the launch path)")
     return ap.parse_args()
 
@@ -293,8 +326,7 @@ def main_ours(args):
         per_eval = (alg - 69.0) / 3.0
         alg = {1: 4 * per_eval + 69.0, 2: 4 * per_eval + 75.0, 3: per_eval + 45.0, 4: per_eval + 45.0}[args.solver]
     achieved = ion_steps_rank * alg / (t_trace * 1e-3)
-    tr = NCU_DRAM_BYTES_PER_LAUNCH.get(args.config) if not (args.ions or args.solver or args.opt or world > 1 and args.scaling == "strong") else None
-    traffic = (tr[0], "per launch, from the ncu --set full capture in %s (not measured by this run)" % tr[1]) if tr else (None, None)
+    traffic = ncu_traffic(args.config, not (args.ions or args.solver or args.opt or args.detector != "config" or world > 1 and args.scaling == "strong"))
     h2d = sum(p.numel() * 8 for p in nodal_pin) + (len(cd) + len(cn)) * 8 * len(cfg.groups) + 4 * (det0.nu + det0.nw) * 8
     d2h = counts.numel() * 8 + summary.numel() * 8
     s_ok = int(summary[:, :5].sum().item()) == n_ions
@@ -362,7 +394,9 @@ def main_ours(args):
 
 if __name__ == "__main__":
     a = parse()
-    if a.oracle_full:
+    if a.csrc_hash:
+        print(csrc_hash())
+    elif a.oracle_full:
         main_oracle_full(a)
     elif a.impl == "reference":
         main_reference(a)

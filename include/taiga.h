@@ -59,7 +59,7 @@ const char* taiga_last_error(const taiga_ctx* ctx);
  *   (A16).  kind 2: nS toroidal planes spanning ONE period nS*ds, periodic cubic spline in phi
  *   (tricubic, A17).  Grids are uniform; node (i,j) sits at Rmin+i*hR, Zmin+j*hZ. */
 typedef struct {
-    int kind, nR, nZ, nS;            /* nR,nZ >= 4; nS = 1 (kind 0), >= 2 (kind 1), >= 3 (kind 2) */
+    int kind, nR, nZ, nS;            /* nR,nZ >= 4; nS = 1 (kind 0), >= 2 (kind 1), 3 ... 128 (kind 2) */
     double Rmin, Rmax, Zmin, Zmax;
     double s0, ds;                   /* first slice time, spacing [s]  |  phi0, dphi [rad]        */
 } taiga_grid;
@@ -186,7 +186,7 @@ int taiga_set_efield(taiga_ctx* ctx, const double E_V_per_m[3]);
  * B and ADDED to the uniform field of taiga_set_efield at every stage of every solver (Boris: at r(t0), as B).  c == NULL
  * removes it.  Must follow taiga_load_field (TAIGA_E_STATE otherwise); a later taiga_load_field removes it.  The table is
  * gathered per evaluation (48 coefficients through L1, no register cache): meant for edge studies, not for the production
- * E = 0 path, whose kernels are unchanged.  fp64 only, like the uniform E. */
+ * E = 0 path, whose kernels are unchanged.  fp64 only, like the uniform E: taiga_trace refuses "precision" = 32 while either is set. */
 int taiga_load_efield(taiga_ctx* ctx, const taiga_coeffs* c);
 
 /* ---- a5: binning + histogram (segment ID per ion; atomically summed
@@ -252,8 +252,9 @@ int taiga_load_loss(taiga_ctx* ctx, const double* psi_nodal, int psi_on_device,
  * or counts) are clamped: negative and NaN count as 0, larger ones as 2^20; ions whose group is >= n_hist are
  * skipped (as in taiga_detector_histogram).
  * Call after taiga_detector_histogram (uses ions->cell); needs ions->weight or ions->w0.  A non-null
- * ions->weight must have been written by the last taiga_trace of this context (a loss model loaded), else
- * TAIGA_E_STATE: pass weight = NULL to count w0 only. */
+ * ions->weight must lie inside a weight array that one of the 16 most recent taiga_trace calls of this context wrote
+ * (a loss model loaded) and that no later trace without a loss model has gone over, else TAIGA_E_STATE: weights of
+ * your own go in w0, with weight = NULL. */
 int taiga_detector_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det,
                                       int n_hist, unsigned long long* wcounts_dev,
                                       unsigned long long* wsummary_dev);
@@ -282,7 +283,7 @@ int taiga_loss_statistics(const unsigned long long wsummary_host[4], double out_
  * control point at the mean of r_n + v_n dt/2 and r_n+1 - v_n+1 dt/2, reading Z1;
  * RKN solvers (the Boris velocities live at half steps), with or without E and the loss model (whose crossing step then
  * counts up to the curve parameter of the hit)), "mma" (kinds 1 and 2, fp64: 1 = warp-cooperative evaluation on the FP64
- * tensor pipe (trace_mma.cu; default for kind 2), 0 = one lane evaluates its own ion (trace.cu; default for kind 1),
+ * tensor pipe (trace_mma.cu; default for kind 2; kind-2 tables with planes more than 0.04 rad apart always take the other path), 0 = one lane evaluates its own ion (trace.cu; default for kind 1),
  * -1 = the default of the kind), "regroup" (kinds 1 / 2: the CTA re-sorts its 128 ions over its lanes by field cell
  * every this many steps, so that the lanes of a warp / of an 8-ion group share cells; default 8; with mma = 0, 0 = off:
  * per-warp tiles), "refill_cta" (mma: the CTA refills its finished lanes from the queue at a re-sort point once this

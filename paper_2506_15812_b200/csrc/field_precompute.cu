@@ -8,8 +8,8 @@
 // The map y -> M is linear, M = H y, and because the (1,4,1) system is diagonally dominant the
 // entries of H decay like (2-sqrt 3)^|i-j| = 0.268^|i-j|: beyond |i-j| = 36 they are below
 // 3e-21 of the diagonal.  So instead of one serial Thomas solve per grid line (a few hundred
-// threads, latency bound) the band of H is built once per line length on the host (O(n^2), by
-// running the reduction above on unit vectors) and every node is then an independent 73-point
+// threads, latency bound) the band of H is built once per line length on the device (k_spline_band:
+// one thread per column runs the reduction above on a unit vector) and every node is then an independent 73-point
 // stencil: one thread per node, coalesced, exact to rounding.  One thread per (cell, component)
 // finally assembles the 16 power-basis coefficients from {y, y_zz, y_rr, y_rrzz} at 4 corners.
 #include "field_device.cuh"
@@ -80,15 +80,17 @@ static int tg_ensure_band(taiga_ctx* ctx, int ax, int n) {
 
 // kind 2: first column G of the inverse of the circulant (1,4,1) matrix of the periodic spline, closed form: with
 // r = sqrt(3) - 2 (root of r^2 + 4 r + 1) the infinite chain has g_k = r^|k| / (2 sqrt 3); summing the periodic images
-// gives G_k = (r^k + r^(n-k)) / ((1 - r^n) 2 sqrt 3).
+// gives G_k = (r^k + r^(n-k)) / ((1 - r^n) 2 sqrt 3) = G_(n-k).  Both powers come from the same forward products r^k, which
+// fade to zero far from the diagonal (the right value to rounding) instead of being divided back up from r^n (which
+// loses digits as n grows and underflows at n ~ 540; taiga_load_field takes n <= TG_MAX_PLANES = 128 anyway).
 __global__ void k_circulant_inverse_col(double* __restrict__ G, int n) {
     if (blockIdx.x || threadIdx.x) return;
     const double s3 = sqrt(3.0), r = s3 - 2.0;
-    double rn = 1.0;
-    for (int k = 0; k < n; ++k) rn *= r;
-    const double norm = 1.0 / ((1.0 - rn) * 2.0 * s3);
-    double up = 1.0, dn = rn;                                       // r^k, r^(n-k)
-    for (int k = 0; k < n; ++k) { G[k] = (up + dn) * norm; up *= r; dn /= r; }
+    double up = 1.0;
+    for (int k = 0; k < n; ++k) { G[k] = up; up *= r; }             // r^k; up ends as r^n
+    const double norm = 1.0 / ((1.0 - up) * 2.0 * s3);
+    G[0] = (1.0 + up) * norm;
+    for (int k = 1; 2 * k <= n; ++k) { const double v = (G[k] + G[n - k]) * norm; G[k] = v; G[n - k] = v; }
 }
 
 // power-basis coefficients of one interval from end values g0,g1 and end second derivatives G0,G1
@@ -242,7 +244,7 @@ int tg_precompute(taiga_ctx* ctx, const taiga_grid* g, const taiga_coeffs* c) {
         double *tmp = Mzr + 3 * nnode, *G = tmp + n_tmp;
         // band operators, cached per line length (device-built)
         for (int ax = 0; ax < 2; ++ax) { rc = tg_ensure_band(ctx, ax, ax ? nR : nZ); if (rc) return rc; }
-        if (g->kind == 2) k_circulant_inverse_col<<<1, 32, 0, st>>>(G, nS);
+        if (g->kind == 2) { k_circulant_inverse_col<<<1, 32, 0, st>>>(G, nS); TG_CUDA(ctx, cudaGetLastError()); }
         for (int m = 0; m < 3; ++m)
             TG_CUDA(ctx, cudaMemcpyAsync(y + (size_t)m * nnode, src[m], nnode * sizeof(double),
                                          c->on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));

@@ -200,10 +200,15 @@ extern "C" int taiga_detector_histogram_weighted(taiga_ctx* ctx, const taiga_ion
     if (n_hist < 1 || n_hist > 65536 || !wcounts || !wsummary) { TG_SET_ERR(ctx, "histogram_weighted: bad n_hist / null output"); return TAIGA_E_ARG; }
     if (ions->n == 0) return TAIGA_OK;
     if (!ions->weight && !ions->w0) { TG_SET_ERR(ctx, "histogram_weighted: ions->weight and ions->w0 are null"); return TAIGA_E_ARG; }
-    if (ions->weight && !ctx->weight_written) {
-        TG_SET_ERR(ctx, "histogram_weighted: ions->weight is set but the last taiga_trace of this context wrote no weights "
-                        "(no loss model loaded); pass weight = null to count w0 only");
-        return TAIGA_E_STATE;
+    if (ions->weight) {
+        bool known = false;
+        for (int q = 0; q < ctx->n_wranges && !known; ++q)
+            known = ctx->wranges[q].p <= ions->weight && ions->weight + ions->n <= ctx->wranges[q].p + ctx->wranges[q].n;
+        if (!known) {
+            TG_SET_ERR(ctx, "histogram_weighted: ions->weight is set but no recent taiga_trace of this context wrote these weights "
+                            "(no loss model loaded, or other ions traced); pass your own weights as w0 with weight = null");
+            return TAIGA_E_STATE;
+        }
     }
     TG_CUDA(ctx, cudaSetDevice(ctx->device));
     return tg_histogram_weighted(ctx, ions, det, n_hist, wcounts, wsummary);

@@ -81,7 +81,10 @@ struct taiga_ctx {
     int opt_sort, opt_min_active, opt_ctas_per_sm, opt_variant, opt_stats;
     int opt_sort_sub, opt_precision, opt_plane_interp, opt_regroup;
     int opt_mma, opt_refill_cta, opt_mma_geom;
-    bool weight_written;                                 // the last taiga_trace wrote ions->weight (loss model)
+    // ions->weight ranges written by recent taiga_trace calls with a loss model (newest last); a trace without one drops
+    // the ranges it overlaps (their weights are stale).  taiga_detector_histogram_weighted accepts a weight array inside one.
+    struct { const double* p; uint64_t n; } wranges[16];
+    int n_wranges;
 };
 
 #define TG_SET_ERR(ctx, ...) snprintf((ctx)->err, sizeof((ctx)->err), __VA_ARGS__)

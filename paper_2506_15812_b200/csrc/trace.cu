@@ -53,6 +53,10 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         TG_SET_ERR(ctx, "the loss model is offered in fp64");
         return TAIGA_E_ARG;
     }
+    if (hasE && f32) {
+        TG_SET_ERR(ctx, "precision=32 is offered without an electric field (the uniform and the gridded E are fp64 only)");
+        return TAIGA_E_ARG;
+    }
     TraceParams P;
     P.f = ctx->field; P.det = det;
     P.loss = ctx->loss; P.hdt = 0.5 * dt; P.weight = ions->weight; P.w0 = ions->w0;
@@ -160,7 +164,17 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
     }
     ++launches;
     TG_CUDA(ctx, cudaGetLastError());
-    ctx->weight_written = loss;
+    if (ions->weight) {        // bookkeeping for taiga_detector_histogram_weighted: which weight arrays hold this context's results
+        const double *lo = ions->weight, *hi = ions->weight + ions->n;
+        int m = 0;
+        for (int q = 0; q < ctx->n_wranges; ++q)
+            if (ctx->wranges[q].p + ctx->wranges[q].n <= lo || hi <= ctx->wranges[q].p) ctx->wranges[m++] = ctx->wranges[q];
+        if (loss) {
+            if (m == 16) { for (int q = 1; q < 16; ++q) ctx->wranges[q - 1] = ctx->wranges[q]; m = 15; }
+            ctx->wranges[m].p = lo; ctx->wranges[m].n = ions->n; ++m;
+        }
+        ctx->n_wranges = m;
+    }
     if (ctx->opt_stats) {
         TG_CUDA(ctx, cudaMemcpyAsync(ctx->counters_host, ctx->counters, 8 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
         TG_CUDA(ctx, cudaStreamSynchronize(st));

@@ -17,7 +17,7 @@
 //  * the velocity is carried as u = (q/m) v, so a = u x B needs no scaling per evaluation;
 //  * classical variant: k2 and k3 share their position, so B is evaluated 3x, not 4x, per step;
 //  * kind 0 (static 2-D): the 48 coefficients of the lane's current cell are cached in
-//    registers and re-read (24 x 128-bit loads, one 128-B line per component) only when the
+//    registers and re-read (12 x 256-bit loads, one 128-B line per component) only when the
 //    lane leaves the cell (~0.35 times per step);
 //  * 1/R by MUFU.RSQ64H seed + one cubic (Halley) step: 6 FP64 instructions instead of ~30.
 #pragma once

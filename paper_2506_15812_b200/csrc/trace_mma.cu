@@ -1,5 +1,6 @@
-// a3 + a4 for the table kinds 1 (time slices) and 2 (R, Z, phi): the field evaluation as a small FP64
-// tensor-core product, coefficients delivered ONCE PER WARP instead of once per lane.
+// a3 + a4 for the (R, Z, phi) tables of kind 2 (the default there) and, on request ("mma" = 1), the time slices of
+// kind 1, which default to k_trace (trace.cu): the field evaluation as a small FP64 tensor-core product,
+// coefficients delivered ONCE PER WARP instead of once per lane.
 //
 // PAPER.md L63 (stored spline coefficients), L177 (field interpolated at every stage), Eq. 5-6; L47 and
 // L406-408 (perturbed, non-axisymmetric fields are what the GPU solver is for).
@@ -550,12 +551,18 @@ static int tg_phi_cells(const FieldDev& f) {
     return (int)r;
 }
 
+// Plane spacing up to which tg_locate_tor's four-term asin series is exact to rounding: the first dropped term of
+// q = asin(s) / ds is (35 / 1152) s^9 / ds <= 0.0304 ds^8 = 2.0e-13 of a cell at ds = 0.04 (|s| <= ds once K has settled);
+// 2.6e-10 at ds = 2 pi / 64 and 6.5e-8 at 2 pi / 32 would break the 1e-9 m parity.  Coarser plane sets (full-torus tables
+// with a few dozen planes) go to the per-lane kernel, which takes the angle from atan2 (tg_locate_cell<2>).
+#define TG_MMA_MAX_DS 0.04
+
 // Is the cooperative kernel offered for this field?  (cell ids are 32-bit; 2 slices / planes at least)
 bool tg_mma_supported(const taiga_ctx* ctx) {
     const FieldDev& f = ctx->field;
     if (f.kind != 1 && f.kind != 2) return false;
     const long long ncell = (long long)f.cR * f.cZ * f.nS;
-    if (f.kind == 2 && tg_phi_cells(f) == 0) return false;
+    if (f.kind == 2 && (tg_phi_cells(f) == 0 || !(f.inv_ds * TG_MMA_MAX_DS >= 1.0))) return false;
     return ncell < (1ll << 31) && f.nS >= 2;
 }
 

@@ -161,6 +161,24 @@ def test_kernel_options_of_the_sliced_fields(tg, icfg, n, opts):
     assert st["flagged"] <= 8, st
 
 
+@pytest.mark.parametrize("nS,ncoil", [(16, 1), (32, 1), (32, 4), (32, 8)])
+@pytest.mark.parametrize("mma", [1, 0])
+def test_coarse_toroidal_planes_parity(tg, nS, ncoil, mma):
+    """(R, Z, phi) tables whose planes are far apart: 16 and 32 planes round the whole torus (ds = 0.39, 0.20), 0.049 just
+    above and 0.0245 below the spacing up to which the cooperative tracer's asin series is exact to rounding
+    (TG_MMA_MAX_DS = 0.04: coarser tables take the atan2 path whatever "mma" says).  Same 1e-9 m bar on every one."""
+    from paper_2506_15812_b200 import taiga
+    tg.set_option("mma", mma)
+    cfg = wl.config(5, n_override=2048 + 5)
+    cfg.field_builder = lambda: wl.nodal_field_ripple(65, 129, nS, ncoil)
+    ions, counts, summary = taiga.run_config(tg, cfg)
+    torch.cuda.synchronize()
+    ref = orc.run_config(cfg)
+    st = compare_groups(ions, ref, "kind 2, %d planes x %d periods, mma=%d" % (nS, ncoil, mma))
+    check_histogram(cfg, ions, counts, summary, ref)
+    assert st["flagged"] <= 8 and int(summary[0, 0]) > 1000
+
+
 def test_roofline_denominators_are_consistent(tg):
     """The microkernels behind bench.py's roofline: the DFMA and DMMA issue rates are within 3 % of 148 x 64 FMA per clock
     at the clock nvidia-smi reports as maximum (never above it), and interleaving both does not exceed either (one FP64 datapath)."""
@@ -318,6 +336,24 @@ def test_field_precompute_vs_oracle_tables(tg, kind):
     out1 = [_np(o) for o in tg.field_eval(torch.from_numpy(R).cuda(), torch.from_numpy(Z).cuda(), torch.from_numpy(s).cuda())]
     for c in range(3):
         assert np.abs(out1[c] - out[c]).max() < 1e-12
+
+
+def test_periodic_spline_at_the_plane_limit(tg):
+    """128 toroidal planes, the most taiga_load_field takes for a kind-2 table (129 are refused with a message): the closed-form
+    circulant inverse against the oracle's dense cyclic elimination, every plane including the seam 127 -> 0."""
+    from paper_2506_15812_b200 import taiga
+    grid, nodal = wl.nodal_field_ripple(5, 6, 128, ncoil=1)
+    rng = np.random.default_rng(5)
+    nodal = [c + 1e-3 * rng.standard_normal(c.shape) for c in nodal]
+    f = orc.OracleField(grid, nodal)
+    tg.load_field(grid, nodal)
+    for comp in range(3):
+        tab = tg.field_table(comp, f.tables[comp].shape)
+        err = np.abs(tab - f.tables[comp]).reshape(128, -1).max(axis=1)
+        assert err.max() < 2e-13 * max(np.abs(f.tables[comp]).max(), 1.0), (comp, int(err.argmax()), err.max())
+    with pytest.raises(taiga.TaigaError) as e:
+        tg.load_field(*wl.nodal_field_ripple(5, 6, 129, ncoil=1))
+    assert e.value.code == taiga.E_ARG and "128" in str(e.value)
 
 
 @pytest.mark.parametrize("n_hist,nu,nw", [(3, 4, 3), (40, 16, 16)])
@@ -916,6 +952,37 @@ def test_error_paths_of_the_widened_entry_points(tg):
     with pytest.raises(taiga.TaigaError) as e:                # weights the last trace did not write (no loss model) are refused
         t2.detector_histogram_weighted(ions, cfg.detector, 1, wc, ws)
     assert e.value.code == taiga.E_STATE
+    # ... per weight array, not per context: trace A with the model, then B, then A's weights still count and C's do not
+    t2.load_loss(wl.nodal_psi(grid), psi0, dpsi, ne, te, wl.E12_LI)
+    ionsB, ionsC = taiga.Ions(64), taiga.Ions(64)
+    for io in (ionsB, ionsC):
+        t2.seed_beam(g.beam, wl.depth_cdf(), wl.normal_cdf(), 0, io)
+    t2.trace(ions, qm, cfg.dt, 5000, cfg.detector)
+    t2.trace(ionsB, qm, cfg.dt, 5000, cfg.detector)
+    for io in (ions, ionsB, ions.view(8, 40)):
+        t2.detector_histogram_weighted(io, cfg.detector, 1, wc, ws)
+    with pytest.raises(taiga.TaigaError) as e:
+        t2.detector_histogram_weighted(ionsC, cfg.detector, 1, wc, ws)
+    assert e.value.code == taiga.E_STATE
+    t2.load_loss(None)
+    t2.trace(ionsB, qm, cfg.dt, 5000, cfg.detector)           # B's weights are stale now, A's are not
+    t2.detector_histogram_weighted(ions, cfg.detector, 1, wc, ws)
+    with pytest.raises(taiga.TaigaError) as e:
+        t2.detector_histogram_weighted(ionsB, cfg.detector, 1, wc, ws)
+    assert e.value.code == taiga.E_STATE
+    # fp32 evaluation with an electric field is not offered
+    g5, n5 = wl.nodal_field_ripple(9, 9, 8)
+    t2.load_field(g5, n5)
+    t2.set_option("precision", 32)
+    t2.set_efield((1e3, 0, 0))
+    with pytest.raises(taiga.TaigaError) as e:
+        t2.trace(ions, qm, cfg.dt, 10, cfg.detector)
+    assert e.value.code == taiga.E_ARG and "electric" in str(e.value)
+    t2.set_efield((0, 0, 0))
+    t2.trace(ions, qm, cfg.dt, 10, cfg.detector)
+    t2.set_option("precision", 64)
+    t2.load_field(grid, nodal)
+    ions.a["weight"].fill_(5.0)
     s = ions.struct(weight=False)
     assert s.w0 is None
     with pytest.raises(taiga.TaigaError):
