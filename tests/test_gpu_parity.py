@@ -390,6 +390,46 @@ def test_histogram_vs_oracle_gapped_detector(tg, n_hist, nu, nw):
     assert np.array_equal(_np(ions.flags)[valid], res["flags"][valid])
 
 
+def test_grazing_flags_match_the_oracle(tg):
+    """The flag bits decide which ions parity leaves out, so the CUDA path must set them where the oracle does (whose own
+    bits are pinned on the CPU, P25): straight flights in a zero field ending a step 5e-10 / 0.9e-9 / 1.1e-9 / 2e-9 m before
+    and behind the detector plane and the four grid boundaries, and starts within the threshold.  cell, steps, flags
+    bit for bit."""
+    from paper_2506_15812_b200 import taiga
+    grid, nodal = wl.nodal_field_2d(9, 17)
+    nodal = [np.zeros_like(c) for c in nodal]
+    tg.load_field(grid, nodal)
+    f = orc.OracleField(grid, nodal)
+    qm = wl.E_CHARGE / wl.MASS_LI7
+    one = [np.array([-1.0]), np.array([1.0])] * 2
+    d = np.array([-5e-10, 5e-10, -0.9e-9, 0.9e-9, -1.1e-9, 1.1e-9, -2e-9, 2e-9, -0.5e-3])
+    cases = []                                               # (detector, x0, z0, vx, vz)
+    det = wl.Detector((0.80, 0, 0), (1, 0, 0), (0, 1, 0), (0, 0, 1), *one)
+    cases.append((det, np.concatenate([0.80 - 3e-3 + d, 0.80 + np.array([-5e-10, 0.0, 5e-10, 1e-3])]), 0.0, 1e6, 0.0))
+    far = wl.Detector((5.0, 0, 0), (1, 0, 0), (0, 1, 0), (0, 0, 1), *one)
+    cases.append((far, np.concatenate([grid.Rmax - 3e-3 + d, grid.Rmax + np.array([-5e-10, 5e-10, 1e-3])]), 0.0, 1e6, 0.0))
+    back = wl.Detector((-5.0, 0, 0), (-1, 0, 0), (0, 1, 0), (0, 0, 1), *one)
+    cases.append((back, grid.Rmin + 3e-3 + d, 0.0, -1e6, 0.0))
+    cases.append((far, np.full(len(d), 0.5), grid.Zmax - 3e-3 + d, 1.0, 1e6))
+    cases.append((far, np.full(len(d), 0.5), grid.Zmin + 3e-3 - d, 1.0, -1e6))
+    seen = 0
+    for det, x0, z0, vx, vz in cases:
+        n = len(x0)
+        st = [np.asarray(x0, float), np.zeros(n), np.broadcast_to(np.asarray(z0, float), (n,)).copy(), np.full(n, vx), np.zeros(n), np.full(n, vz)]
+        ref = orc.trace(f, qm, st, None, 1e-9, 20, det)
+        ions = taiga.Ions(n)
+        for k, a in zip(("x", "y", "z", "vx", "vy", "vz"), st):
+            ions.a[k].copy_(torch.from_numpy(a))
+        tg.trace(ions, qm, 1e-9, 20, det)
+        torch.cuda.synchronize()
+        assert np.array_equal(_np(ions.flags), ref["flags"]), (_np(ions.flags), ref["flags"])
+        assert np.array_equal(_np(ions.steps).astype(np.uint32), ref["steps"])
+        assert np.array_equal(_np(ions.cell), np.where(ref["status"] == 0, -1, ref["status"]))
+        seen |= int(np.bitwise_or.reduce(ref["flags"]))
+        assert (ref["flags"] == 0).sum() >= 3
+    assert seen == 6
+
+
 def test_edge_cases_and_errors(tg):
     from paper_2506_15812_b200 import taiga
     cfg = wl.config(1)
