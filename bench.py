@@ -84,6 +84,9 @@ def parse():
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = every rank traces the config's ions (default), strong = the config's ions are split")
     ap.add_argument("--oracle-full", action="store_true", help="time the oracle ONCE on the full config (16 threads and 1 thread on a prefix) and exit")
+    ap.add_argument("--extras", default="auto", choices=["auto", "on", "off"],
+                    help="configs 1, 3, 4, 5 and the variant kernels in the same line (auto: on for the default line on one GPU)")
+    ap.add_argument("--extras-ions", type=int, default=0, help="ions per group for the extras (default: full size)")
     ap.add_argument("--csrc-hash", action="store_true", help="print the hash of the kernel sources that profiles/traffic.json entries carry, and exit")
     ap.add_argument("--dry-run-ranks", action="store_true", help="stop after the rank / shard set-up (CPU test of the launch path)")
     return ap.parse_args()
@@ -183,6 +186,149 @@ def main_reference(args):
         "ions_per_s": n_ions * args.steps / tot_t}))
 
 
+def alg_instr(kind, solver):
+    """The method's FP64 instructions per ion-step; other solvers: 4 (solver 1, 2) / 1 (Boris) evaluations."""
+    alg = ALG_FP64_INSTR_PER_ION_STEP[kind]
+    if solver:
+        per_eval = (alg - 69.0) / 3.0
+        alg = {1: 4 * per_eval + 69.0, 2: 4 * per_eval + 75.0, 3: per_eval + 45.0, 4: per_eval + 45.0}[solver]
+    return alg
+
+
+def measure_case(local, peak_dfma, icfg, ions_override=0, solver=0, opts=(), setup=None, weighted=False, steps=2, warmup=1):
+    """One more workload beside the headline: the whole path a1-a5 of BASELINE config `icfg` at full size (nodal field
+    resident in HBM), `warmup` untimed steps, then `steps` timed ones with CUDA events around the step and around the trace
+    kernel(s), an L2 flush in between, clocks sampled meanwhile.  Own context, so no option leaks into the next case.
+    `setup(tg, grid, wl)` loads what the variant needs (loss model, E) after the first load_field."""
+    import numpy as np
+    import torch
+    from paper_2506_15812_b200 import taiga, workloads as wl
+    dev = "cuda:%d" % local
+    cfg = wl.config(icfg, n_override=ions_override or None)
+    grid, nodal = cfg.field_builder()
+    nodal_dev = [torch.from_numpy(np.ascontiguousarray(c)).to(dev) for c in nodal]
+    tg = taiga.Taiga(local)
+    for k, v in opts:
+        tg.set_option(k, v)
+    tg.load_field(grid, nodal_dev)
+    if setup:
+        setup(tg, grid, wl)
+    ions = taiga.Ions(cfg.n_ions, dev)
+    det0 = cfg.detector or cfg.groups[0].detector
+    counts = torch.zeros((cfg.n_hist, det0.nw, det0.nu), dtype=torch.int64, device=dev)
+    summary = torch.zeros((cfg.n_hist, 6), dtype=torch.int64, device=dev)
+    wcounts, wsummary = torch.zeros_like(counts), torch.zeros((cfg.n_hist, 4), dtype=torch.int64, device=dev)
+    cd, cn = wl.depth_cdf(), wl.normal_cdf()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def step():
+        marks = [ev() for _ in range(5)]
+        marks[0].record()
+        tg.load_field(grid, nodal_dev)
+        if setup:
+            setup(tg, grid, wl)
+        counts.zero_(); summary.zero_(); wcounts.zero_(); wsummary.zero_()
+        off, spans = 0, []
+        for g in cfg.groups:
+            v = ions.view(off, off + g.n_ions)
+            tg.seed_beam(g.beam, cd, cn, cfg.seed, v, g.first_index, g.group, g.t0)
+            spans.append((v, g)); off += g.n_ions
+        whole = [(ions, cfg.groups[0], cfg.detector)] if cfg.detector is not None else [(v, g, g.detector) for v, g in spans]
+        marks[1].record()
+        for v, g, d in whole:
+            tg.trace(v, g.beam.charge_C / g.beam.mass_kg, cfg.dt, cfg.max_steps, d, solver)
+        marks[2].record()
+        for v, g, d in whole:
+            tg.detector_histogram(v, d, cfg.n_hist, counts, summary)
+        marks[3].record()
+        if weighted:
+            for v, g, d in whole:
+                tg.detector_histogram_weighted(v, d, cfg.n_hist, wcounts, wsummary)
+        marks[4].record()
+        return marks
+
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    t_step = t_trace = t_hist = t_whist = 0.0
+    for _ in range(steps):
+        flush.zero_()
+        torch.cuda.synchronize()
+        m = step()
+        torch.cuda.synchronize()
+        t_step += m[0].elapsed_time(m[4]); t_trace += m[1].elapsed_time(m[2]); t_hist += m[2].elapsed_time(m[3]); t_whist += m[3].elapsed_time(m[4])
+    sampler.stop_flag = True
+    ion_steps = int(ions.steps.to(torch.int64).sum().item())
+    ok = int(summary[:, :5].sum().item()) == cfg.n_ions
+    t_step, t_trace, t_hist, t_whist = (t / steps for t in (t_step, t_trace, t_hist, t_whist))
+    kind = grid.kind
+    o = dict(opts)
+    f32 = o.get("precision") == 32
+    mma = kind != 0 and not f32 and (o.get("mma", -1) == 1 or (o.get("mma", -1) == -1 and kind == 2))
+    rate = ion_steps / (t_trace * 1e-3)
+    alg = alg_instr(kind, solver)
+    out = {"workload": "BASELINE config %d (%s): %d ions, grid %dx%dx%d kind %d, dt=%g, max_steps=%d" % (
+               icfg, cfg.name, cfg.n_ions, grid.nR, grid.nZ, grid.nS, kind, cfg.dt, cfg.max_steps),
+           "steps": steps, "warmup": warmup, "ms_per_step": t_step, "ion_steps_per_step": ion_steps,
+           "trace_kernel": {"ms": t_trace, "launches": len(cfg.groups) if cfg.detector is None else 1,
+                            "kernel": "k_trace_mma" if mma else "k_trace"},
+           "ion_steps_per_s": ion_steps / (t_step * 1e-3), "ions_per_s": cfg.n_ions / (t_step * 1e-3),
+           "trace_ion_steps_per_s": rate, "histogram_ms": t_hist,
+           "frac": rate * alg / peak_dfma, "frac_nominal": rate * alg / NOMINAL_FP64_INSTR_PER_S, "alg_fp64_instr_per_ion_step": alg,
+           "summary": [int(v) for v in summary.sum(dim=0).tolist()], "invariant_counts_sum_to_n": ok, "clocks": sampler.summary()}
+    if weighted:
+        out["weighted_histogram_ms"] = t_whist
+    if cfg.detector is None:                   # energy scan: per-group share of the steps (the 20 keV group is mostly non-crossers)
+        off, per = 0, []
+        for g in cfg.groups:
+            v = ions.view(off, off + g.n_ions)
+            per.append({"energy_eV": g.beam.energy_eV, "ion_steps": int(v.steps.to(torch.int64).sum().item()),
+                        "maxsteps_ions": int((v.cell == taiga.CELL_MAXSTEPS).sum().item())})
+            off += g.n_ions
+        out["groups"] = per
+    tg.close()
+    del ions, flush, nodal_dev
+    torch.cuda.empty_cache()
+    return out
+
+
+def extras(local, peak_dfma, ions_override=0):
+    """"configs": the other four BASELINE configs at full size; "variants": the widened kernels on config 2 and the fp32
+    evaluation on config 5 (SURVEY.md 8(d) "report per config")."""
+    import numpy as np
+
+    def loss(tg, grid, wl):
+        psi0, dpsi, ne, te = wl.loss_profile_inputs()
+        tg.load_loss(wl.nodal_psi(grid), psi0, dpsi, ne, te, wl.E12_LI)
+
+    def uniform_e(tg, grid, wl):
+        tg.set_efield((1.0e4, 0.0, -5.0e3))
+
+    def gridded_e(tg, grid, wl):
+        R = np.linspace(grid.Rmin, grid.Rmax, grid.nR)[:, None] * np.ones((1, grid.nZ))
+        Z = np.ones((grid.nR, 1)) * np.linspace(grid.Zmin, grid.Zmax, grid.nZ)[None, :]
+        tg.load_efield((4.0e4 * np.exp((R - 0.8) / 0.05) - 1.0e4 * 0.56 / R, 6.0e4 * Z, 2.0e4 + 0.0 * R))
+
+    n = ions_override
+    configs = {str(i): measure_case(local, peak_dfma, i, n) for i in (1, 3, 4, 5)}
+    variants = {
+        "cfg2 loss (Eq. 2) + weighted counters": measure_case(local, peak_dfma, 2, n, setup=loss, weighted=True),
+        "cfg2 Bezier plane interpolation": measure_case(local, peak_dfma, 2, n, opts=(("plane_interp", 1),)),
+        "cfg2 uniform E": measure_case(local, peak_dfma, 2, n, setup=uniform_e),
+        "cfg2 gridded E(R,Z)": measure_case(local, peak_dfma, 2, n, setup=gridded_e),
+        "cfg2 RK4 (solver 2)": measure_case(local, peak_dfma, 2, n, solver=2),
+        "cfg2 Boris-Verlet (solver 3)": measure_case(local, peak_dfma, 2, n, solver=3),
+        "cfg5 precision=32": measure_case(local, peak_dfma, 5, n, opts=(("precision", 32),)),
+    }
+    for k in ("cfg2 loss (Eq. 2) + weighted counters", "cfg2 Bezier plane interpolation", "cfg2 uniform E", "cfg2 gridded E(R,Z)", "cfg5 precision=32"):
+        for drop in ("frac", "frac_nominal", "alg_fp64_instr_per_ion_step"):      # no instruction count is claimed for these kernels
+            variants[k].pop(drop)
+    return configs, variants
+
+
 def launches_per_step(cfg, kind):
     a1 = 3 + 3 + (1 if kind == 2 else 0)       # 3 second-derivative stencils + 3 assembles [+ phi spline]
     ntrace = 1 if cfg.detector is not None else len(cfg.groups)
@@ -219,7 +365,11 @@ def main_ours(args):
     torch.cuda.set_device(local)
     if world > 1:
         import torch.distributed as dist
-        os.environ.setdefault("NCCL_DEBUG", "WARN")
+        # rank 0 logs the communicator set-up (transport, NVLS) to stderr, so that a scaling run can be checked against it;
+        # stdout stays the one JSON line
+        os.environ.setdefault("NCCL_DEBUG", "INFO" if rank == 0 else "WARN")
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+        os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     from paper_2506_15812_b200 import taiga
     dev = "cuda:%d" % local
@@ -232,6 +382,7 @@ def main_ours(args):
     grid, nodal = cfg.field_builder()
     nodal_dev = [torch.from_numpy(np.ascontiguousarray(c)).to(dev) for c in nodal]
     nodal_pin = [torch.from_numpy(np.ascontiguousarray(c)).pin_memory() for c in nodal]
+    nodal_host = [p.numpy() for p in nodal_pin]                                      # numpy views of the pinned buffers: host pointers for the ABI
     tg = taiga.Taiga(local)
     for kv in args.opt:
         k, v = kv.split("=")
@@ -252,11 +403,9 @@ def main_ours(args):
     trace_ms, hist_ms = [], []
 
     def step(host, record=False):
-        if host:
-            fld = [d.copy_(p, non_blocking=True) for d, p in zip(nodal_dev, nodal_pin)]   # H2D from pinned
-        else:
-            fld = nodal_dev
-        tg.load_field(grid, fld)                                                        # a1
+        # e2e: the ABI's own host-buffer path (taiga_coeffs.on_device = 0): the library copies the pinned nodal arrays to
+        # the device on its stream and waits for the copy before it returns
+        tg.load_field(grid, nodal_host if host else nodal_dev)                           # a1
         counts.zero_(); summary.zero_()
         off, spans = 0, []
         for g in cfg.groups:
@@ -321,10 +470,7 @@ def main_ours(args):
     ion_steps, n_ions = int(tsum[0]), int(tsum[1])
     t_trace = sum(a.elapsed_time(b) for a, b in trace_ms) / len(trace_ms)
     kind = grid.kind
-    alg = ALG_FP64_INSTR_PER_ION_STEP[kind]
-    if args.solver:                             # other solvers: field evaluations per step 4 (solver 1, 2) / 1 (Boris)
-        per_eval = (alg - 69.0) / 3.0
-        alg = {1: 4 * per_eval + 69.0, 2: 4 * per_eval + 75.0, 3: per_eval + 45.0, 4: per_eval + 45.0}[args.solver]
+    alg = alg_instr(kind, args.solver)
     achieved = ion_steps_rank * alg / (t_trace * 1e-3)
     traffic = ncu_traffic(args.config, not (args.ions or args.solver or args.opt or args.detector != "config" or world > 1 and args.scaling == "strong"))
     h2d = sum(p.numel() * 8 for p in nodal_pin) + (len(cd) + len(cn)) * 8 * len(cfg.groups) + 4 * (det0.nu + det0.nw) * 8
@@ -345,7 +491,8 @@ def main_ours(args):
                              "hits_in_segments": int(summary[:, 0].sum().item()), "hits_in_gaps_or_outside": int(summary[:, 1].sum().item())},
         "e2e": {"value": ion_steps * args.steps / (total_ms_e2e * 1e-3), "unit": "ion-steps/s",
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": total_ms_e2e / args.steps,
-                "timing": "host wall clock around the C-ABI calls incl. pinned H2D of the nodal field and D2H of the counters"},
+                "timing": "host wall clock around the C-ABI calls; taiga_load_field is given the pinned HOST arrays (on_device = 0: "
+                          "its own H2D + wait inside the call), CDF tables and detector edges are host pointers too, counters read back D2H"},
         "gpu_launches": launches_per_step(cfg, kind) * args.steps,
         "roofline": {"bound": "alu", "achieved": 2e-12 * achieved, "peak": 2e-12 * peak_dfma,
                      "unit": "TFLOP/s (FP64 pipe; every FP64 instruction counted as one FMA = 2 flop)",
@@ -376,6 +523,14 @@ def main_ours(args):
                            "alg_l1_bytes_per_ion_step": l1_bytes, "fp64_frac": achieved / peak_dfma,
                            "peak_source": "measured live: L1-resident 256-bit gather microkernel, all lanes of a warp in one cell "
                                           "(taiga_measure_l1_gather_peak, spread 1: 128 B/clk/SM; 64 with two cells per warp, 32 with four or more)"}
+    tg.close()
+    default_line = not (args.ions or args.solver or args.opt or args.detector != "config" or args.config != 2)
+    if world == 1 and (args.extras == "on" or (args.extras == "auto" and default_line)):
+        del ions, flush
+        torch.cuda.empty_cache()
+        out["configs"], out["variants"] = extras(local, peak_dfma, args.extras_ions)
+        out["extras"] = ("configs / variants: each the whole path a1-a5 at %s, 1 warm-up + 2 timed steps (CUDA events, L2 flush between), "
+                         "frac against the DFMA rate measured in this run" % ("full size" if not args.extras_ions else "%d ions per group" % args.extras_ions))
     if rank == 0:
         if world == 1:
             s, n, dt, cores, _ = oracle_run(args.config, args.oracle_sample, solver=args.solver)
@@ -387,7 +542,6 @@ def main_ours(args):
                                    "sample": "first %d ions of config %d (prefix sample, identical ions), whole path a1-a5, OpenMP over ions; "
                                              "value_1thread on the first %d ions" % (n, args.config, n1)}
         print(json.dumps(out))
-    tg.close()
     if world > 1:
         dist.destroy_process_group()
 

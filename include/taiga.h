@@ -11,8 +11,9 @@
  *  - All kernels are enqueued on the ctx's stream and the caller synchronises.  Exceptions:
  *    taiga_load_field / taiga_load_efield / taiga_load_loss wait for the upload of HOST input arrays (so that the
  *    caller may reuse them on return; device inputs are not synchronised, and every table is built on the device);
- *    taiga_trace synchronises at its end only while the "stats" option is on (default; it reads the counters back);
- *    taiga_field_table and the taiga_measure_* calls always do.  Small host tables (CDFs, detector edges) are staged
+ *    taiga_trace only enqueues (its counters reach the host when taiga_get_stats asks for them, which waits for the
+ *    stream; the "stats" option = 1 makes taiga_trace itself wait, off by default);
+ *    taiga_field_table and the taiga_measure_* calls always synchronise.  Small host tables (CDFs, detector edges) are staged
  *    through a pinned buffer of the ctx and never synchronise.
  *  - Coordinates: right-handed Cartesian (X,Y,Z), Z vertical, torus axis = Z,
  *    R = sqrt(X^2+Y^2); (R,phi,Z) right-handed; SI units.
@@ -274,8 +275,8 @@ int taiga_loss_statistics(const unsigned long long wsummary_host[4], double out_
  * 8 warps/SM in 32-thread CTAs (default); 4 predictive refill after each evaluation; 5 refill on demand only; 3 the
  * same at 12 warps/SM; 1 / 2 no cache at 8 / 16 warps/SM; 7 the same in 128-thread CTAs at 223 registers; time-sliced fields: 0 time-blended cell
  * cache in registers with the slice difference in per-lane shared-memory slots (default), 6 the same
- * with the difference gathered through L1, 4 slice cache with rolling refill), "stats" (1: read counters back,
- * default), "precision" (64 default; 32 = the fp32 variant of BASELINE config 5: kind-2 fields
+ * with the difference gathered through L1, 4 slice cache with rolling refill), "stats" (1: taiga_trace waits for its
+ * counters itself; default 0: taiga_get_stats does), "precision" (64 default; 32 = the fp32 variant of BASELINE config 5: kind-2 fields
  * with the RKN solver only, tricubic evaluation and its table in fp32, cell location and the ion
  * state in fp64; hit coordinates then agree with fp64 to 1e-5 m, integer outputs are not
  * bit-exact; taiga_trace returns TAIGA_E_ARG for other kinds / solvers), "plane_interp" (0 default:
@@ -292,7 +293,7 @@ int taiga_loss_statistics(const unsigned long long wsummary_host[4], double out_
  * CTA x register cap: 0 = 128 x 128, four CTAs per SM (default); 1 = 128 x 168; 2 = 64 x 144; 3 = 32 x 144; 4 = 32 x 128;
  * 5 = 64 x 128).  Values out of range are refused with TAIGA_E_ARG when set. */
 int taiga_set_option(taiga_ctx* ctx, const char* key, long long value);
-/* counters of the last taiga_trace (valid with "stats" on): [0] ion-steps, [1] warp-steps*32
+/* counters of the last taiga_trace; waits for the ctx's stream when that trace has not been collected yet: [0] ion-steps, [1] warp-steps*32
  * (lane slots issued), [2] 1, [3] kernel launches, [4] cell refills, [5..7] 0. */
 int taiga_get_stats(taiga_ctx* ctx, unsigned long long stats_host[8]);
 /* register-resident DFMA microkernel: measured FP64 FMA instructions per second (thread-level,

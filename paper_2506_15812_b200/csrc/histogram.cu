@@ -139,28 +139,84 @@ int tg_histogram(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* d
 // ------------------------------------------------------------------------------------------
 // Weighted counters: q = floor(w 2^32 + 1/2) per plane-crossing ion, 64-bit
 // integer atomics, so the sums do not depend on the order of accumulation.
-__global__ void k_histogram_weighted(const int32_t* __restrict__ cell, const double* __restrict__ weight,
-                                     const uint16_t* __restrict__ group, uint32_t n, int n_hist, int ncell,
-                                     unsigned long long* __restrict__ wcounts, unsigned long long* __restrict__ wsummary) {
-    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    int g = group ? (int)group[i] : 0, c = cell[i];
-    if (g >= n_hist || c < TAIGA_CELL_MISS) return;
-    double wv = weight[i];
-    if (!(wv >= 0.0)) wv = 0.0;                // negative / NaN weights count as 0
-    if (wv > 1048576.0) wv = 1048576.0;        // keeps q < 2^52 (weights are <= 1 for this method)
-    unsigned long long q = (unsigned long long)floor(fma(wv, 4294967296.0, 0.5));
-    if (c >= 0) { atomicAdd(&wcounts[(size_t)g * ncell + c], q); atomicAdd(&wsummary[g * 4 + 0], q); }
-    else atomicAdd(&wsummary[g * 4 + 1], q);
-    atomicAdd(&wsummary[g * 4 + 2], __umul64hi(q, q) << 32 | (q * q) >> 32);
-    atomicAdd(&wsummary[g * 4 + 3], 1ull);
+// Per-segment sums: block-private shared counters flushed once when the matrix fits (<= 4096 x 8 B), else one global
+// atomic per ion (distinct addresses for the most part).  The four summary sums of a histogram, which every crossing ion
+// of the grid used to add to the same three addresses, are reduced over the warp first when its ions belong to one
+// histogram (the rule: groups are contiguous runs of ions), so a warp issues at most four atomics on them.
+#define WHIST_SMEM_BINS 4096
+
+__device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v) {
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+template <bool SMEM>
+__global__ void __launch_bounds__(256) k_histogram_weighted(const int32_t* __restrict__ cell, const double* __restrict__ weight,
+                                                            const uint16_t* __restrict__ group, uint32_t n, int n_hist, int ncell,
+                                                            unsigned long long* __restrict__ wcounts, unsigned long long* __restrict__ wsummary) {
+    __shared__ unsigned long long sh[SMEM ? WHIST_SMEM_BINS : 1];
+    const int nbins = n_hist * ncell;
+    if (SMEM) {
+        for (int b = threadIdx.x; b < nbins; b += blockDim.x) sh[b] = 0ull;
+        __syncthreads();
+    }
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    int g = -1, c = TAIGA_CELL_MISS;
+    unsigned long long q = 0ull;
+    if (i < n) {
+        const int gi = group ? (int)group[i] : 0;
+        c = cell[i];
+        if (gi < n_hist && c >= TAIGA_CELL_MISS) {
+            g = gi;
+            double wv = weight[i];
+            if (!(wv >= 0.0)) wv = 0.0;                // negative / NaN weights count as 0
+            if (wv > 1048576.0) wv = 1048576.0;        // keeps q < 2^52 (weights are <= 1 for this method)
+            q = (unsigned long long)floor(fma(wv, 4294967296.0, 0.5));
+        }
+    }
+    const bool crosser = g >= 0;
+    if (crosser && c >= 0) {
+        if (SMEM) atomicAdd(&sh[g * ncell + c], q);
+        else atomicAdd(&wcounts[(size_t)g * ncell + c], q);
+    }
+    const unsigned long long q_in = (crosser && c >= 0) ? q : 0ull, q_out = (crosser && c < 0) ? q : 0ull;
+    const unsigned long long q2 = crosser ? (__umul64hi(q, q) << 32 | (q * q) >> 32) : 0ull;
+    const unsigned FULL = 0xffffffffu;
+    const unsigned act = __ballot_sync(FULL, crosser);
+    const int gmin = __reduce_min_sync(FULL, crosser ? g : 0x7fffffff), gmax = __reduce_max_sync(FULL, crosser ? g : -1);
+    if (act && gmin == gmax) {                         // one histogram in this warp: reduce, then four atomics
+        const unsigned long long s_in = warp_sum_u64(q_in), s_out = warp_sum_u64(q_out), s2 = warp_sum_u64(q2);
+        if ((threadIdx.x & 31) == 0) {
+            unsigned long long* ws = wsummary + (size_t)gmin * 4;
+            if (s_in) atomicAdd(ws + 0, s_in);
+            if (s_out) atomicAdd(ws + 1, s_out);
+            if (s2) atomicAdd(ws + 2, s2);
+            atomicAdd(ws + 3, (unsigned long long)__popc(act));
+        }
+    } else if (crosser) {                              // a warp across a group border, or interleaved groups
+        unsigned long long* ws = wsummary + (size_t)g * 4;
+        atomicAdd(ws + (c >= 0 ? 0 : 1), q);
+        atomicAdd(ws + 2, q2);
+        atomicAdd(ws + 3, 1ull);
+    }
+    if (SMEM) {
+        __syncthreads();
+        for (int b = threadIdx.x; b < nbins; b += blockDim.x) {
+            const unsigned long long v = sh[b];
+            if (v) atomicAdd(&wcounts[b], v);
+        }
+    }
 }
 
 int tg_histogram_weighted(taiga_ctx* ctx, const taiga_ions* ions, const taiga_detector* det, int n_hist,
                           unsigned long long* wcounts, unsigned long long* wsummary) {
-    uint32_t n = (uint32_t)ions->n;
-    k_histogram_weighted<<<(n + 255) / 256, 256, 0, ctx->stream>>>(ions->cell, ions->weight ? ions->weight : ions->w0, ions->group, n, n_hist,
-                                                                   det->nu * det->nw, wcounts, wsummary);
+    const uint32_t n = (uint32_t)ions->n;
+    const int ncell = det->nu * det->nw;
+    const double* wt = ions->weight ? ions->weight : ions->w0;
+    if ((long long)n_hist * ncell <= WHIST_SMEM_BINS)
+        k_histogram_weighted<true><<<(n + 255) / 256, 256, 0, ctx->stream>>>(ions->cell, wt, ions->group, n, n_hist, ncell, wcounts, wsummary);
+    else
+        k_histogram_weighted<false><<<(n + 255) / 256, 256, 0, ctx->stream>>>(ions->cell, wt, ions->group, n, n_hist, ncell, wcounts, wsummary);
     TG_CUDA(ctx, cudaGetLastError());
     return TAIGA_OK;
 }

@@ -42,7 +42,7 @@ extern "C" int taiga_create(taiga_ctx** out, int device, void* cuda_stream) {
     }
     ctx->opt_sort = 1; ctx->opt_sort_sub = 16;
     ctx->opt_min_active = 32;
-    ctx->opt_ctas_per_sm = 0; ctx->opt_variant = 0; ctx->opt_stats = 1; ctx->opt_precision = 64; ctx->opt_plane_interp = 0; ctx->opt_regroup = 8;
+    ctx->opt_ctas_per_sm = 0; ctx->opt_variant = 0; ctx->opt_stats = 0; ctx->opt_precision = 64; ctx->opt_plane_interp = 0; ctx->opt_regroup = 8;
     ctx->opt_mma = -1; ctx->opt_refill_cta = 0;
     strcpy(ctx->err, "ok");
     *out = ctx;
@@ -288,6 +288,11 @@ extern "C" int taiga_set_option(taiga_ctx* ctx, const char* key, long long v) {
 
 extern "C" int taiga_get_stats(taiga_ctx* ctx, unsigned long long out[8]) {
     if (!ctx || !out) return TAIGA_E_ARG;
+    if (ctx->stats_pending) {                   // the one place the trace path waits for the device
+        TG_CUDA(ctx, cudaSetDevice(ctx->device));
+        int rc = tg_collect_stats(ctx);
+        if (rc) return rc;
+    }
     for (int i = 0; i < 8; ++i) out[i] = ctx->stats[i];
     return TAIGA_OK;
 }

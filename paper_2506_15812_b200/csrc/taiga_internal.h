@@ -76,6 +76,7 @@ struct taiga_ctx {
     unsigned long long* counters;                        // device counters (16)
     unsigned long long* counters_host;                   // pinned mirror
     unsigned long long stats[8];
+    bool stats_pending;  int stats_launches;             // the last trace's counters are on their way to counters_host
 
     // options
     int opt_sort, opt_min_active, opt_ctas_per_sm, opt_variant, opt_stats;
@@ -130,6 +131,7 @@ int tg_seed(taiga_ctx* ctx, const taiga_beam_params* p, uint64_t seed, taiga_ion
 int tg_build_order(taiga_ctx* ctx, const taiga_ions* ions);      // queue_sort.cu: fills ctx->order
 int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t max_steps,
              const DetDev& det, int variant);
+int tg_collect_stats(taiga_ctx* ctx);                            // trace.cu: waits for the stream, fills ctx->stats
 struct TraceParams;
 int tg_trace_mma(taiga_ctx* ctx, TraceParams& P, int solver, bool hasE, bool loss, bool bez, uint64_t n);   // trace_mma.cu
 bool tg_mma_supported(const taiga_ctx* ctx);

@@ -31,6 +31,19 @@ static const TgVariant tg_variants_a[] = {
 
 const TgVariant* tg_trace_variants_b(int* n);       // trace_variants.cu
 
+int tg_collect_stats(taiga_ctx* ctx) {
+    if (!ctx->stats_pending) return TAIGA_OK;
+    TG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->stats[0] = ctx->counters_host[3];
+    ctx->stats[1] = ctx->counters_host[1] * 32ull;
+    ctx->stats[2] = 1;
+    ctx->stats[3] = (unsigned long long)ctx->stats_launches;
+    ctx->stats[4] = ctx->counters_host[2];
+    ctx->stats[5] = 0;
+    ctx->stats_pending = false;
+    return TAIGA_OK;
+}
+
 int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t max_steps, const DetDev& det, int variant) {
     cudaStream_t st = ctx->stream;
     const int kind = ctx->field.kind;
@@ -175,15 +188,11 @@ int tg_trace(taiga_ctx* ctx, taiga_ions* ions, double qm, double dt, uint32_t ma
         }
         ctx->n_wranges = m;
     }
-    if (ctx->opt_stats) {
-        TG_CUDA(ctx, cudaMemcpyAsync(ctx->counters_host, ctx->counters, 8 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
-        TG_CUDA(ctx, cudaStreamSynchronize(st));
-        ctx->stats[0] = ctx->counters_host[3];
-        ctx->stats[1] = ctx->counters_host[1] * 32ull;
-        ctx->stats[2] = 1;
-        ctx->stats[3] = (unsigned long long)launches;
-        ctx->stats[4] = ctx->counters_host[2];
-        ctx->stats[5] = 0;
-    }
+    // counters of this trace: copied to the pinned mirror in stream order; taiga_get_stats waits for the stream and reads
+    // them ("stats" = 1: wait here, as the library did before round 3)
+    TG_CUDA(ctx, cudaMemcpyAsync(ctx->counters_host, ctx->counters, 8 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    ctx->stats_launches = launches;
+    ctx->stats_pending = true;
+    if (ctx->opt_stats) return tg_collect_stats(ctx);
     return TAIGA_OK;
 }

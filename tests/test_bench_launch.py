@@ -71,3 +71,29 @@ def test_bench_line_carries_the_contract_keys():
     assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["value_1thread"] > 0 and "sample" in c
     assert line["gpu_launches"] == 14 * line["steps"]
     assert line["value"] * line["ms_per_step"] * 1e-3 == pytest.approx(line["config"]["ion_steps_per_step"], rel=1e-6)
+
+
+@pytest.mark.gpu
+def test_bench_line_reports_every_config_and_the_variant_kernels():
+    """`configs` (BASELINE configs 1, 3, 4, 5) and `variants` (loss, Bezier, uniform / gridded E, RK4, Boris on config 2,
+    fp32 on config 5) ride in the same JSON line (report per config); here at 4,096 ions per group."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--ions", "8192", "--steps", "2", "--warmup", "3", "--oracle-sample", "512",
+                          "--extras", "on", "--extras-ions", "4096"], capture_output=True, text=True, timeout=900)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    assert sorted(line["configs"]) == ["1", "3", "4", "5"] and len(line["variants"]) == 7
+    for name, c in list(line["configs"].items()) + list(line["variants"].items()):
+        for k in ("workload", "ms_per_step", "trace_kernel", "ion_steps_per_s", "ions_per_s", "trace_ion_steps_per_s", "clocks"):
+            assert k in c, (name, k)
+        assert c["invariant_counts_sum_to_n"] is True, name
+        assert 0.0 < c["trace_kernel"]["ms"] <= c["ms_per_step"] and c["ion_steps_per_step"] > 0, name
+        assert c["summary"][0] > 0, name                            # ions reach the detector in every case
+    for name, c in line["configs"].items():
+        assert 0.0 < c["frac"] < 1.0 and c["frac_nominal"] > 0.0, name
+    assert line["configs"]["5"]["trace_kernel"]["kernel"] == "k_trace_mma" and line["configs"]["4"]["trace_kernel"]["kernel"] == "k_trace"
+    assert len(line["configs"]["3"]["groups"]) == 4 and line["configs"]["3"]["trace_kernel"]["launches"] == 4
+    assert "weighted_histogram_ms" in line["variants"]["cfg2 loss (Eq. 2) + weighted counters"]
+    assert line["roofline"]["traffic"] is None                      # --ions: not the configuration of the ncu capture
