@@ -278,7 +278,7 @@ int taiga_loss_statistics(const unsigned long long wsummary_host[4], double out_
  * with the difference gathered through L1, 4 slice cache with rolling refill), "stats" (1: taiga_trace waits for its
  * counters itself; default 0: taiga_get_stats does), "precision" (64 default; 32 = the fp32 variant of BASELINE config 5: kind-2 fields
  * with the RKN solver only, tricubic evaluation and its table in fp32, cell location and the ion
- * state in fp64; hit coordinates then agree with fp64 to 1e-5 m, integer outputs are not
+ * state in fp64; offered for that accuracy statement, not for speed: it is slower than fp64 on the cooperative tracer (8.5 s against 6.7 s on BASELINE config 5); hit coordinates then agree with fp64 to 1e-5 m, integer outputs are not
  * bit-exact; taiga_trace returns TAIGA_E_ARG for other kinds / solvers), "plane_interp" (0 default:
  * linear interpolation to the detector plane; 1: quadratic Bezier through r_n, r_n+1 with the
  * control point at the mean of r_n + v_n dt/2 and r_n+1 - v_n+1 dt/2, reading Z1;
